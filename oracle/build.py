@@ -1,0 +1,28 @@
+"""Build the CPU oracle's shared object (gcc -O2 -fopenmp, no -ffast-math).
+
+TEST INFRASTRUCTURE: see ck_oracle.h.  `python -m oracle.build` or oracle.build.build().
+"""
+from __future__ import annotations
+
+import os
+import subprocess
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SRC = os.path.join(HERE, "ck_oracle.c")
+HDR = os.path.join(HERE, "ck_oracle.h")
+LIB = os.path.join(HERE, "libck_oracle.so")
+
+
+def build(force: bool = False) -> str:
+    newest = max(os.path.getmtime(SRC), os.path.getmtime(HDR))
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
+        return LIB
+    cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra",
+           "-o", LIB + ".tmp", SRC, "-lm"]
+    subprocess.run(cmd, check=True, cwd=HERE)
+    os.replace(LIB + ".tmp", LIB)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force=True))

@@ -1,0 +1,70 @@
+/* ck_oracle.h -- CPU oracle for the batched chemical source term.  TEST INFRASTRUCTURE.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+ * legs may use anything under oracle/.  It shares no code, header or table with the CUDA
+ * library (paper_2008_08483_b200/, include/ck.h) and neither includes the other.
+ *
+ * What it computes: the plain definition of the source term in the classic rate-law
+ * (product) form, one cell and one reaction at a time, in fp64:
+ *   Eq. 1-3   mechanism, species production, law of mass action
+ *   Eq. 5   Arrhenius forward rate constant
+ *   Eq. 7-8   reverse constant through the equilibrium constant
+ *   NASA-7 h, s, cp polynomials with a cutoff temperature
+ *   Sec. 2.4 third bodies, falloff, irreversible reactions
+ * plus the pieces the paper implies but does not print:
+ * concentrations from (T, P, Y), textbook Lindemann / Troe falloff, and the
+ * constant-pressure energy equation dT/dt = -sum_k h_k wdot_k / (rho cp).
+ *
+ * Pins: tests/test_oracle_*.py (closed forms computed at 50 digits, conservation of
+ * mass and elements, detailed balance at a constructed equilibrium, thermodynamic
+ * identities by finite differences, falloff limits, and a numpy restatement of the
+ * paper's matrix equations 2, 4, 6, 10, 11).  Troe's constants and the Troe blending
+ * function are pinned only by the 50-digit closed form and its limits -- no external
+ * code (Cantera) is available: "parity unpinned" against third-party software.
+ */
+#ifndef CK_ORACLE_H
+#define CK_ORACLE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ck_oracle_mech {
+  int32_t S, R;
+  const double *W;          /* [S] kg/kmol */
+  const double *nu_reac;    /* [S*R] nu'_kj  at k*R+j */
+  const double *nu_prod;    /* [S*R] nu''_kj */
+  const double *ln_A;       /* [R] */
+  const double *b;          /* [R] */
+  const double *Ea_over_R;  /* [R] K */
+  const uint8_t *reversible;/* [R] */
+  const double *nasa_lo;    /* [S*7] a1..a7, T <= T_mid */
+  const double *nasa_hi;    /* [S*7] a1..a7, T >  T_mid */
+  const double *T_mid;      /* [S] */
+  const uint8_t *rxn_type;  /* [R] 0 elementary, 1 three-body, 2 Lindemann, 3 Troe */
+  const double *eff;        /* [S*R] E_kj */
+  const double *ln_A0, *b0, *Ea0_over_R; /* [R] low-pressure limit */
+  const double *troe;       /* [R*4] alpha, T***, T*, T** */
+  double p_ref;             /* Pa */
+} ck_oracle_mech;
+
+/* wdot[S][N] (kmol/m^3/s) and dTdt[N] (K/s) from T[N] (K), P[N] (Pa), Y[S][N].
+ * nthreads <= 0 -> all OpenMP threads.  Returns the number of threads used. */
+int ck_oracle_source_terms(const ck_oracle_mech *m, const double *T, const double *P,
+                           const double *Y, int64_t N, double *wdot, double *dTdt,
+                           int nthreads);
+
+/* Every intermediate of one cell, for the pins.  Y has stride ldY between species.
+ * Any output pointer may be NULL.  Sizes: per-species [S], per-reaction [R]. */
+void ck_oracle_cell_detail(const ck_oracle_mech *m, double T, double P, const double *Y,
+                           int64_t ldY, double *rho, double *cp_mass,
+                           double *C, double *cp_R, double *h_RT, double *s_R, double *g_RT,
+                           double *kf, double *Kc, double *kr, double *M, double *qf,
+                           double *qr, double *Q, double *wdot, double *dTdt);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

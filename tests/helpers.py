@@ -1,0 +1,120 @@
+"""Shared test helpers: the north_star parity tolerance and a numpy restatement of the
+paper's matrix equations (a second, independent derivation used to pin the oracle)."""
+import numpy as np
+
+RU = 8314.46261815324  # J/(kmol K)
+
+
+def parity_violations(wdot, dTdt, wdot_ref, dTdt_ref):
+    """north_star tolerance (BASELINE.json):
+       |d wdot_k| <= 1e-10 * max_k |wdot_k| + 1e-12 * |wdot_k|   per cell
+       |d dT/dt|  <= 1e-10 * |dT/dt| + 1e-12 K/s
+    Returns (worst wdot ratio err/tol, worst dTdt ratio err/tol); both must be <= 1."""
+    wmax = np.abs(wdot_ref).max(axis=0, keepdims=True)
+    tol_w = 1e-10 * wmax + 1e-12 * np.abs(wdot_ref)
+    err_w = np.abs(wdot - wdot_ref)
+    tol_t = 1e-10 * np.abs(dTdt_ref) + 1e-12
+    err_t = np.abs(dTdt - dTdt_ref)
+    # tol_w can be 0 only if the whole reference column is 0; then err must be 0 too
+    rw = np.where(tol_w > 0, err_w / np.where(tol_w > 0, tol_w, 1.0), np.where(err_w > 0, np.inf, 0.0))
+    rt = err_t / tol_t
+    if not (np.isfinite(wdot).all() and np.isfinite(dTdt).all()):
+        return np.inf, np.inf
+    return float(rw.max()) if rw.size else 0.0, float(rt.max()) if rt.size else 0.0
+
+
+def energy_condition_number(mech, T, wdot_ref, h_RT):
+    """kappa = sum|h_k wdot_k| / |sum h_k wdot_k| per cell."""
+    hw = h_RT * RU * T[None, :] * wdot_ref
+    return np.abs(hw).sum(0) / np.maximum(np.abs(hw.sum(0)), 1e-300)
+
+
+def paper_matrix_form(mech, T, P, Y):
+    """Literal numpy evaluation of the paper's ANN-form equations, dense matrices,
+    batch dimension leading.  Returns (Omega[N,S], dTdt[N]).
+
+    Eq. 6    log Kf = X_f W_f + B_f
+    Eq. 10  G = X_G W_G + B_G, alpha from NASA-7 by range
+    Eq. 11  log Kc = -(G - log(p_ref/(Ru T))) nu
+    Sec 2.4 log M added to log Kf, M = C E; falloff non-matrix
+    Eq. 4       Q_net = exp(log C nu' + log Kf) - exp(log C nu'' + log Kr)
+    Eq. 2    Omega = Q_net nu^T
+    """
+    S, R = mech.n_species, mech.n_reactions
+    T = np.asarray(T, dtype=np.float64)
+    N = T.shape[0]
+    Yc = np.ascontiguousarray(Y.T)                      # [N, S]
+    W = mech.mol_weight
+    nu1, nu2 = mech.nu_reac, mech.nu_prod               # [S, R]
+    nu = nu2 - nu1
+
+    # concentrations
+    Wmix = 1.0 / (Yc / W).sum(1)
+    rho = P * Wmix / (RU * T)
+    C = np.maximum(rho[:, None] * Yc / W, 1e-300)       # [N, S]
+    logC = np.log(C)
+
+    # Eq. 6
+    X_f = np.stack([np.log(T), 1.0 / T], axis=1)        # [N, 2]
+    W_f = np.stack([mech.b, -mech.Ea_over_R], axis=0)   # [2, R]
+    logKf = X_f @ W_f + mech.ln_A[None, :]
+
+    # Eq. 10: alpha (7 x S) per temperature range, g/RT = h/RT - s/R collected on X_G
+    X_G = np.stack([np.log(T), T, T**2, T**3, T**4, 1.0 / T], axis=1)     # [N, 6]
+
+    def alpha(a):                                       # a: [S, 7] NASA a1..a7
+        Wg = np.stack([-a[:, 0], -a[:, 1] / 2, -a[:, 2] / 6, -a[:, 3] / 12, -a[:, 4] / 20,
+                       a[:, 5]], axis=0)                # [6, S]
+        Bg = a[:, 0] - a[:, 6]                          # [S]
+        return Wg, Bg
+
+    Wg_lo, Bg_lo = alpha(mech.nasa_lo)
+    Wg_hi, Bg_hi = alpha(mech.nasa_hi)
+    low = T[:, None] <= mech.T_mid[None, :]             # [N, S]
+    G = np.where(low, X_G @ Wg_lo + Bg_lo, X_G @ Wg_hi + Bg_hi)
+
+    # Eq. 11 with the standard-concentration term in the bias
+    logKc = -(G - np.log(mech.p_ref / (RU * T))[:, None]) @ nu            # [N, R]
+
+    # Sec. 2.4: third bodies and falloff
+    tb = mech.rxn_type == 1
+    fo = (mech.rxn_type == 2) | (mech.rxn_type == 3)
+    M = C @ mech.eff                                     # [N, R]
+    logKf = logKf + np.where(tb[None, :], np.log(M), 0.0)
+    if fo.any():
+        W_0 = np.stack([mech.b0, -mech.Ea0_over_R], axis=0)
+        logK0 = X_f @ W_0 + mech.ln_A0[None, :]
+        Pr = np.exp(logK0 - logKf) * M
+        al, T3, T1, T2 = (mech.troe[:, i][None, :] for i in range(4))
+        with np.errstate(divide="ignore", invalid="ignore"):
+            Fc = (1 - al) * np.exp(-T[:, None] / T3) + al * np.exp(-T[:, None] / T1) \
+                + np.exp(-T2 / T[:, None])
+            lFc = np.log10(Fc)
+            c = -0.4 - 0.67 * lFc
+            n = 0.75 - 1.27 * lFc
+            lPr = np.log10(np.maximum(Pr, 1e-300))
+            f1 = (lPr + c) / (n - 0.14 * (lPr + c))
+            logF = np.log(10.0) * lFc / (1 + f1 * f1)
+        logF = np.where((mech.rxn_type == 3)[None, :], logF, 0.0)
+        logKf = np.where(fo[None, :], logKf + np.log(Pr / (1 + Pr)) + logF, logKf)
+    logKr = logKf - logKc                                # Eq. 7 in log space
+
+    # Eq. 4 and Eq. 2
+    Qf = np.exp(logC @ nu1 + logKf)
+    Qr = np.exp(logC @ nu2 + logKr) * mech.reversible[None, :]
+    Omega = (Qf - Qr) @ nu.T                             # [N, S]
+
+    # energy equation (north_star step 6)
+    def cp_h(a):
+        cp = a[:, 0] + X_G[:, 1:2] * a[:, 1] + X_G[:, 2:3] * a[:, 2] + X_G[:, 3:4] * a[:, 3] \
+            + X_G[:, 4:5] * a[:, 4]
+        h = a[:, 0] + X_G[:, 1:2] * a[:, 1] / 2 + X_G[:, 2:3] * a[:, 2] / 3 \
+            + X_G[:, 3:4] * a[:, 3] / 4 + X_G[:, 4:5] * a[:, 4] / 5 + X_G[:, 5:6] * a[:, 5]
+        return cp, h
+    cp_lo, h_lo = cp_h(mech.nasa_lo)
+    cp_hi, h_hi = cp_h(mech.nasa_hi)
+    cp_R = np.where(low, cp_lo, cp_hi)
+    h_RT = np.where(low, h_lo, h_hi)
+    cp_mass = (Yc * cp_R * RU / W).sum(1)
+    dTdt = -(h_RT * RU * T[:, None] * Omega).sum(1) / (rho * cp_mass)
+    return Omega, dTdt
