@@ -1,0 +1,303 @@
+#!/usr/bin/env python
+"""bench.py -- cell source-term evaluations per second (fp64) and fraction of roofline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload mid_1m|tiny_1m|large_256k|...]
+
+A "step" is one pass of the whole hot path (ck_source_terms: every layer of the paper's
+ANN form, include/ck.h (1)-(6)) over one batch of seeded synthetic cells.  The default
+workload is the one BASELINE.json's metric is quoted on: S=53, R=325, N=2^20 cells, fp64.
+Prints ONE JSON line (rank 0).  N>1: launched by torchrun, one process per GPU, cells
+sharded across ranks with no collective (weak scaling: N cells per GPU).
+
+--impl reference times the CPU oracle (oracle/, test infrastructure) on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "cell source-term evals/sec (fp64) at S=53,R=325; fraction of roofline"
+UNIT = "cells/s"
+
+
+def algorithmic_fp64_instr_per_cell(info):
+    """SURVEY.md section 8(d) / DESIGN.md: algorithmic FP64-pipe instructions per cell
+    (FMA, add, mul = 1; exp = 15, log = 28, div = 8 by CUDA 12.9's sm_100a fast paths)."""
+    S, R = info["S"], info["R"]
+    n_fo = info["n_lindemann"] + info["n_troe"]
+    n_exp = 2 * R + 5 * info["n_troe"] + info["n_lindemann"]
+    n_log = S + 1 + 2 * n_fo
+    n_div = 3 + 3 * n_fo
+    fma = 20 * S + 2 * (R + n_fo) + info["nnz_reac"] + 2 * info["nnz_net"] + info["nnz_eff"]
+    return fma + 15 * n_exp + 28 * n_log + 8 * n_div
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _loop(self):
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "hw_thermal_slowdown": 0x40,
+                 "sw_thermal_slowdown": 0x20, "hw_power_brake_slowdown": 0x80,
+                 "sync_boost": 0x10, "applications_clocks_setting": 0x2}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for n, bit in names.items():
+                    if mask & bit:
+                        self.reasons.add(n)
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thread = threading.Thread(target=self._loop, daemon=True)
+            self._thread.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thread:
+            self._thread.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def time_oracle(mech, T, P, Y, target_s=15.0):
+    """Oracle as it stands on a bounded sample: grow the sample until ~target_s of work."""
+    import oracle
+    om = oracle.OracleMechanism(mech)
+    n = min(4096, T.shape[0])
+    t0 = time.perf_counter()
+    _, _, cores = oracle.source_terms(om, T[:n], P[:n], np.ascontiguousarray(Y[:, :n]))
+    rate = n / max(time.perf_counter() - t0, 1e-9)
+    n = int(min(T.shape[0], max(n, rate * target_s)))
+    t0 = time.perf_counter()
+    oracle.source_terms(om, T[:n], P[:n], np.ascontiguousarray(Y[:, :n]))
+    dt = time.perf_counter() - t0
+    return {"value": n / dt, "unit": UNIT, "cores": int(cores), "kind": "oracle",
+            "sample": "first %d cells of the workload, %.1f s, OpenMP static over cells" % (n, dt)}
+
+
+def run_reference(args, cfg, mech):
+    """--impl reference: the CPU oracle on the host cores, rank 0 only."""
+    import ckgen
+    import oracle
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    n = min(cfg.N, args.ref_cells)
+    T, P, Y = ckgen.states(cfg, N=n)
+    om = oracle.OracleMechanism(mech)
+    cores = 0
+    for _ in range(args.warmup):
+        _, _, cores = oracle.source_terms(om, T[:4096], P[:4096], np.ascontiguousarray(Y[:, :4096]))
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        _, _, cores = oracle.source_terms(om, T, P, Y)
+    dt = time.perf_counter() - t0
+    value = n * args.steps / dt
+    sample = "each step = first %d cells of the workload (oracle, OpenMP static)" % n
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": workload_config(cfg, mech, n),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": int(cores), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def workload_config(cfg, mech, n_per_gpu):
+    S, R = mech.n_species, mech.n_reactions
+    step_mb = 8 * (2 * S + 3) * n_per_gpu / 1e6
+    return {"workload": "%s: S=%d R=%d N=%d cells per GPU, fp64 SoA T[N] P[N] Y[S][N], seeded "
+                        "synthetic mechanism + states (ckgen)" % (cfg.name, S, R, n_per_gpu),
+            "S": S, "R": R, "cells_per_gpu": int(n_per_gpu),
+            "l2": "no flush: %.0f MB of state in+out per step vs 126 MB L2" % step_mb
+                  if step_mb > 126 else "state (%.1f MB per step) is L2 resident" % step_mb}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="mid_1m")
+    ap.add_argument("--cells", type=int, default=0, help="override cells per GPU")
+    ap.add_argument("--ref-cells", type=int, default=65536, help="cells per step of --impl reference")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+
+    import ckgen
+    cfg = ckgen.CONFIGS[args.workload]
+    mech = ckgen.mechanism(cfg.mech)
+    if args.impl == "reference":
+        run_reference(args, cfg, mech)
+        return
+
+    import torch
+    import paper_2008_08483_b200 as ck
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    N = args.cells or cfg.N
+    S = mech.n_species
+    # each rank owns its own cells (cells are independent): no collective
+    T, P, Y = ckgen.states(cfg, N=N, seed_offset=rank)
+    gm = ck.Mechanism(mech)
+    info = {k: gm.info(k) for k in ck.INFO}
+    stream = torch.cuda.current_stream().cuda_stream
+    Td, Pd, Yd = (torch.from_numpy(a).to(dev) for a in (T, P, Y))
+    w = torch.empty((S, N), dtype=torch.float64, device=dev)
+    d = torch.empty(N, dtype=torch.float64, device=dev)
+
+    fp64_fma_per_s = ck.ck_measure_fp64_peak(stream)
+
+    for _ in range(args.warmup):
+        gm.source_terms(Td, Pd, Yd, w, d, stream=stream)
+    barrier()
+
+    # ---- timed region: K steps, device-resident inputs, CUDA events on the launch stream
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    with ClockSampler(local_rank) as clocks:
+        barrier()
+        ev[0].record()
+        for s in range(args.steps):
+            gm.source_terms(Td, Pd, Yd, w, d, stream=stream)
+            ev[s + 1].record()
+        barrier()
+    total_ms = ev[0].elapsed_time(ev[-1])
+    step_ms = [ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps)]
+    kernel_ms = float(np.mean(step_ms))          # one kernel launch per step
+    if dist is not None:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    value = world * N * args.steps / (total_ms * 1e-3)
+
+    # ---- end to end through the public host entry point (pinned host buffers) ---------
+    Th, Ph, Yh = (torch.from_numpy(a).pin_memory() for a in (T, P, Y))
+    wh = torch.empty((S, N), dtype=torch.float64).pin_memory()
+    dh = torch.empty(N, dtype=torch.float64).pin_memory()
+    e2e_steps = max(3, min(args.steps, 10))
+    gm.source_terms_host(Th, Ph, Yh, wh, dh, stream=stream)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        gm.source_terms_host(Th, Ph, Yh, wh, dh, stream=stream)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_value = world * N * e2e_steps / e2e_s
+    assert np.array_equal(dh.numpy(), d.cpu().numpy()), "host and device entry points disagree"
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the (single) kernel: FP64-pipe bound -------------------
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    i_cell = algorithmic_fp64_instr_per_cell(info)
+    achieved_tflops = 2.0 * i_cell * N / (kernel_ms * 1e-3) / 1e12
+    peak_tflops = 2.0 * fp64_fma_per_s / 1e12
+    hbm_bytes = 8.0 * (2 * S + 3) * N
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    traffic = None
+    try:
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(cfg.name)
+    except Exception:
+        pass
+    roofline = {
+        "bound": "alu", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
+        "frac": achieved_tflops / peak_tflops, "traffic": traffic,
+        "kernel": "ck::source_terms_kernel", "kernel_ms": kernel_ms,
+        "fp64_instr_per_cell": i_cell,
+        "peak_source": "DFMA microbenchmark run by this bench (ck_measure_fp64_peak), x2 flop/FMA; "
+                       "nominal 148 SM x 64 lanes x 2 x sm_max_mhz = %.1f TFLOP/s"
+                       % (148 * 64 * 2 * (clocks.max_mhz or 1965.0) * 1e6 / 1e12),
+        "hbm": {"achieved": hbm_bytes / (kernel_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                "frac": hbm_bytes / (kernel_ms * 1e-3) / 1e9 / hbm_peak,
+                "peak_source": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6650 GB/s"},
+    }
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(cfg, mech, N),
+        "clocks": clocks.summary(),
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(8 * (S + 2) * N),
+                "d2h_bytes_per_step": int(8 * (S + 1) * N), "steps": e2e_steps},
+        "gpu_launches": int(args.steps * info["launches_per_call"]),
+        "roofline": roofline,
+        "launch": {"threads": info["threads"], "blocks_per_sm": info["blocks_per_sm"],
+                   "smem_bytes": info["smem_bytes"]},
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = time_oracle(mech, T, P, Y)
+    print(json.dumps(out))
+    gm.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,125 @@
+/* ck.h -- C ABI of the B200-native batched chemical source-term library.
+ *
+ * The library evaluates, for N independent reacting cells, the paper's ANN-form source
+ * term (Barwey & Raman, arXiv 2008.08483; line numbers are /root/reference/PAPER.md):
+ *
+ *   (1) Arrhenius layer      ln k_f = [ln A, b, -Ea/R] . [1, ln T, 1/T]        Eq. 5-6, l.72-83
+ *   (2) NASA-7 thermo layer  g/RT, h/RT, cp/R from X_G = [ln T, T..T^4, 1/T]   Eq. 10,  l.101-108
+ *   (3) equilibrium layer    ln Kc = -nu^T (g/RT - ln(p_ref/(Ru T)))           Eq. 8-11, l.93-114
+ *                            ln k_r = ln k_f - ln Kc                           Eq. 7,   l.87-91
+ *   (4) third bodies M = C E, Lindemann / Troe falloff                         Sec. 2.4, l.157-159
+ *   (5) log-rate layers      q_f = exp(nu'^T ln C + ln k_f),
+ *                            q_r = exp(nu''^T ln C + ln k_r)                   Eq. 4,   l.58
+ *   (6) net-rate contraction wdot = (nu'' - nu') (q_f - q_r)                   Eq. 2,   l.49-51
+ *       energy term          dT/dt = -sum_k h_k wdot_k / (rho cp)              l.185 (const.-P reactor)
+ *
+ * Every step runs in hand-written CUDA kernels for sm_100a; there is no CPU fallback.
+ * Units are SI-kmol: T [K], P [Pa], W [kg/kmol], C [kmol/m^3], wdot [kmol/m^3/s],
+ * Ru = 8314.46261815324 J/(kmol K).  All floating point is IEEE fp64.
+ *
+ * Error behaviour: every function returns CK_OK (0) or a positive ck_status; nothing
+ * throws or aborts across this boundary.  ck_last_error() returns a thread-local,
+ * human-readable message for the last non-zero status on the calling thread.
+ */
+#ifndef CK_H
+#define CK_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum ck_status {
+  CK_OK = 0,
+  CK_EINVAL = 1,       /* bad argument (NULL, negative size, invalid mechanism data) */
+  CK_ENOMEM = 2,       /* host or device allocation failed */
+  CK_ECUDA = 3,        /* a CUDA runtime call failed; see ck_last_error() */
+  CK_EUNSUPPORTED = 4  /* unknown reaction type, or a mechanism too large for the kernels */
+} ck_status;
+
+/* reaction types (Sec. 2.4) */
+enum { CK_ELEMENTARY = 0, CK_THREE_BODY = 1, CK_LINDEMANN = 2, CK_TROE = 3 };
+
+typedef struct ck_mech ck_mech; /* opaque; owns device memory on the device current at create */
+
+/* Mechanism description.  All pointers are HOST pointers; the arrays are copied by
+ * ck_mech_create and stay owned by the caller.  S = n_species, R = n_reactions.
+ * Matrices are row-major with the species index first: element (k, j) at k*R + j. */
+typedef struct ck_mech_desc {
+  int32_t n_species;         /* S >= 1 */
+  int32_t n_reactions;       /* R >= 1 */
+  const double *mol_weight;  /* [S]   W_k > 0, kg/kmol */
+  const double *nu_reac;     /* [S*R] nu'_kj  >= 0; real values allowed */
+  const double *nu_prod;     /* [S*R] nu''_kj >= 0 */
+  const double *ln_A;        /* [R]   ln of the pre-exponential factor (Eq. 5-6), SI-kmol units */
+  const double *b;           /* [R]   temperature exponent */
+  const double *Ea_over_R;   /* [R]   activation temperature Ea/R, K */
+  const uint8_t *reversible; /* [R]   1/0; NULL => all reversible */
+  const double *nasa_lo;     /* [S*7] a1..a7 of species k at k*7, used for T <= T_mid[k] */
+  const double *nasa_hi;     /* [S*7] a1..a7, used for T > T_mid[k] */
+  const double *T_mid;       /* [S]   cutoff temperature, K */
+  const uint8_t *rxn_type;   /* [R]   CK_ELEMENTARY..CK_TROE; NULL => all elementary */
+  const double *eff;         /* [S*R] third-body efficiencies E_kj; read only in
+                                      columns with rxn_type != 0; NULL => all 1 */
+  const double *ln_A0;       /* [R]   low-pressure-limit Arrhenius set; read where rxn_type is */
+  const double *b0;          /* [R]   CK_LINDEMANN or CK_TROE (the main set is then k_inf);   */
+  const double *Ea0_over_R;  /* [R]   may be NULL if there is no falloff reaction             */
+  const double *troe;        /* [R*4] alpha, T***, T*, T** at j*4; T** = +INF gives the
+                                      3-parameter form; read where rxn_type == CK_TROE */
+  double p_ref;              /* Pa, standard-state pressure of the NASA data (Eq. 8) */
+} ck_mech_desc;
+
+/* Validate `desc`, build the device-resident mechanism (sorted reaction program, folded
+ * equilibrium-layer coefficients, thermo tables, efficiency matrix) on the current CUDA
+ * device and return an opaque handle in *out.  Synchronous.
+ * Errors: CK_EINVAL (NULL pointers, S/R < 1, W <= 0, negative or non-finite nu, a reaction
+ * without reactants or without products, T_mid <= 0, non-positive Troe temperatures,
+ * p_ref <= 0), CK_EUNSUPPORTED (unknown rxn_type; S or R beyond the kernels' limits),
+ * CK_ENOMEM, CK_ECUDA.  On error *out is set to NULL. */
+int ck_mech_create(const ck_mech_desc *desc, ck_mech **out);
+
+/* Source terms of N cells.  T, P, Y, wdot, dTdt are DEVICE pointers, fp64, 8-byte aligned:
+ *   T[N] K, P[N] Pa, Y[S][N] mass fractions with species k at Y + k*N (SoA);
+ *   wdot[S][N] kmol/m^3/s (Eq. 2), dTdt[N] K/s.
+ * `stream` is a cudaStream_t (NULL = default stream).  The call is asynchronous on
+ * `stream`, allocates nothing, synchronises nothing and is deterministic run to run.
+ * Inputs are not modified; outputs must not alias inputs.  Calls that share one handle
+ * must be ordered on one stream (the handle owns a scratch area).  N == 0 is a
+ * successful no-op.  Concentrations are floored at 1e-300 kmol/m^3, so Y_k <= 0 acts as
+ * an absent species; T must be finite and > 0, P > 0; inputs are not screened for NaN.
+ * Errors: CK_EINVAL (NULL handle or pointer with N > 0, N < 0), CK_ECUDA. */
+int ck_source_terms(const ck_mech *m, const double *T, const double *P, const double *Y,
+                    int64_t N, double *wdot, double *dTdt, void *stream);
+
+/* Same computation with HOST buffers: copies T, P, Y to the device, runs
+ * ck_source_terms and copies wdot, dTdt back, all on `stream`, then synchronises it.
+ * Pinned host memory makes the copies asynchronous; pageable memory also works.
+ * Device staging buffers are owned by the handle and grow on demand. */
+int ck_source_terms_host(ck_mech *m, const double *T, const double *P, const double *Y,
+                         int64_t N, double *wdot, double *dTdt, void *stream);
+
+/* Free the handle and its device memory.  NULL is a no-op. */
+void ck_mech_destroy(ck_mech *m);
+
+/* Message for the last non-zero status returned on this thread ("" if none). */
+const char *ck_last_error(void);
+
+/* Introspection (for the harness: roofline accounting and launch reporting).
+ * what: 0 S, 1 R, 2 nnz(nu'), 3 nnz(nu''), 4 nnz(nu''-nu'), 5 #three-body, 6 #Lindemann,
+ *       7 #Troe, 8 #temperature ranges, 9 threads per block, 10 blocks per SM,
+ *       11 dynamic shared memory per block (bytes), 12 kernels launched per
+ *       ck_source_terms call, 13 nnz(E) counted over third-body and falloff columns.
+ * Returns -1 for a NULL handle or unknown `what`. */
+int64_t ck_mech_info(const ck_mech *m, int what);
+
+/* Measured FP64 FMA throughput of the current device, in FMA instructions (thread level)
+ * per second: a register-resident DFMA loop on every SM, timed with CUDA events on
+ * `stream`.  Used as the roofline denominator for this FP64-pipe-bound path.
+ * Returns CK_OK and writes *fma_per_s, or CK_ECUDA. */
+int ck_measure_fp64_peak(double *fma_per_s, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CK_H */

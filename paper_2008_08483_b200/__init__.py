@@ -1,0 +1,214 @@
+"""paper_2008_08483_b200 -- B200-native batched chemical source terms (arXiv 2008.08483).
+
+Thin Python binding of the C ABI in include/ck.h (libck.so, hand-written CUDA for
+sm_100a).  Argument marshalling only: every step of the path runs in the CUDA kernels.
+There is no CPU fallback; importing this package fails loudly if the library is missing
+and cannot be built.  PyTorch (optional here) is only used by callers for device memory
+and streams; this module accepts anything exposing `data_ptr()` or raw integer addresses.
+
+    mech = Mechanism(ckgen_mechanism)                  # ck_mech_create
+    mech.source_terms(T, P, Y, wdot, dTdt, stream=0)   # ck_source_terms (device pointers)
+    mech.source_terms_host(T, P, Y)                    # ck_source_terms_host (numpy, host)
+    mech.close()                                       # ck_mech_destroy
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import _build
+
+__all__ = ["Mechanism", "CkError", "ck_mech_create", "ck_source_terms", "ck_source_terms_host",
+           "ck_mech_destroy", "ck_last_error", "ck_mech_info", "ck_measure_fp64_peak",
+           "library_path", "RU", "INFO"]
+
+RU = 8314.46261815324  # J/(kmol K), the constant compiled into the kernels
+INFO = {"S": 0, "R": 1, "nnz_reac": 2, "nnz_prod": 3, "nnz_net": 4, "n_three_body": 5,
+        "n_lindemann": 6, "n_troe": 7, "n_ranges": 8, "threads": 9, "blocks_per_sm": 10,
+        "smem_bytes": 11, "launches_per_call": 12, "nnz_eff": 13}
+
+_dp = C.POINTER(C.c_double)
+_bp = C.POINTER(C.c_uint8)
+
+
+class _Desc(C.Structure):
+    _fields_ = [
+        ("n_species", C.c_int32), ("n_reactions", C.c_int32),
+        ("mol_weight", _dp), ("nu_reac", _dp), ("nu_prod", _dp),
+        ("ln_A", _dp), ("b", _dp), ("Ea_over_R", _dp), ("reversible", _bp),
+        ("nasa_lo", _dp), ("nasa_hi", _dp), ("T_mid", _dp), ("rxn_type", _bp),
+        ("eff", _dp), ("ln_A0", _dp), ("b0", _dp), ("Ea0_over_R", _dp), ("troe", _dp),
+        ("p_ref", C.c_double),
+    ]
+
+
+class CkError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__("ck status %d: %s" % (status, message))
+        self.status = status
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def _load():
+    path = _build.LIB
+    if not os.path.exists(path) or os.path.getmtime(path) < _build._newest_source():
+        path = _build.build()          # raises if nvcc is missing or compilation fails
+    lib = C.CDLL(path)
+    lib.ck_mech_create.restype = C.c_int
+    lib.ck_mech_create.argtypes = [C.POINTER(_Desc), C.POINTER(C.c_void_p)]
+    lib.ck_source_terms.restype = C.c_int
+    lib.ck_source_terms.argtypes = [C.c_void_p] * 4 + [C.c_int64] + [C.c_void_p] * 3
+    lib.ck_source_terms_host.restype = C.c_int
+    lib.ck_source_terms_host.argtypes = [C.c_void_p] * 4 + [C.c_int64] + [C.c_void_p] * 3
+    lib.ck_mech_destroy.restype = None
+    lib.ck_mech_destroy.argtypes = [C.c_void_p]
+    lib.ck_last_error.restype = C.c_char_p
+    lib.ck_last_error.argtypes = []
+    lib.ck_mech_info.restype = C.c_int64
+    lib.ck_mech_info.argtypes = [C.c_void_p, C.c_int]
+    lib.ck_measure_fp64_peak.restype = C.c_int
+    lib.ck_measure_fp64_peak.argtypes = [_dp, C.c_void_p]
+    return lib
+
+
+_lib = _load()
+
+
+def _addr(x):
+    """Raw address of a device/host buffer: int, None, torch tensor or numpy array."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if isinstance(x, np.ndarray):
+        return x.ctypes.data
+    raise TypeError("expected an address, a tensor or a numpy array, got %r" % type(x))
+
+
+def _check(status):
+    if status != 0:
+        raise CkError(status, _lib.ck_last_error().decode())
+
+
+# ---- the C entry points, same names, status codes raised as CkError -------------------
+
+def ck_last_error() -> str:
+    return _lib.ck_last_error().decode()
+
+
+def ck_mech_create(desc: "_Desc") -> int:
+    handle = C.c_void_p()
+    _check(_lib.ck_mech_create(C.byref(desc), C.byref(handle)))
+    return handle.value
+
+
+def ck_source_terms(handle, T, P, Y, N, wdot, dTdt, stream=0) -> None:
+    _check(_lib.ck_source_terms(handle, _addr(T), _addr(P), _addr(Y), int(N), _addr(wdot),
+                                _addr(dTdt), stream or None))
+
+
+def ck_source_terms_host(handle, T, P, Y, N, wdot, dTdt, stream=0) -> None:
+    _check(_lib.ck_source_terms_host(handle, _addr(T), _addr(P), _addr(Y), int(N), _addr(wdot),
+                                     _addr(dTdt), stream or None))
+
+
+def ck_mech_destroy(handle) -> None:
+    _lib.ck_mech_destroy(handle)
+
+
+def ck_mech_info(handle, what) -> int:
+    return int(_lib.ck_mech_info(handle, INFO[what] if isinstance(what, str) else int(what)))
+
+
+def ck_measure_fp64_peak(stream=0) -> float:
+    out = C.c_double()
+    _check(_lib.ck_measure_fp64_peak(C.byref(out), stream or None))
+    return out.value
+
+
+# ---- convenience wrapper -----------------------------------------------------------------
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _u8(a):
+    return np.ascontiguousarray(a, dtype=np.uint8)
+
+
+def make_desc(mech):
+    """ck_mech_desc from any object with ckgen.Mechanism's array attributes.
+    Returns (desc, keepalive) -- keepalive owns the host arrays the desc points to."""
+    S, R = int(mech.nu_reac.shape[0]), int(mech.nu_reac.shape[1])
+    keep = dict(
+        mol_weight=_f64(mech.mol_weight), nu_reac=_f64(mech.nu_reac), nu_prod=_f64(mech.nu_prod),
+        ln_A=_f64(mech.ln_A), b=_f64(mech.b), Ea_over_R=_f64(mech.Ea_over_R),
+        reversible=_u8(mech.reversible), nasa_lo=_f64(mech.nasa_lo), nasa_hi=_f64(mech.nasa_hi),
+        T_mid=_f64(mech.T_mid), rxn_type=_u8(mech.rxn_type), eff=_f64(mech.eff),
+        ln_A0=_f64(mech.ln_A0), b0=_f64(mech.b0), Ea0_over_R=_f64(mech.Ea0_over_R),
+        troe=_f64(mech.troe))
+    shapes = dict(mol_weight=(S,), nu_reac=(S, R), nu_prod=(S, R), ln_A=(R,), b=(R,),
+                  Ea_over_R=(R,), reversible=(R,), nasa_lo=(S, 7), nasa_hi=(S, 7), T_mid=(S,),
+                  rxn_type=(R,), eff=(S, R), ln_A0=(R,), b0=(R,), Ea0_over_R=(R,), troe=(R, 4))
+    for name, shp in shapes.items():
+        if keep[name].shape != shp:
+            raise ValueError("%s has shape %s, expected %s" % (name, keep[name].shape, shp))
+    d = _Desc()
+    d.n_species, d.n_reactions, d.p_ref = S, R, float(mech.p_ref)
+    for name, arr in keep.items():
+        setattr(d, name, arr.ctypes.data_as(_bp if arr.dtype == np.uint8 else _dp))
+    return d, keep
+
+
+class Mechanism:
+    """Owns a ck_mech handle created from a mechanism's arrays."""
+
+    def __init__(self, mech):
+        desc, keep = make_desc(mech)
+        self.handle = ck_mech_create(desc)
+        del keep                      # the library copied everything it needs
+        self.S = ck_mech_info(self.handle, "S")
+        self.R = ck_mech_info(self.handle, "R")
+
+    def info(self, what) -> int:
+        return ck_mech_info(self.handle, what)
+
+    def source_terms(self, T, P, Y, wdot, dTdt, N=None, stream=0) -> None:
+        """Device buffers (torch CUDA tensors or addresses); asynchronous on `stream`."""
+        if N is None:
+            N = T.shape[0]
+        ck_source_terms(self.handle, T, P, Y, N, wdot, dTdt, stream)
+
+    def source_terms_host(self, T, P, Y, wdot=None, dTdt=None, stream=0):
+        """Host buffers (numpy or pinned torch CPU tensors); synchronous. Returns (wdot, dTdt)."""
+        N = int(T.shape[0])
+        if wdot is None:
+            wdot = np.empty((self.S, N))
+        if dTdt is None:
+            dTdt = np.empty(N)
+        ck_source_terms_host(self.handle, T, P, Y, N, wdot, dTdt, stream)
+        return wdot, dTdt
+
+    def close(self) -> None:
+        if getattr(self, "handle", None):
+            ck_mech_destroy(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

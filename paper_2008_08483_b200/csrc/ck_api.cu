@@ -1,0 +1,375 @@
+// ck_api.cu -- the C ABI of include/ck.h: validation, mechanism build (host
+// preprocessing of the paper's matrices into the device reaction program), launches.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/ck.h"
+#include "ck_internal.h"
+
+namespace {
+
+thread_local std::string g_last_error;
+
+int fail(int status, const std::string &msg) {
+  g_last_error = msg;
+  return status;
+}
+
+int fail_cuda(cudaError_t e, const char *what) {
+  g_last_error = std::string(what) + ": " + cudaGetErrorString(e);
+  return CK_ECUDA;
+}
+
+// byte buffer with aligned appends; returns the offset of the appended block
+struct Packer {
+  std::vector<unsigned char> bytes;
+  size_t append(const void *p, size_t n, size_t align = 256) {
+    size_t off = (bytes.size() + align - 1) / align * align;
+    bytes.resize(off + n);
+    if (n) std::memcpy(bytes.data() + off, p, n);
+    return off;
+  }
+};
+
+int validate(const ck_mech_desc *d) {
+  if (!d) return fail(CK_EINVAL, "desc is NULL");
+  const int S = d->n_species, R = d->n_reactions;
+  if (S < 1 || R < 1) return fail(CK_EINVAL, "n_species and n_reactions must be >= 1");
+  if (!d->mol_weight || !d->nu_reac || !d->nu_prod || !d->ln_A || !d->b || !d->Ea_over_R ||
+      !d->nasa_lo || !d->nasa_hi || !d->T_mid)
+    return fail(CK_EINVAL, "a required array pointer is NULL");
+  if (!(d->p_ref > 0.0) || !std::isfinite(d->p_ref)) return fail(CK_EINVAL, "p_ref must be > 0");
+  for (int k = 0; k < S; ++k) {
+    if (!(d->mol_weight[k] > 0.0) || !std::isfinite(d->mol_weight[k]))
+      return fail(CK_EINVAL, "mol_weight must be finite and > 0");
+    if (!(d->T_mid[k] > 0.0) || !std::isfinite(d->T_mid[k]))
+      return fail(CK_EINVAL, "T_mid must be finite and > 0");
+    for (int i = 0; i < 7; ++i)
+      if (!std::isfinite(d->nasa_lo[k * 7 + i]) || !std::isfinite(d->nasa_hi[k * 7 + i]))
+        return fail(CK_EINVAL, "NASA coefficients must be finite");
+  }
+  for (int j = 0; j < R; ++j) {
+    const int type = d->rxn_type ? d->rxn_type[j] : CK_ELEMENTARY;
+    if (type < CK_ELEMENTARY || type > CK_TROE)
+      return fail(CK_EUNSUPPORTED, "unknown rxn_type code (only 0..3 are supported)");
+    if (!std::isfinite(d->ln_A[j]) || !std::isfinite(d->b[j]) || !std::isfinite(d->Ea_over_R[j]))
+      return fail(CK_EINVAL, "Arrhenius parameters must be finite");
+    double sum_r = 0, sum_p = 0;
+    for (int k = 0; k < S; ++k) {
+      const double a = d->nu_reac[(size_t)k * R + j], b = d->nu_prod[(size_t)k * R + j];
+      if (!(a >= 0.0) || !(b >= 0.0) || !std::isfinite(a) || !std::isfinite(b))
+        return fail(CK_EINVAL, "stoichiometric coefficients must be finite and >= 0");
+      sum_r += a;
+      sum_p += b;
+      if (type != CK_ELEMENTARY && d->eff) {
+        const double e = d->eff[(size_t)k * R + j];
+        if (!(e >= 0.0) || !std::isfinite(e))
+          return fail(CK_EINVAL, "third-body efficiencies must be finite and >= 0");
+      }
+    }
+    if (sum_r <= 0.0 || sum_p <= 0.0)
+      return fail(CK_EINVAL, "every reaction needs at least one reactant and one product");
+    if (type == CK_LINDEMANN || type == CK_TROE) {
+      if (!d->ln_A0 || !d->b0 || !d->Ea0_over_R)
+        return fail(CK_EINVAL, "falloff reactions need ln_A0, b0 and Ea0_over_R");
+      if (!std::isfinite(d->ln_A0[j]) || !std::isfinite(d->b0[j]) || !std::isfinite(d->Ea0_over_R[j]))
+        return fail(CK_EINVAL, "low-pressure Arrhenius parameters must be finite");
+    }
+    if (type == CK_TROE) {
+      if (!d->troe) return fail(CK_EINVAL, "Troe reactions need the troe array");
+      const double *t = d->troe + 4 * (size_t)j;
+      if (!std::isfinite(t[0])) return fail(CK_EINVAL, "Troe alpha must be finite");
+      if (!(t[1] > 0.0) || !(t[2] > 0.0) || !(t[3] > 0.0) || std::isnan(t[3]) ||
+          !std::isfinite(t[1]) || !std::isfinite(t[2]))
+        return fail(CK_EINVAL, "Troe temperatures must be > 0 (T** may be +INF)");
+    }
+  }
+  return CK_OK;
+}
+
+// g'_k = g_k/RT - ln(p_ref/(Ru T)) on the features [1, ln T, T, T^2, T^3, T^4, 1/T]
+// (Eq. 10 with the standard-concentration term folded into the bias)
+void gibbs_feature_row(const double *a, double p_ref, long double out[7]) {
+  out[0] = (long double)a[0] - (long double)a[6] - logl((long double)p_ref / (long double)ck::kRu);
+  out[1] = 1.0L - (long double)a[0];
+  out[2] = -(long double)a[1] / 2.0L;
+  out[3] = -(long double)a[2] / 6.0L;
+  out[4] = -(long double)a[3] / 12.0L;
+  out[5] = -(long double)a[4] / 20.0L;
+  out[6] = (long double)a[5];
+}
+
+}  // namespace
+
+extern "C" const char *ck_last_error(void) { return g_last_error.c_str(); }
+
+extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
+  if (!out) return fail(CK_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (int st = validate(d)) return st;
+  const int S = d->n_species, R = d->n_reactions;
+
+  ck_mech *m = new (std::nothrow) ck_mech();
+  if (!m) return fail(CK_ENOMEM, "host allocation failed");
+  cudaError_t ce = cudaGetDevice(&m->device);
+  if (ce != cudaSuccess) { delete m; return fail_cuda(ce, "cudaGetDevice"); }
+  cudaDeviceProp prop;
+  ce = cudaGetDeviceProperties(&prop, m->device);
+  if (ce != cudaSuccess) { delete m; return fail_cuda(ce, "cudaGetDeviceProperties"); }
+  m->num_sms = prop.multiProcessorCount;
+
+  // ---- launch shape: as many resident cells per SM as shared memory allows ----------
+  int best_threads = 0, best_bps = 0;
+  size_t best_smem = 0;
+  for (int threads : {128, 64, 32}) {
+    size_t smem = (size_t)2 * S * threads * sizeof(double);
+    if (smem > (size_t)prop.sharedMemPerBlockOptin) continue;
+    int bps = 0;
+    ce = ck::kernel_configure(threads, smem, &bps);
+    if (ce != cudaSuccess) { delete m; return fail_cuda(ce, "kernel_configure"); }
+    if (bps * threads > best_bps * best_threads) {
+      best_threads = threads; best_bps = bps; best_smem = smem;
+    }
+  }
+  if (best_threads == 0) {
+    delete m;
+    return fail(CK_EUNSUPPORTED, "n_species too large for the shared-memory resident kernel");
+  }
+  ce = ck::kernel_configure(best_threads, best_smem, &best_bps);   // leave the attribute set
+  if (ce != cudaSuccess) { delete m; return fail_cuda(ce, "kernel_configure"); }
+  m->blocks_per_sm = best_bps;
+  m->smem_bytes = best_smem;
+  m->grid_max = m->num_sms * best_bps;
+
+  // ---- temperature ranges from the distinct T_mid values --------------
+  std::vector<double> range_T(d->T_mid, d->T_mid + S);
+  std::sort(range_T.begin(), range_T.end());
+  range_T.erase(std::unique(range_T.begin(), range_T.end()), range_T.end());
+  const int n_ranges = (int)range_T.size() + 1;
+  std::vector<int> rank(S);
+  for (int k = 0; k < S; ++k)
+    rank[k] = (int)(std::lower_bound(range_T.begin(), range_T.end(), d->T_mid[k]) - range_T.begin());
+
+  // ---- per-species tables -------------------------------------------------------------
+  std::vector<double> inv_W(S), thermo((size_t)S * ck::kThermoStride, 0.0);
+  std::vector<long double> gfeat((size_t)S * 2 * 7);
+  for (int k = 0; k < S; ++k) {
+    inv_W[k] = 1.0 / d->mol_weight[k];
+    double *t = &thermo[(size_t)k * ck::kThermoStride];
+    const double *lo = d->nasa_lo + 7 * k, *hi = d->nasa_hi + 7 * k;
+    t[0] = d->T_mid[k];
+    for (int i = 0; i < 5; ++i) { t[1 + i] = lo[i]; t[6 + i] = hi[i]; }
+    for (int i = 0; i < 5; ++i) { t[11 + i] = lo[i] / (i + 1); t[17 + i] = hi[i] / (i + 1); }
+    t[16] = lo[5];
+    t[22] = hi[5];
+    gibbs_feature_row(lo, d->p_ref, &gfeat[((size_t)k * 2 + 0) * 7]);
+    gibbs_feature_row(hi, d->p_ref, &gfeat[((size_t)k * 2 + 1) * 7]);
+  }
+
+  // ---- reaction program ------------------------------------------------------------------
+  std::vector<unsigned char> program;
+  std::vector<double> falloff;
+  std::vector<int> m_rows;       // reaction index of each row of M
+  for (int j = 0; j < R; ++j) {
+    const int type = d->rxn_type ? d->rxn_type[j] : CK_ELEMENTARY;
+    const int rev = d->reversible ? (d->reversible[j] != 0) : 1;
+    std::vector<int> off_r, off_p, off_s;
+    std::vector<double> c_r, c_p, c_s;
+    for (int k = 0; k < S; ++k) {
+      const double a = d->nu_reac[(size_t)k * R + j], b = d->nu_prod[(size_t)k * R + j];
+      if (a != 0.0) { off_r.push_back(k); c_r.push_back(a); }
+      if (b != 0.0) { off_p.push_back(k); c_p.push_back(b); }
+      if (b - a != 0.0) { off_s.push_back(k); c_s.push_back(b - a); }
+    }
+    m->nnz_reac += (int64_t)off_r.size();
+    m->nnz_prod += (int64_t)off_p.size();
+    m->nnz_net += (int64_t)off_s.size();
+
+    ck::RecHeader h{};
+    h.nr = (int)off_r.size(); h.np = (int)off_p.size(); h.nsc = (int)off_s.size();
+    h.type = type; h.reversible = rev; h.m_slot = -1; h.fo_idx = -1;
+    if (type != CK_ELEMENTARY) {
+      h.m_slot = (int)m_rows.size();
+      m_rows.push_back(j);
+      for (int k = 0; k < S; ++k)
+        if (!d->eff || d->eff[(size_t)k * R + j] != 0.0) m->nnz_eff++;
+    }
+    if (type == CK_THREE_BODY) m->n_three_body++;
+    if (type == CK_LINDEMANN || type == CK_TROE) {
+      h.fo_idx = (int)(falloff.size() / ck::kFalloffStride);
+      double row[ck::kFalloffStride] = {d->ln_A0[j], d->b0[j], -d->Ea0_over_R[j], 0, 0, 0, 0,
+                                        (double)type};
+      if (type == CK_TROE) {
+        const double *t = d->troe + 4 * (size_t)j;
+        row[3] = t[0]; row[4] = -1.0 / t[1]; row[5] = -1.0 / t[2]; row[6] = -t[3];
+        m->n_troe++;
+      } else {
+        m->n_lindemann++;
+      }
+      falloff.insert(falloff.end(), row, row + ck::kFalloffStride);
+    }
+
+    std::vector<double> dbl;
+    dbl.push_back(d->ln_A[j]); dbl.push_back(d->b[j]); dbl.push_back(-d->Ea_over_R[j]);
+    dbl.push_back(0.0);
+    for (int r = 0; r < n_ranges; ++r) {
+      long double f[7] = {(long double)d->ln_A[j], (long double)d->b[j], 0, 0, 0, 0,
+                          -(long double)d->Ea_over_R[j]};
+      for (size_t e = 0; e < off_s.size(); ++e) {
+        const int k = off_s[e];
+        const int variant = (r > rank[k]) ? 1 : 0;   // T > T_mid[k] throughout range r
+        const long double *g = &gfeat[((size_t)k * 2 + variant) * 7];
+        for (int i = 0; i < 7; ++i) f[i] += (long double)c_s[e] * g[i];
+      }
+      for (int i = 0; i < 7; ++i) dbl.push_back((double)f[i]);
+      dbl.push_back(0.0);
+    }
+    dbl.insert(dbl.end(), c_r.begin(), c_r.end());
+    dbl.insert(dbl.end(), c_p.begin(), c_p.end());
+    dbl.insert(dbl.end(), c_s.begin(), c_s.end());
+    if (dbl.size() % 2) dbl.push_back(0.0);
+    std::vector<int32_t> ints;
+    ints.insert(ints.end(), off_r.begin(), off_r.end());
+    ints.insert(ints.end(), off_p.begin(), off_p.end());
+    ints.insert(ints.end(), off_s.begin(), off_s.end());
+    while (ints.size() % 4) ints.push_back(0);
+
+    h.size_bytes = (int32_t)(sizeof(h) + dbl.size() * sizeof(double) + ints.size() * sizeof(int32_t));
+    const size_t at = program.size();
+    program.resize(at + h.size_bytes);
+    std::memcpy(&program[at], &h, sizeof(h));
+    std::memcpy(&program[at + sizeof(h)], dbl.data(), dbl.size() * sizeof(double));
+    std::memcpy(&program[at + sizeof(h) + dbl.size() * sizeof(double)], ints.data(),
+                ints.size() * sizeof(int32_t));
+  }
+
+  // ---- third-body efficiency matrix, blocked for the register-tiled M = C E -----------
+  const int n_m = (int)m_rows.size();
+  const int n_mb = (n_m + ck::kMBlock - 1) / ck::kMBlock;
+  std::vector<double> eff((size_t)std::max(n_mb, 1) * S * ck::kMBlock, 0.0);
+  for (int s = 0; s < n_m; ++s) {
+    const int j = m_rows[s];
+    for (int k = 0; k < S; ++k)
+      eff[((size_t)(s / ck::kMBlock) * S + k) * ck::kMBlock + (s % ck::kMBlock)] =
+          d->eff ? d->eff[(size_t)k * R + j] : 1.0;
+  }
+  if (falloff.empty()) falloff.resize(ck::kFalloffStride, 0.0);
+  if (range_T.empty()) range_T.push_back(0.0);
+
+  // ---- one device allocation for all tables -------------------------------------------
+  Packer pk;
+  const size_t o_invW = pk.append(inv_W.data(), inv_W.size() * sizeof(double));
+  const size_t o_rng = pk.append(range_T.data(), range_T.size() * sizeof(double));
+  const size_t o_thermo = pk.append(thermo.data(), thermo.size() * sizeof(double));
+  const size_t o_eff = pk.append(eff.data(), eff.size() * sizeof(double));
+  const size_t o_fo = pk.append(falloff.data(), falloff.size() * sizeof(double));
+  const size_t o_prog = pk.append(program.data(), program.size());
+  ce = cudaMalloc(&m->d_tables, pk.bytes.size());
+  if (ce != cudaSuccess) { delete m; return fail(CK_ENOMEM, std::string("cudaMalloc tables: ") + cudaGetErrorString(ce)); }
+  ce = cudaMemcpy(m->d_tables, pk.bytes.data(), pk.bytes.size(), cudaMemcpyHostToDevice);
+  if (ce != cudaSuccess) { ck_mech_destroy(m); return fail_cuda(ce, "cudaMemcpy tables"); }
+  const size_t scratch_elems = (size_t)m->grid_max * std::max(n_mb, 1) * ck::kMBlock * best_threads;
+  ce = cudaMalloc((void **)&m->d_scratch, scratch_elems * sizeof(double));
+  if (ce != cudaSuccess) { ck_mech_destroy(m); return fail(CK_ENOMEM, std::string("cudaMalloc scratch: ") + cudaGetErrorString(ce)); }
+
+  unsigned char *base = (unsigned char *)m->d_tables;
+  ck::DeviceMech &dm = m->dev;
+  dm.S = S; dm.R = R; dm.n_ranges = n_ranges; dm.n_m = n_m; dm.n_m_blocks = n_mb;
+  dm.threads = best_threads;
+  dm.inv_W = (const double *)(base + o_invW);
+  dm.range_T = (const double *)(base + o_rng);
+  dm.thermo = (const double *)(base + o_thermo);
+  dm.eff = (const double *)(base + o_eff);
+  dm.falloff = (const double *)(base + o_fo);
+  dm.program = base + o_prog;
+  dm.m_scratch = m->d_scratch;
+  *out = m;
+  return CK_OK;
+}
+
+extern "C" void ck_mech_destroy(ck_mech *m) {
+  if (!m) return;
+  if (m->d_tables) cudaFree(m->d_tables);
+  if (m->d_scratch) cudaFree(m->d_scratch);
+  if (m->d_stage) cudaFree(m->d_stage);
+  delete m;
+}
+
+extern "C" int ck_source_terms(const ck_mech *m, const double *T, const double *P,
+                               const double *Y, int64_t N, double *wdot, double *dTdt,
+                               void *stream) {
+  if (!m) return fail(CK_EINVAL, "mechanism handle is NULL");
+  if (N < 0) return fail(CK_EINVAL, "N must be >= 0");
+  if (N == 0) return CK_OK;
+  if (!T || !P || !Y || !wdot || !dTdt) return fail(CK_EINVAL, "a state or result pointer is NULL");
+  if (((uintptr_t)T | (uintptr_t)P | (uintptr_t)Y | (uintptr_t)wdot | (uintptr_t)dTdt) & 7u)
+    return fail(CK_EINVAL, "pointers must be 8-byte aligned");
+  cudaError_t ce = ck::launch_source_terms(m, T, P, Y, N, wdot, dTdt, (cudaStream_t)stream);
+  if (ce != cudaSuccess) return fail_cuda(ce, "ck_source_terms launch");
+  return CK_OK;
+}
+
+extern "C" int ck_source_terms_host(ck_mech *m, const double *T, const double *P,
+                                    const double *Y, int64_t N, double *wdot, double *dTdt,
+                                    void *stream) {
+  if (!m) return fail(CK_EINVAL, "mechanism handle is NULL");
+  if (N < 0) return fail(CK_EINVAL, "N must be >= 0");
+  if (N == 0) return CK_OK;
+  if (!T || !P || !Y || !wdot || !dTdt) return fail(CK_EINVAL, "a state or result pointer is NULL");
+  const int64_t S = m->dev.S;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t ce;
+  if (m->stage_cells < N) {
+    if (m->d_stage) { cudaFree(m->d_stage); m->d_stage = nullptr; m->stage_cells = 0; }
+    ce = cudaMalloc((void **)&m->d_stage, (size_t)(2 * S + 3) * N * sizeof(double));
+    if (ce != cudaSuccess) return fail(CK_ENOMEM, std::string("cudaMalloc staging: ") + cudaGetErrorString(ce));
+    m->stage_cells = N;
+  }
+  double *dT = m->d_stage, *dP = dT + N, *dY = dP + N, *dW = dY + S * N, *dD = dW + S * N;
+  const size_t col = (size_t)N * sizeof(double);
+  if ((ce = cudaMemcpyAsync(dT, T, col, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+      (ce = cudaMemcpyAsync(dP, P, col, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+      (ce = cudaMemcpyAsync(dY, Y, col * S, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+    return fail_cuda(ce, "host to device copy");
+  if (int rc = ck_source_terms(m, dT, dP, dY, N, dW, dD, stream)) return rc;
+  if ((ce = cudaMemcpyAsync(wdot, dW, col * S, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+      (ce = cudaMemcpyAsync(dTdt, dD, col, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+    return fail_cuda(ce, "device to host copy");
+  if ((ce = cudaStreamSynchronize(st)) != cudaSuccess) return fail_cuda(ce, "cudaStreamSynchronize");
+  return CK_OK;
+}
+
+extern "C" int64_t ck_mech_info(const ck_mech *m, int what) {
+  if (!m) return -1;
+  switch (what) {
+    case 0: return m->dev.S;
+    case 1: return m->dev.R;
+    case 2: return m->nnz_reac;
+    case 3: return m->nnz_prod;
+    case 4: return m->nnz_net;
+    case 5: return m->n_three_body;
+    case 6: return m->n_lindemann;
+    case 7: return m->n_troe;
+    case 8: return m->dev.n_ranges;
+    case 9: return m->dev.threads;
+    case 10: return m->blocks_per_sm;
+    case 11: return (int64_t)m->smem_bytes;
+    case 12: return 1;
+    case 13: return m->nnz_eff;
+    default: return -1;
+  }
+}
+
+extern "C" int ck_measure_fp64_peak(double *fma_per_s, void *stream) {
+  if (!fma_per_s) return fail(CK_EINVAL, "fma_per_s is NULL");
+  cudaError_t ce = ck::measure_fp64_peak(fma_per_s, (cudaStream_t)stream);
+  if (ce != cudaSuccess) return fail_cuda(ce, "ck_measure_fp64_peak");
+  return CK_OK;
+}

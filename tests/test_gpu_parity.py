@@ -1,0 +1,272 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element,
+with the north_star tolerance:
+   |d wdot_k| <= 1e-10 max_k|wdot_k| + 1e-12 |wdot_k|,  |d dT/dt| <= 1e-10 |dT/dt| + 1e-12 K/s.
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import ckgen
+import oracle
+from helpers import RU, parity_violations
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def ck():
+    import paper_2008_08483_b200 as ck
+    assert torch.cuda.is_available()
+    return ck
+
+
+def gpu_run(ck, mech, T, P, Y, gm=None):
+    """T, P, Y numpy -> (wdot[S,N], dTdt[N]) numpy via ck_source_terms on device buffers."""
+    own = gm is None
+    gm = gm or ck.Mechanism(mech)
+    dev = torch.device("cuda:0")
+    N = T.shape[0]
+    Td = torch.from_numpy(np.ascontiguousarray(T)).to(dev)
+    Pd = torch.from_numpy(np.ascontiguousarray(P)).to(dev)
+    Yd = torch.from_numpy(np.ascontiguousarray(Y)).to(dev)
+    w = torch.full((mech.n_species, N), float("nan"), dtype=torch.float64, device=dev)
+    d = torch.full((N,), float("nan"), dtype=torch.float64, device=dev)
+    gm.source_terms(Td, Pd, Yd, w, d, N=N, stream=torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    if own:
+        gm.close()
+    return w.cpu().numpy(), d.cpu().numpy()
+
+
+def assert_parity(ck, mech, T, P, Y, label=""):
+    w, d = gpu_run(ck, mech, T, P, Y)
+    wr, dr, _ = oracle.source_terms(oracle.OracleMechanism(mech), T, P, Y)
+    rw, rt = parity_violations(w, d, wr, dr)
+    assert rw <= 1.0, "%s wdot error is %.3g x tolerance" % (label, rw)
+    if rt > 1.0:
+        # report the conditioning of the energy sum rather than loosening the bound
+        i = int(np.argmax(np.abs(d - dr) / (1e-10 * np.abs(dr) + 1e-12)))
+        om = oracle.OracleMechanism(mech)
+        det = oracle.cell_detail(om, T[i], P[i], Y[:, i])
+        hw = det["h_RT"] * det["wdot"]
+        kappa = np.abs(hw).sum() / max(abs(hw.sum()), 1e-300)
+        raise AssertionError("%s dT/dt error is %.3g x tolerance at cell %d (kappa = %.3g)"
+                             % (label, rt, i, kappa))
+    return w, d, wr, dr
+
+
+# ---------------------------------------------------------------- the five configs, small N
+
+@pytest.mark.parametrize("cfg_name,N", [("tiny_1k", 1024), ("mid_1m", 2000), ("large_256k", 700),
+                                        ("mid_rk4", 515)])
+def test_config_parity_all_cells(ck, cfg_name, N):
+    """Every cell, sizes spanning several 128-cell tiles and a ragged tail."""
+    cfg = ckgen.CONFIGS[cfg_name]
+    mech = ckgen.mechanism(cfg.mech)
+    T, P, Y = ckgen.states(cfg, N=N)
+    assert_parity(ck, mech, T, P, Y, cfg_name)
+
+
+@pytest.mark.parametrize("cfg_name", ["tiny_1m", "mid_1m", "large_256k"])
+def test_full_size_sampled_parity_and_conservation(ck, cfg_name):
+    """BASELINE.json's full sizes in the launch configuration bench.py times: the oracle
+    checks a seeded sample of cells one by one; mass and element conservation (which hold
+    at any size) are checked on every cell on the device."""
+    cfg = ckgen.CONFIGS[cfg_name]
+    mech = ckgen.mechanism(cfg.mech)
+    T, P, Y = ckgen.states(cfg)
+    N = cfg.N
+    dev = torch.device("cuda:0")
+    gm = ck.Mechanism(mech)
+    Td, Pd, Yd = (torch.from_numpy(a).to(dev) for a in (T, P, Y))
+    w = torch.empty((mech.n_species, N), dtype=torch.float64, device=dev)
+    d = torch.empty((N,), dtype=torch.float64, device=dev)
+    gm.source_terms(Td, Pd, Yd, w, d, stream=torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert torch.isfinite(w).all() and torch.isfinite(d).all()
+    weights = [mech.mol_weight] + [mech.elem_count[:, e].astype(float) for e in range(mech.elem_count.shape[1])]
+    for wt in weights:
+        terms = torch.from_numpy(wt).to(dev)[:, None] * w
+        assert (terms.sum(0).abs() <= 1e-11 * terms.abs().sum(0) + 1e-300).all()
+    rng = np.random.default_rng(12345)
+    idx = np.unique(np.concatenate([rng.integers(0, N, size=1500), [0, 127, 128, N - 129, N - 1]]))
+    wr, dr, _ = oracle.source_terms(oracle.OracleMechanism(mech), T[idx], P[idx],
+                                    np.ascontiguousarray(Y[:, idx]))
+    rw, rt = parity_violations(w[:, idx].cpu().numpy(), d[idx].cpu().numpy(), wr, dr)
+    assert rw <= 1.0 and rt <= 1.0, (rw, rt)
+    gm.close()
+
+
+# ---------------------------------------------------------------- every reaction on its own
+
+@pytest.mark.parametrize("spec", [ckgen.MECH_TINY, ckgen.MECH_MID], ids=lambda s: s.name)
+def test_single_reaction_mechanisms(ck, spec):
+    """Each reaction as a mechanism of its own: with one reaction the north_star tolerance
+    is a relative 1e-10 on that reaction's rate, so no reaction hides behind a larger one.
+    Covers elementary, three-body and Troe records and both temperature ranges."""
+    mech = ckgen.mechanism(spec)
+    cfg = ckgen.CONFIGS["tiny_1k" if spec is ckgen.MECH_TINY else "mid_1m"]
+    cfg = dataclasses.replace(cfg, T_range=(600.0, 2800.0))
+    T, P, Y = ckgen.states(cfg, N=160)
+    R = mech.n_reactions
+    picks = range(R) if R <= 32 else np.unique(np.concatenate(
+        [np.flatnonzero(mech.rxn_type == 3)[:6], np.flatnonzero(mech.rxn_type == 1)[:6],
+         np.flatnonzero(mech.rxn_type == 0)[:12]]))
+    for j in picks:
+        assert_parity(ck, mech.subset([j]), T, P, Y, "%s reaction %d" % (spec.name, j))
+
+
+# ---------------------------------------------------------------- edge cases
+
+@pytest.mark.parametrize("N", [1, 31, 127, 128, 129, 257])
+def test_ragged_sizes(ck, N):
+    cfg = ckgen.CONFIGS["tiny_1k"]
+    mech = ckgen.mechanism(cfg.mech)
+    T, P, Y = ckgen.states(cfg, N=N)
+    assert_parity(ck, mech, T, P, Y, "N=%d" % N)
+
+
+def test_empty_batch_is_a_noop(ck):
+    mech = ckgen.mechanism(ckgen.MECH_TINY)
+    gm = ck.Mechanism(mech)
+    ck.ck_source_terms(gm.handle, 0, 0, 0, 0, 0, 0)      # N == 0: pointers are not touched
+    gm.close()
+
+
+def test_temperature_at_below_and_across_T_mid(ck):
+    cfg = ckgen.CONFIGS["mid_1m"]
+    mech = ckgen.mechanism(cfg.mech)
+    T, P, Y = ckgen.states(dataclasses.replace(cfg, T_range=(300.0, 1100.0)), N=300)
+    T[:8] = 1000.0                                   # exactly T_mid: low range (reading Q4)
+    T[8:16] = np.nextafter(1000.0, 2000.0)
+    assert_parity(ck, mech, T, P, Y, "T around T_mid")
+
+
+def test_distinct_T_mid_per_species(ck):
+    """Several temperature ranges: the folded equilibrium layer keeps one coefficient row
+    per range delimited by the distinct T_mid values."""
+    cfg = ckgen.CONFIGS["tiny_1k"]
+    mech = ckgen.mechanism(cfg.mech)
+    rng = np.random.default_rng(3)
+    T_mid = rng.choice([800.0, 1000.0, 1400.0, 2000.0], size=mech.n_species)
+    mech = dataclasses.replace(mech, T_mid=T_mid)
+    T, P, Y = ckgen.states(dataclasses.replace(cfg, T_range=(500.0, 2600.0)), N=640)
+    T[:4] = [800.0, 1000.0, 1400.0, 2000.0]
+    assert_parity(ck, mech, T, P, Y, "distinct T_mid")
+
+
+def test_absent_species_and_tiny_mass_fractions(ck):
+    cfg = ckgen.CONFIGS["tiny_1k"]
+    mech = ckgen.mechanism(cfg.mech)
+    T, P, Y = ckgen.states(cfg, N=256)
+    Y = Y.copy()
+    Y[1, :64] = 0.0
+    Y[3, 32:96] = 0.0
+    Y[5, 200:] = 1e-300
+    Y /= Y.sum(0, keepdims=True)
+    assert_parity(ck, mech, T, P, Y, "absent species")
+
+
+def test_irreversible_lindemann_and_real_valued_nu(ck):
+    cfg = ckgen.CONFIGS["tiny_1k"]
+    mech = ckgen.mechanism(cfg.mech)
+    rev = mech.reversible.copy()
+    rev[::3] = 0
+    typ = mech.rxn_type.copy()
+    typ[typ == 3] = 2                                   # Troe -> Lindemann
+    nu_r = mech.nu_reac.copy()
+    k = int(np.flatnonzero(nu_r[:, 1])[0])
+    nu_r[k, 1] = 1.5
+    mech2 = dataclasses.replace(mech, reversible=rev, rxn_type=typ, nu_reac=nu_r)
+    T, P, Y = ckgen.states(cfg, N=200)
+    assert_parity(ck, mech2, T, P, Y, "irreversible/lindemann/real nu")
+    # 3-parameter Troe (T** = +INF)
+    troe = mech.troe.copy()
+    troe[:, 3] = np.inf
+    assert_parity(ck, dataclasses.replace(mech, troe=troe), T, P, Y, "Troe 3-parameter")
+
+
+def test_species_on_both_sides(ck):
+    """A + B -> A + C style reactions: nu' and nu'' overlap, the net list is shorter."""
+    cfg = ckgen.CONFIGS["tiny_1k"]
+    mech = ckgen.mechanism(cfg.mech)
+    nu_r, nu_p = mech.nu_reac.copy(), mech.nu_prod.copy()
+    free = int(np.flatnonzero((nu_r[:, 0] == 0) & (nu_p[:, 0] == 0))[0])
+    nu_r[free, 0] += 1.0
+    nu_p[free, 0] += 1.0
+    assert_parity(ck, dataclasses.replace(mech, nu_reac=nu_r, nu_prod=nu_p),
+                  *ckgen.states(cfg, N=130), label="catalyst species")
+
+
+def test_detailed_balance_on_the_device(ck):
+    """At a constructed equilibrium the net rates vanish to rounding:
+    |wdot_k| <= 1e-10 sum_j |nu_kj| phi_j q_f,j."""
+    mech = ckgen.mechanism(ckgen.MECH_MID)
+    om = oracle.OracleMechanism(mech)
+    S = mech.n_species
+    Ts = np.array([800.0, 1500.0, 2600.0])
+    Ps, Ys, bounds = [], [], []
+    rng = np.random.default_rng(7)
+    for T in Ts:
+        g = oracle.cell_detail(om, T, 1e5, np.full(S, 1.0 / S))["g_RT"]
+        lam = rng.uniform(-3.0, 0.0, size=mech.elem_count.shape[1])
+        lnC = -g + np.log(mech.p_ref / (RU * T)) + mech.elem_count @ lam
+        n_atoms = mech.elem_count.sum(1).astype(float)
+        lo, hi = -200.0, 200.0
+        for _ in range(100):
+            mid = 0.5 * (lo + hi)
+            lo, hi = (mid, hi) if (lnC + mid * n_atoms).max() < np.log(1e-3) else (lo, mid)
+        C = np.exp(lnC + lo * n_atoms)
+        P = C.sum() * RU * T
+        Y = C * mech.mol_weight / (C * mech.mol_weight).sum()
+        det = oracle.cell_detail(om, T, P, Y)
+        phi = np.where(mech.rxn_type == 1, det["M"], 1.0)
+        bounds.append(1e-10 * (np.abs(mech.nu_prod - mech.nu_reac) @ (phi * det["qf"])))
+        Ps.append(P)
+        Ys.append(Y)
+    w, d = gpu_run(ck, mech, Ts, np.array(Ps), np.ascontiguousarray(np.array(Ys).T))
+    assert (np.abs(w) <= np.array(bounds).T + 1e-300).all()
+
+
+def test_deterministic_and_host_entry_point(ck):
+    cfg = ckgen.CONFIGS["mid_1m"]
+    mech = ckgen.mechanism(cfg.mech)
+    T, P, Y = ckgen.states(cfg, N=5000)
+    gm = ck.Mechanism(mech)
+    w1, d1 = gpu_run(ck, mech, T, P, Y, gm)
+    w2, d2 = gpu_run(ck, mech, T, P, Y, gm)
+    assert np.array_equal(w1, w2) and np.array_equal(d1, d2)         # bitwise run to run
+    wh, dh = gm.source_terms_host(T, P, Y)
+    assert np.array_equal(wh, w1) and np.array_equal(dh, d1)         # same kernels, host buffers
+    Tp, Pp, Yp = (torch.from_numpy(a).pin_memory() for a in (T, P, Y))
+    wp = torch.empty((mech.n_species, 5000), dtype=torch.float64).pin_memory()
+    dp = torch.empty(5000, dtype=torch.float64).pin_memory()
+    gm.source_terms_host(Tp, Pp, Yp, wp, dp)
+    assert np.array_equal(wp.numpy(), w1) and np.array_equal(dp.numpy(), d1)
+    gm.close()
+
+
+def test_error_codes(ck):
+    mech = ckgen.mechanism(ckgen.MECH_TINY)
+    gm = ck.Mechanism(mech)
+    with pytest.raises(ck.CkError) as e:
+        ck.ck_source_terms(gm.handle, 0, 0, 0, 16, 0, 0)
+    assert e.value.status == 1
+    with pytest.raises(ck.CkError) as e:
+        ck.ck_source_terms(gm.handle, 8, 8, 8, -1, 8, 8)
+    assert e.value.status == 1
+    with pytest.raises(ck.CkError) as e:
+        ck.ck_source_terms(None, 8, 8, 8, 4, 8, 8)
+    assert e.value.status == 1
+    gm.close()
+    bad = dataclasses.replace(mech, rxn_type=np.full(mech.n_reactions, 9, np.uint8))
+    with pytest.raises(ck.CkError) as e:
+        ck.Mechanism(bad)
+    assert e.value.status == 4
+    bad = dataclasses.replace(mech, mol_weight=-mech.mol_weight)
+    with pytest.raises(ck.CkError) as e:
+        ck.Mechanism(bad)
+    assert e.value.status == 1
