@@ -73,6 +73,12 @@ typedef struct ck_mech_desc {
 /* Validate `desc`, build the device-resident mechanism (sorted reaction program, folded
  * equilibrium-layer coefficients, thermo tables, efficiency matrix) on the current CUDA
  * device and return an opaque handle in *out.  Synchronous.
+ * Kernel variant: by default (environment CK_KERNEL unset or "auto") a kernel specialised
+ * to the mechanism's structure is compiled with NVRTC for sm_100a when the species
+ * accumulators fit in registers (S <= 103), falling back to the generic table-driven kernel
+ * otherwise or if NVRTC is unavailable; CK_KERNEL=generic forces the generic kernel,
+ * CK_KERNEL=jit makes a failed specialisation an error.  Compiled cubins are cached under
+ * $CK_JIT_CACHE (default ~/.cache/ck_jit; empty string disables the cache).
  * Errors: CK_EINVAL (NULL pointers, S/R < 1, W <= 0, negative or non-finite nu, a reaction
  * without reactants or without products, T_mid <= 0, non-positive Troe temperatures,
  * p_ref <= 0), CK_EUNSUPPORTED (unknown rxn_type; S or R beyond the kernels' limits),
@@ -109,7 +115,8 @@ const char *ck_last_error(void);
  * what: 0 S, 1 R, 2 nnz(nu'), 3 nnz(nu''), 4 nnz(nu''-nu'), 5 #three-body, 6 #Lindemann,
  *       7 #Troe, 8 #temperature ranges, 9 threads per block, 10 blocks per SM,
  *       11 dynamic shared memory per block (bytes), 12 kernels launched per
- *       ck_source_terms call, 13 nnz(E) counted over third-body and falloff columns.
+ *       ck_source_terms call, 13 nnz(E) counted over third-body and falloff columns,
+ *       14 kernel variant in use (0 generic table-driven kernel, 1 mechanism-specialised).
  * Returns -1 for a NULL handle or unknown `what`. */
 int64_t ck_mech_info(const ck_mech *m, int what);
 

@@ -12,8 +12,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libck.so")
-SOURCES = ["ck_api.cu", "ck_kernels.cu"]
-HEADERS = ["ck_internal.h", "ck_program.h"]
+SOURCES = ["ck_api.cu", "ck_kernels.cu", "ck_jit.cu"]
+HEADERS = ["ck_internal.h", "ck_program.h", "ck_jit_kernel.cuh"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]
 
@@ -23,12 +23,24 @@ def _newest_source() -> float:
     return max(os.path.getmtime(f) for f in files)
 
 
+def _embed_jit_source() -> None:
+    """ck_jit_kernel.cuh -> ck_jit_source.inc: the kernel text as C++ raw string literals
+    (the text NVRTC compiles at ck_mech_create time)."""
+    text = open(os.path.join(CSRC, "ck_jit_kernel.cuh")).read()
+    assert ')CKJIT"' not in text
+    chunks = [text[i:i + 8000] for i in range(0, len(text), 8000)]
+    with open(os.path.join(CSRC, "ck_jit_source.inc"), "w") as fh:
+        for c in chunks:
+            fh.write('R"CKJIT(' + c + ')CKJIT"\n')
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_source():
         return LIB
+    _embed_jit_source()
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-          ["-o", LIB + ".tmp"] + [os.path.join(CSRC, f) for f in SOURCES]
+          ["-o", LIB + ".tmp"] + [os.path.join(CSRC, f) for f in SOURCES] + ["-ldl"]
     subprocess.run(cmd, check=True, cwd=CSRC)
     os.replace(LIB + ".tmp", LIB)
     return LIB

@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -106,6 +107,71 @@ void gibbs_feature_row(const double *a, double p_ref, long double out[7]) {
   out[6] = (long double)a[5];
 }
 
+// Decides whether to use the specialised kernel (env CK_KERNEL = auto | generic | jit),
+// picks its launch shape, compiles and loads it.  Returns CK_OK also when it falls back to
+// the generic kernel in auto mode (m->jit_note says why).
+int setup_jit(ck_mech *m, ck::JitSpec &spec, const cudaDeviceProp &prop) {
+  const char *mode_env = std::getenv("CK_KERNEL");
+  const std::string mode = mode_env ? mode_env : "auto";
+  if (mode == "generic") { m->jit_note = "CK_KERNEL=generic"; return CK_OK; }
+  if (mode != "auto" && mode != "jit") return fail(CK_EINVAL, "CK_KERNEL must be auto, generic or jit");
+  const bool required = (mode == "jit");
+  auto give_up = [&](const std::string &why) {
+    m->jit_note = why;
+    return required ? fail(CK_EUNSUPPORTED, "CK_KERNEL=jit but " + why) : (int)CK_OK;
+  };
+  const int S = spec.S, R = spec.R;
+  // the accumulators of Eq. 2 need 2 registers per species, plus ~48 for the rest
+  const int regs_needed = 2 * S + 48;
+  if (regs_needed > 255) return give_up("too many species for register-resident accumulators");
+
+  const size_t tab_bytes = (size_t)spec.n_ranges * R * 10 * sizeof(double);
+  const size_t smem_sm = (size_t)prop.sharedMemPerMultiprocessor;      // 228 KB
+  const size_t smem_blk = (size_t)prop.sharedMemPerBlockOptin;         // 227 KB
+  int best_nt = 0, best_b = 0;
+  bool best_tab = false;
+  size_t best_smem = 0;
+  for (int tab_smem = 1; tab_smem >= 0 && best_nt == 0; --tab_smem) {
+    for (int nt : {512, 384, 256, 128}) {
+      for (int b = 1; b <= 4; ++b) {
+        const int regcap = std::min(255, (65536 / (nt * b)) / 8 * 8);
+        if (regcap < regs_needed) continue;
+        const size_t smem = (size_t)S * nt * 8 + 32 * 8 + (tab_smem ? tab_bytes : 0);
+        if (smem > smem_blk || b * (smem + 1024) > smem_sm) continue;
+        if (nt * b > best_nt * best_b || (nt * b == best_nt * best_b && nt > best_nt)) {
+          best_nt = nt; best_b = b; best_tab = tab_smem != 0; best_smem = smem;
+        }
+      }
+    }
+  }
+  if (best_nt == 0) return give_up("no launch shape fits shared memory");
+  spec.threads = best_nt; spec.min_blocks = best_b; spec.tab_in_smem = best_tab;
+
+  const std::string src = ck::jit_generate_source(spec);
+  std::vector<char> cubin;
+  const std::string err = ck::jit_compile(src, &cubin);
+  if (!err.empty()) return give_up(err);
+  cudaError_t ce = cudaLibraryLoadData(&m->jit_lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
+  if (ce != cudaSuccess) return give_up(std::string("cudaLibraryLoadData: ") + cudaGetErrorString(ce));
+  ce = cudaLibraryGetKernel(&m->jit_kernel, m->jit_lib, "ck_source_terms_jit");
+  if (ce == cudaSuccess)
+    ce = cudaKernelSetAttributeForDevice(m->jit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)best_smem, m->device);
+  if (ce != cudaSuccess) {
+    cudaLibraryUnload(m->jit_lib);
+    m->jit_lib = nullptr; m->jit_kernel = nullptr;
+    return give_up(std::string("loading the specialised kernel: ") + cudaGetErrorString(ce));
+  }
+  m->jit_threads = best_nt; m->jit_blocks_per_sm = best_b; m->jit_smem = best_smem;
+  m->jit_grid_max = m->num_sms * best_b;
+  const int n_mb = (spec.n_m + ck::kMBlock - 1) / ck::kMBlock;
+  const size_t elems = (size_t)m->jit_grid_max * std::max(n_mb, 1) * ck::kMBlock * best_nt;
+  ce = cudaMalloc((void **)&m->d_jit_scratch, elems * sizeof(double));
+  if (ce != cudaSuccess) return fail(CK_ENOMEM, std::string("cudaMalloc scratch: ") + cudaGetErrorString(ce));
+  m->jit_params.m_scratch = m->d_jit_scratch;
+  return CK_OK;
+}
+
 }  // namespace
 
 extern "C" const char *ck_last_error(void) { return g_last_error.c_str(); }
@@ -177,6 +243,9 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   std::vector<unsigned char> program;
   std::vector<double> falloff;
   std::vector<int> m_rows;       // reaction index of each row of M
+  ck::JitSpec spec;
+  spec.S = S; spec.R = R; spec.n_ranges = n_ranges;
+  std::vector<double> jit_tab((size_t)n_ranges * R * 10, 0.0);
   for (int j = 0; j < R; ++j) {
     const int type = d->rxn_type ? d->rxn_type[j] : CK_ELEMENTARY;
     const int rev = d->reversible ? (d->reversible[j] != 0) : 1;
@@ -230,6 +299,19 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
       }
       for (int i = 0; i < 7; ++i) dbl.push_back((double)f[i]);
       dbl.push_back(0.0);
+      // row of the specialised kernel's rate table (ck_jit_kernel.cuh)
+      double *row = &jit_tab[((size_t)r * R + j) * 10];
+      row[0] = d->ln_A[j]; row[1] = d->b[j]; row[2] = -d->Ea_over_R[j];
+      row[3] = (double)f[0]; row[4] = (double)f[1]; row[5] = (double)f[6];
+      row[6] = (double)f[2]; row[7] = (double)f[3]; row[8] = (double)f[4]; row[9] = (double)f[5];
+    }
+    {
+      ck::JitReaction jr;
+      jr.index = j; jr.type = type; jr.reversible = rev; jr.m_slot = h.m_slot; jr.fo_idx = h.fo_idx;
+      for (size_t e = 0; e < off_r.size(); ++e) jr.reac.emplace_back(off_r[e], c_r[e]);
+      for (size_t e = 0; e < off_p.size(); ++e) jr.prod.emplace_back(off_p[e], c_p[e]);
+      for (size_t e = 0; e < off_s.size(); ++e) jr.net.emplace_back(off_s[e], c_s[e]);
+      spec.rxn.push_back(std::move(jr));
     }
     dbl.insert(dbl.end(), c_r.begin(), c_r.end());
     dbl.insert(dbl.end(), c_p.begin(), c_p.end());
@@ -271,6 +353,7 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   const size_t o_eff = pk.append(eff.data(), eff.size() * sizeof(double));
   const size_t o_fo = pk.append(falloff.data(), falloff.size() * sizeof(double));
   const size_t o_prog = pk.append(program.data(), program.size());
+  const size_t o_jtab = pk.append(jit_tab.data(), jit_tab.size() * sizeof(double));
   ce = cudaMalloc(&m->d_tables, pk.bytes.size());
   if (ce != cudaSuccess) { delete m; return fail(CK_ENOMEM, std::string("cudaMalloc tables: ") + cudaGetErrorString(ce)); }
   ce = cudaMemcpy(m->d_tables, pk.bytes.data(), pk.bytes.size(), cudaMemcpyHostToDevice);
@@ -290,6 +373,14 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   dm.falloff = (const double *)(base + o_fo);
   dm.program = base + o_prog;
   dm.m_scratch = m->d_scratch;
+
+  // ---- mechanism-specialised kernel (ck_jit.cu); the generic kernel stays as fallback ---
+  spec.n_m = n_m;
+  spec.n_fo = m->n_lindemann + m->n_troe;
+  m->jit_params.inv_W = dm.inv_W; m->jit_params.range_T = dm.range_T; m->jit_params.thermo = dm.thermo;
+  m->jit_params.eff = dm.eff; m->jit_params.falloff = dm.falloff;
+  m->jit_params.tab = (const double *)(base + o_jtab);
+  if (int st = setup_jit(m, spec, prop)) { ck_mech_destroy(m); return st; }
   *out = m;
   return CK_OK;
 }
@@ -299,6 +390,8 @@ extern "C" void ck_mech_destroy(ck_mech *m) {
   if (m->d_tables) cudaFree(m->d_tables);
   if (m->d_scratch) cudaFree(m->d_scratch);
   if (m->d_stage) cudaFree(m->d_stage);
+  if (m->d_jit_scratch) cudaFree(m->d_jit_scratch);
+  if (m->jit_lib) cudaLibraryUnload(m->jit_lib);
   delete m;
 }
 
@@ -311,7 +404,18 @@ extern "C" int ck_source_terms(const ck_mech *m, const double *T, const double *
   if (!T || !P || !Y || !wdot || !dTdt) return fail(CK_EINVAL, "a state or result pointer is NULL");
   if (((uintptr_t)T | (uintptr_t)P | (uintptr_t)Y | (uintptr_t)wdot | (uintptr_t)dTdt) & 7u)
     return fail(CK_EINVAL, "pointers must be 8-byte aligned");
-  cudaError_t ce = ck::launch_source_terms(m, T, P, Y, N, wdot, dTdt, (cudaStream_t)stream);
+  cudaError_t ce;
+  if (m->jit_kernel) {
+    ck::JitParams prm = m->jit_params;
+    prm.T = T; prm.P = P; prm.Y = Y; prm.wdot = wdot; prm.dTdt = dTdt; prm.N = N;
+    const int64_t n_tiles = (N + m->jit_threads - 1) / m->jit_threads;
+    const int grid = (int)std::min<int64_t>(n_tiles, m->jit_grid_max);
+    void *args[] = {&prm};
+    ce = cudaLaunchKernel((const void *)m->jit_kernel, dim3(grid), dim3(m->jit_threads), args,
+                          m->jit_smem, (cudaStream_t)stream);
+  } else {
+    ce = ck::launch_source_terms(m, T, P, Y, N, wdot, dTdt, (cudaStream_t)stream);
+  }
   if (ce != cudaSuccess) return fail_cuda(ce, "ck_source_terms launch");
   return CK_OK;
 }
@@ -358,11 +462,12 @@ extern "C" int64_t ck_mech_info(const ck_mech *m, int what) {
     case 6: return m->n_lindemann;
     case 7: return m->n_troe;
     case 8: return m->dev.n_ranges;
-    case 9: return m->dev.threads;
-    case 10: return m->blocks_per_sm;
-    case 11: return (int64_t)m->smem_bytes;
+    case 9: return m->jit_kernel ? m->jit_threads : m->dev.threads;
+    case 10: return m->jit_kernel ? m->jit_blocks_per_sm : m->blocks_per_sm;
+    case 11: return (int64_t)(m->jit_kernel ? m->jit_smem : m->smem_bytes);
     case 12: return 1;
     case 13: return m->nnz_eff;
+    case 14: return m->jit_kernel ? 1 : 0;
     default: return -1;
   }
 }

@@ -5,9 +5,39 @@
 
 #include <cstdint>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "ck_program.h"
+
+namespace ck {
+
+// Kernel argument of the mechanism-specialised kernel; must match CkParams in
+// ck_jit_kernel.cuh field for field.
+struct JitParams {
+  const double *inv_W, *range_T, *thermo, *eff, *falloff, *tab;
+  double *m_scratch;
+  const double *T, *P, *Y;
+  double *wdot, *dTdt;
+  long long N;
+};
+
+struct JitReaction {
+  int index = 0, type = 0, reversible = 1, m_slot = -1, fo_idx = -1;
+  std::vector<std::pair<int, double>> reac, prod, net;   // (species, coefficient)
+};
+
+struct JitSpec {
+  int S = 0, R = 0, threads = 0, min_blocks = 1, n_ranges = 1, n_m = 0, n_fo = 0;
+  bool tab_in_smem = true;
+  std::vector<JitReaction> rxn;
+};
+
+std::string jit_generate_source(const JitSpec &spec);
+// Compiles to a cubin for sm_100a with NVRTC; returns "" on success, else the error text.
+std::string jit_compile(const std::string &src, std::vector<char> *cubin);
+
+}  // namespace ck
 
 struct ck_mech {
   ck::DeviceMech dev{};       // device pointers + sizes, passed to the kernel by value
@@ -22,6 +52,14 @@ struct ck_mech {
   // one device allocation holding every table; m_scratch separately
   void *d_tables = nullptr;
   double *d_scratch = nullptr;
+  // mechanism-specialised kernel (NULL kernel => the generic kernel is used)
+  cudaLibrary_t jit_lib = nullptr;
+  cudaKernel_t jit_kernel = nullptr;
+  ck::JitParams jit_params{};
+  int jit_threads = 0, jit_blocks_per_sm = 0, jit_grid_max = 0;
+  size_t jit_smem = 0;
+  double *d_jit_scratch = nullptr;
+  std::string jit_note;       // why the specialised kernel is not in use, if so
   // staging for ck_source_terms_host
   double *d_stage = nullptr;
   int64_t stage_cells = 0;

@@ -1,0 +1,197 @@
+// ck_jit.cu -- run-time specialisation of the fused kernel to one mechanism.
+//
+// generate_source() writes the unrolled reaction list (ck_reactions) for the mechanism
+// into the hand-written kernel text of ck_jit_kernel.cuh; NVRTC compiles it for sm_100a;
+// the CUDA runtime's library API loads the cubin.  NVRTC is opened with dlopen so that
+// libck.so itself has no link-time dependency on it (the library must load, and report
+// errors through the ABI, on machines without NVRTC or without a GPU).
+#include <cuda_runtime.h>
+#include <dlfcn.h>
+#include <nvrtc.h>
+#include <sys/stat.h>
+#include <unistd.h>
+
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <fstream>
+#include <sstream>
+#include <string>
+#include <vector>
+
+#include "ck_internal.h"
+
+namespace ck {
+
+namespace {
+
+const char *kKernelText =
+#include "ck_jit_source.inc"
+    ;
+
+struct Nvrtc {
+  void *handle = nullptr;
+  decltype(&nvrtcCreateProgram) CreateProgram = nullptr;
+  decltype(&nvrtcCompileProgram) CompileProgram = nullptr;
+  decltype(&nvrtcDestroyProgram) DestroyProgram = nullptr;
+  decltype(&nvrtcGetCUBINSize) GetCUBINSize = nullptr;
+  decltype(&nvrtcGetCUBIN) GetCUBIN = nullptr;
+  decltype(&nvrtcGetProgramLogSize) GetProgramLogSize = nullptr;
+  decltype(&nvrtcGetProgramLog) GetProgramLog = nullptr;
+  decltype(&nvrtcGetErrorString) GetErrorString = nullptr;
+  decltype(&nvrtcVersion) Version = nullptr;
+  bool ok = false;
+};
+
+Nvrtc &nvrtc() {
+  static Nvrtc n = [] {
+    Nvrtc r;
+    const char *names[] = {"libnvrtc.so.12", "libnvrtc.so", "/usr/local/cuda/lib64/libnvrtc.so.12",
+                           "/usr/local/cuda/lib64/libnvrtc.so"};
+    for (const char *nm : names) {
+      r.handle = dlopen(nm, RTLD_NOW | RTLD_LOCAL);
+      if (r.handle) break;
+    }
+    if (!r.handle) return r;
+#define CK_SYM(f) r.f = (decltype(r.f))dlsym(r.handle, "nvrtc" #f)
+    CK_SYM(CreateProgram); CK_SYM(CompileProgram); CK_SYM(DestroyProgram); CK_SYM(GetCUBINSize);
+    CK_SYM(GetCUBIN); CK_SYM(GetProgramLogSize); CK_SYM(GetProgramLog); CK_SYM(GetErrorString);
+    CK_SYM(Version);
+#undef CK_SYM
+    r.ok = r.CreateProgram && r.CompileProgram && r.DestroyProgram && r.GetCUBINSize && r.GetCUBIN &&
+           r.GetProgramLogSize && r.GetProgramLog && r.GetErrorString && r.Version;
+    return r;
+  }();
+  return n;
+}
+
+std::string lit(double v) {
+  char buf[40];
+  std::snprintf(buf, sizeof buf, "%.17g", v);
+  std::string s(buf);
+  if (s.find_first_of(".eEni") == std::string::npos) s += ".0";
+  return s;
+}
+
+void gather(std::ostringstream &o, const char *acc, int k, double c) {
+  if (c == 1.0)
+    o << "    " << acc << " += CK_LNC(" << k << ");\n";
+  else
+    o << "    " << acc << " = fma(" << lit(c) << ", CK_LNC(" << k << "), " << acc << ");\n";
+}
+
+uint64_t fnv1a(const std::string &s, uint64_t h) {
+  for (unsigned char c : s) { h ^= c; h *= 1099511628211ull; }
+  return h;
+}
+
+std::string cache_dir() {
+  const char *e = std::getenv("CK_JIT_CACHE");
+  if (e && !*e) return "";            // CK_JIT_CACHE="" disables the cache
+  std::string d = e ? e : "";
+  if (d.empty()) {
+    const char *home = std::getenv("HOME");
+    d = std::string(home ? home : "/tmp") + "/.cache/ck_jit";
+  }
+  ::mkdir((d.substr(0, d.find_last_of('/'))).c_str(), 0755);
+  ::mkdir(d.c_str(), 0755);
+  return d;
+}
+
+}  // namespace
+
+std::string jit_generate_source(const JitSpec &s) {
+  std::ostringstream o;
+  o << "#define CK_S " << s.S << "\n#define CK_R " << s.R << "\n#define CK_NT " << s.threads
+    << "\n#define CK_MINB " << s.min_blocks << "\n#define CK_NRANGES " << s.n_ranges
+    << "\n#define CK_NM " << s.n_m << "\n#define CK_NMB " << (s.n_m + kMBlock - 1) / kMBlock
+    << "\n#define CK_NFO " << s.n_fo << "\n#define CK_TAB_SMEM " << (s.tab_in_smem ? 1 : 0) << "\n";
+  const std::string text(kKernelText);
+  const std::string marker = "//@@CK_GENERATED_REACTIONS@@";
+  const size_t at = text.find(marker);
+  o << text.substr(0, at);
+  o << "__device__ __forceinline__ void ck_reactions(const CkCtx &x, double (&w)[CK_S]) {\n";
+  for (size_t j = 0; j < s.rxn.size(); ++j) {
+    const JitReaction &r = s.rxn[j];
+    o << "  {  // reaction " << r.index << "\n    const double lkf = CK_LNKF(" << j << ");\n    double lf = lkf;\n";
+    for (size_t e = 0; e < r.reac.size(); ++e) gather(o, "lf", r.reac[e].first, r.reac[e].second);
+    if (r.reversible) {
+      o << "    double lr = CK_LNKR(" << j << ");\n";
+      for (size_t e = 0; e < r.prod.size(); ++e) gather(o, "lr", r.prod[e].first, r.prod[e].second);
+      o << "    double q = CK_EXP(lf) - CK_EXP(lr);\n";
+    } else {
+      o << "    double q = CK_EXP(lf);\n";
+    }
+    if (r.type == 1)
+      o << "    q *= CK_M(" << r.m_slot << ");\n";
+    else if (r.type >= 2)
+      o << "    q *= CK_FALLOFF(" << r.fo_idx << ", lkf, CK_M(" << r.m_slot << "));\n";
+    for (size_t e = 0; e < r.net.size(); ++e) {
+      const int k = r.net[e].first;
+      const double c = r.net[e].second;
+      if (c == 1.0) o << "    w[" << k << "] += q;\n";
+      else if (c == -1.0) o << "    w[" << k << "] -= q;\n";
+      else o << "    w[" << k << "] = fma(" << lit(c) << ", q, w[" << k << "]);\n";
+    }
+    o << "  }\n";
+  }
+  o << "}\n";
+  o << text.substr(at + marker.size());
+  return o.str();
+}
+
+// Compiles `src` to a cubin for sm_100a.  Returns "" on success, else an error message.
+std::string jit_compile(const std::string &src, std::vector<char> *cubin) {
+  Nvrtc &n = nvrtc();
+  if (!n.ok) return "NVRTC (libnvrtc.so.12) could not be loaded";
+  int major = 0, minor = 0;
+  n.Version(&major, &minor);
+
+  // cubin cache keyed by the source text and the NVRTC version
+  std::string path;
+  const std::string dir = cache_dir();
+  if (!dir.empty()) {
+    char name[96];
+    const uint64_t h1 = fnv1a(src, 1469598103934665603ull), h2 = fnv1a(src, 0x9E3779B97F4A7C15ull);
+    std::snprintf(name, sizeof name, "/ck_%016llx%016llx_nvrtc%d_%d.cubin", (unsigned long long)h1,
+                  (unsigned long long)h2, major, minor);
+    path = dir + name;
+    std::ifstream in(path, std::ios::binary);
+    if (in) {
+      cubin->assign(std::istreambuf_iterator<char>(in), std::istreambuf_iterator<char>());
+      if (!cubin->empty()) return "";
+    }
+  }
+
+  nvrtcProgram prog;
+  nvrtcResult rc = n.CreateProgram(&prog, src.c_str(), "ck_source_terms_jit.cu", 0, nullptr, nullptr);
+  if (rc != NVRTC_SUCCESS) return std::string("nvrtcCreateProgram: ") + n.GetErrorString(rc);
+  const char *opts[] = {"--gpu-architecture=sm_100a", "--std=c++17", "-lineinfo", "--fmad=true"};
+  rc = n.CompileProgram(prog, (int)(sizeof opts / sizeof opts[0]), opts);
+  if (rc != NVRTC_SUCCESS) {
+    size_t ls = 0;
+    n.GetProgramLogSize(prog, &ls);
+    std::string log(ls, '\0');
+    if (ls) n.GetProgramLog(prog, &log[0]);
+    n.DestroyProgram(&prog);
+    return std::string("nvrtcCompileProgram: ") + n.GetErrorString(rc) + "\n" + log;
+  }
+  size_t sz = 0;
+  rc = n.GetCUBINSize(prog, &sz);
+  if (rc == NVRTC_SUCCESS) {
+    cubin->resize(sz);
+    rc = n.GetCUBIN(prog, cubin->data());
+  }
+  n.DestroyProgram(&prog);
+  if (rc != NVRTC_SUCCESS) return std::string("nvrtcGetCUBIN: ") + n.GetErrorString(rc);
+  if (!path.empty()) {
+    const std::string tmp = path + ".tmp" + std::to_string((long)getpid());
+    std::ofstream out(tmp, std::ios::binary);
+    out.write(cubin->data(), (std::streamsize)cubin->size());
+    out.close();
+    if (out) std::rename(tmp.c_str(), path.c_str());
+  }
+  return "";
+}
+
+}  // namespace ck

@@ -23,6 +23,20 @@ def ck():
     return ck
 
 
+@pytest.fixture(autouse=True, params=["auto", "generic"])
+def kernel_variant(request, monkeypatch):
+    """Every test runs twice: with the mechanism-specialised (NVRTC) kernel that
+    ck_mech_create picks by default, and with the generic table-driven kernel."""
+    monkeypatch.setenv("CK_KERNEL", request.param)
+    return request.param
+
+
+def test_variant_selection(ck, kernel_variant):
+    for spec in (ckgen.MECH_TINY, ckgen.MECH_MID):
+        with ck.Mechanism(ckgen.mechanism(spec)) as gm:
+            assert gm.info("jit") == (1 if kernel_variant == "auto" else 0)
+
+
 def gpu_run(ck, mech, T, P, Y, gm=None):
     """T, P, Y numpy -> (wdot[S,N], dTdt[N]) numpy via ck_source_terms on device buffers."""
     own = gm is None
