@@ -120,6 +120,13 @@ const char *ck_last_error(void);
  * Returns -1 for a NULL handle or unknown `what`. */
 int64_t ck_mech_info(const ck_mech *m, int what);
 
+/* The CUDA source of the mechanism-specialised kernel ck_mech_create would compile for
+ * `desc` on a B200 (generated reaction list inside the hand-written kernel text of
+ * csrc/ck_jit_kernel.cuh).  Needs no GPU.  Writes at most cap bytes (NUL terminated) to
+ * buf (may be NULL) and returns the size needed including the NUL, or -1 if the
+ * description is invalid or the mechanism cannot be specialised (see ck_last_error()). */
+int64_t ck_mech_jit_source(const ck_mech_desc *desc, char *buf, int64_t cap);
+
 /* Measured FP64 FMA throughput of the current device, in FMA instructions (thread level)
  * per second: a register-resident DFMA loop on every SM, timed with CUDA events on
  * `stream`.  Used as the roofline denominator for this FP64-pipe-bound path.

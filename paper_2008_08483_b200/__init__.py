@@ -22,6 +22,7 @@ from . import _build
 
 __all__ = ["Mechanism", "CkError", "ck_mech_create", "ck_source_terms", "ck_source_terms_host",
            "ck_mech_destroy", "ck_last_error", "ck_mech_info", "ck_measure_fp64_peak",
+           "ck_mech_jit_source",
            "library_path", "RU", "INFO"]
 
 RU = 8314.46261815324  # J/(kmol K), the constant compiled into the kernels
@@ -71,6 +72,8 @@ def _load():
     lib.ck_last_error.argtypes = []
     lib.ck_mech_info.restype = C.c_int64
     lib.ck_mech_info.argtypes = [C.c_void_p, C.c_int]
+    lib.ck_mech_jit_source.restype = C.c_int64
+    lib.ck_mech_jit_source.argtypes = [C.POINTER(_Desc), C.c_char_p, C.c_int64]
     lib.ck_measure_fp64_peak.restype = C.c_int
     lib.ck_measure_fp64_peak.argtypes = [_dp, C.c_void_p]
     return lib
@@ -125,6 +128,18 @@ def ck_mech_destroy(handle) -> None:
 
 def ck_mech_info(handle, what) -> int:
     return int(_lib.ck_mech_info(handle, INFO[what] if isinstance(what, str) else int(what)))
+
+
+def ck_mech_jit_source(mech) -> str:
+    """Generated CUDA source of the specialised kernel for `mech` (needs no GPU)."""
+    desc, keep = make_desc(mech)
+    n = _lib.ck_mech_jit_source(C.byref(desc), None, 0)
+    if n < 0:
+        raise CkError(4, _lib.ck_last_error().decode())
+    buf = C.create_string_buffer(n)
+    _lib.ck_mech_jit_source(C.byref(desc), buf, n)
+    del keep
+    return buf.value.decode()
 
 
 def ck_measure_fp64_peak(stream=0) -> float:

@@ -107,115 +107,22 @@ void gibbs_feature_row(const double *a, double p_ref, long double out[7]) {
   out[6] = (long double)a[5];
 }
 
-// Decides whether to use the specialised kernel (env CK_KERNEL = auto | generic | jit),
-// picks its launch shape, compiles and loads it.  Returns CK_OK also when it falls back to
-// the generic kernel in auto mode (m->jit_note says why).
-int setup_jit(ck_mech *m, ck::JitSpec &spec, const cudaDeviceProp &prop) {
-  const char *mode_env = std::getenv("CK_KERNEL");
-  const std::string mode = mode_env ? mode_env : "auto";
-  if (mode == "generic") { m->jit_note = "CK_KERNEL=generic"; return CK_OK; }
-  if (mode != "auto" && mode != "jit") return fail(CK_EINVAL, "CK_KERNEL must be auto, generic or jit");
-  const bool required = (mode == "jit");
-  auto give_up = [&](const std::string &why) {
-    m->jit_note = why;
-    return required ? fail(CK_EUNSUPPORTED, "CK_KERNEL=jit but " + why) : (int)CK_OK;
-  };
-  const int S = spec.S, R = spec.R;
-  // the accumulators of Eq. 2 need 2 registers per species, plus ~48 for the rest
-  const int regs_needed = 2 * S + 48;
-  if (regs_needed > 255) return give_up("too many species for register-resident accumulators");
+// Everything ck_mech_create derives from the description on the host (no CUDA calls).
+struct HostBuild {
+  int n_ranges = 1, n_m = 0, n_mb = 0;
+  std::vector<double> range_T, inv_W, thermo, eff, eff_frag, falloff, jit_tab;
+  std::vector<unsigned char> program;
+  ck::JitSpec spec;
+  int64_t nnz_reac = 0, nnz_prod = 0, nnz_net = 0, nnz_eff = 0;
+  int n_three_body = 0, n_lindemann = 0, n_troe = 0;
+};
 
-  const size_t tab_bytes = (size_t)spec.n_ranges * R * 10 * sizeof(double);
-  const size_t smem_sm = (size_t)prop.sharedMemPerMultiprocessor;      // 228 KB
-  const size_t smem_blk = (size_t)prop.sharedMemPerBlockOptin;         // 227 KB
-  int best_nt = 0, best_b = 0;
-  bool best_tab = false;
-  size_t best_smem = 0;
-  for (int tab_smem = 1; tab_smem >= 0 && best_nt == 0; --tab_smem) {
-    for (int nt : {512, 384, 256, 128}) {
-      for (int b = 1; b <= 4; ++b) {
-        const int regcap = std::min(255, (65536 / (nt * b)) / 8 * 8);
-        if (regcap < regs_needed) continue;
-        const size_t smem = (size_t)S * nt * 8 + 32 * 8 + (tab_smem ? tab_bytes : 0);
-        if (smem > smem_blk || b * (smem + 1024) > smem_sm) continue;
-        if (nt * b > best_nt * best_b || (nt * b == best_nt * best_b && nt > best_nt)) {
-          best_nt = nt; best_b = b; best_tab = tab_smem != 0; best_smem = smem;
-        }
-      }
-    }
-  }
-  if (best_nt == 0) return give_up("no launch shape fits shared memory");
-  spec.threads = best_nt; spec.min_blocks = best_b; spec.tab_in_smem = best_tab;
-
-  const std::string src = ck::jit_generate_source(spec);
-  std::vector<char> cubin;
-  const std::string err = ck::jit_compile(src, &cubin);
-  if (!err.empty()) return give_up(err);
-  cudaError_t ce = cudaLibraryLoadData(&m->jit_lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
-  if (ce != cudaSuccess) return give_up(std::string("cudaLibraryLoadData: ") + cudaGetErrorString(ce));
-  ce = cudaLibraryGetKernel(&m->jit_kernel, m->jit_lib, "ck_source_terms_jit");
-  if (ce == cudaSuccess)
-    ce = cudaKernelSetAttributeForDevice(m->jit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)best_smem, m->device);
-  if (ce != cudaSuccess) {
-    cudaLibraryUnload(m->jit_lib);
-    m->jit_lib = nullptr; m->jit_kernel = nullptr;
-    return give_up(std::string("loading the specialised kernel: ") + cudaGetErrorString(ce));
-  }
-  m->jit_threads = best_nt; m->jit_blocks_per_sm = best_b; m->jit_smem = best_smem;
-  m->jit_grid_max = m->num_sms * best_b;
-  const int n_mb = (spec.n_m + ck::kMBlock - 1) / ck::kMBlock;
-  const size_t elems = (size_t)m->jit_grid_max * std::max(n_mb, 1) * ck::kMBlock * best_nt;
-  ce = cudaMalloc((void **)&m->d_jit_scratch, elems * sizeof(double));
-  if (ce != cudaSuccess) return fail(CK_ENOMEM, std::string("cudaMalloc scratch: ") + cudaGetErrorString(ce));
-  m->jit_params.m_scratch = m->d_jit_scratch;
-  return CK_OK;
-}
-
-}  // namespace
-
-extern "C" const char *ck_last_error(void) { return g_last_error.c_str(); }
-
-extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
-  if (!out) return fail(CK_EINVAL, "out is NULL");
-  *out = nullptr;
-  if (int st = validate(d)) return st;
+void build_host(const ck_mech_desc *d, HostBuild *hb) {
   const int S = d->n_species, R = d->n_reactions;
-
-  ck_mech *m = new (std::nothrow) ck_mech();
-  if (!m) return fail(CK_ENOMEM, "host allocation failed");
-  cudaError_t ce = cudaGetDevice(&m->device);
-  if (ce != cudaSuccess) { delete m; return fail_cuda(ce, "cudaGetDevice"); }
-  cudaDeviceProp prop;
-  ce = cudaGetDeviceProperties(&prop, m->device);
-  if (ce != cudaSuccess) { delete m; return fail_cuda(ce, "cudaGetDeviceProperties"); }
-  m->num_sms = prop.multiProcessorCount;
-
-  // ---- launch shape: as many resident cells per SM as shared memory allows ----------
-  int best_threads = 0, best_bps = 0;
-  size_t best_smem = 0;
-  for (int threads : {128, 64, 32}) {
-    size_t smem = (size_t)2 * S * threads * sizeof(double);
-    if (smem > (size_t)prop.sharedMemPerBlockOptin) continue;
-    int bps = 0;
-    ce = ck::kernel_configure(threads, smem, &bps);
-    if (ce != cudaSuccess) { delete m; return fail_cuda(ce, "kernel_configure"); }
-    if (bps * threads > best_bps * best_threads) {
-      best_threads = threads; best_bps = bps; best_smem = smem;
-    }
-  }
-  if (best_threads == 0) {
-    delete m;
-    return fail(CK_EUNSUPPORTED, "n_species too large for the shared-memory resident kernel");
-  }
-  ce = ck::kernel_configure(best_threads, best_smem, &best_bps);   // leave the attribute set
-  if (ce != cudaSuccess) { delete m; return fail_cuda(ce, "kernel_configure"); }
-  m->blocks_per_sm = best_bps;
-  m->smem_bytes = best_smem;
-  m->grid_max = m->num_sms * best_bps;
-
+  HostBuild *m = hb;   // statistics are accumulated on the same names as in ck_mech
   // ---- temperature ranges from the distinct T_mid values --------------
-  std::vector<double> range_T(d->T_mid, d->T_mid + S);
+  std::vector<double> &range_T = hb->range_T;
+  range_T.assign(d->T_mid, d->T_mid + S);
   std::sort(range_T.begin(), range_T.end());
   range_T.erase(std::unique(range_T.begin(), range_T.end()), range_T.end());
   const int n_ranges = (int)range_T.size() + 1;
@@ -224,7 +131,9 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
     rank[k] = (int)(std::lower_bound(range_T.begin(), range_T.end(), d->T_mid[k]) - range_T.begin());
 
   // ---- per-species tables -------------------------------------------------------------
-  std::vector<double> inv_W(S), thermo((size_t)S * ck::kThermoStride, 0.0);
+  std::vector<double> &inv_W = hb->inv_W, &thermo = hb->thermo;
+  inv_W.assign(S, 0.0);
+  thermo.assign((size_t)S * ck::kThermoStride, 0.0);
   std::vector<long double> gfeat((size_t)S * 2 * 7);
   for (int k = 0; k < S; ++k) {
     inv_W[k] = 1.0 / d->mol_weight[k];
@@ -240,12 +149,13 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   }
 
   // ---- reaction program ------------------------------------------------------------------
-  std::vector<unsigned char> program;
-  std::vector<double> falloff;
+  std::vector<unsigned char> &program = hb->program;
+  std::vector<double> &falloff = hb->falloff;
   std::vector<int> m_rows;       // reaction index of each row of M
-  ck::JitSpec spec;
+  ck::JitSpec &spec = hb->spec;
   spec.S = S; spec.R = R; spec.n_ranges = n_ranges;
-  std::vector<double> jit_tab((size_t)n_ranges * R * 10, 0.0);
+  std::vector<double> &jit_tab = hb->jit_tab;
+  jit_tab.assign((size_t)n_ranges * R * 10, 0.0);
   for (int j = 0; j < R; ++j) {
     const int type = d->rxn_type ? d->rxn_type[j] : CK_ELEMENTARY;
     const int rev = d->reversible ? (d->reversible[j] != 0) : 1;
@@ -277,7 +187,8 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
                                         (double)type};
       if (type == CK_TROE) {
         const double *t = d->troe + 4 * (size_t)j;
-        row[3] = t[0]; row[4] = -1.0 / t[1]; row[5] = -1.0 / t[2]; row[6] = -t[3];
+        row[3] = t[0]; row[4] = -1.0 / t[1]; row[5] = -1.0 / t[2];
+        row[6] = std::isinf(t[3]) ? -1e300 : -t[3];   // exp(-T**/T) -> 0 for T** = +INF
         m->n_troe++;
       } else {
         m->n_lindemann++;
@@ -335,15 +246,176 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   // ---- third-body efficiency matrix, blocked for the register-tiled M = C E -----------
   const int n_m = (int)m_rows.size();
   const int n_mb = (n_m + ck::kMBlock - 1) / ck::kMBlock;
-  std::vector<double> eff((size_t)std::max(n_mb, 1) * S * ck::kMBlock, 0.0);
+  std::vector<double> &eff = hb->eff;
+  eff.assign((size_t)std::max(n_mb, 1) * S * ck::kMBlock, 0.0);
   for (int s = 0; s < n_m; ++s) {
     const int j = m_rows[s];
     for (int k = 0; k < S; ++k)
       eff[((size_t)(s / ck::kMBlock) * S + k) * ck::kMBlock + (s % ck::kMBlock)] =
           d->eff ? d->eff[(size_t)k * R + j] : 1.0;
   }
+  // the same matrix as DMMA.8x8x4 B fragments: [n-tile][k-step][lane], lane holds
+  // E[4 ks + lane%4][8 nt + lane/4], zero padded in both directions
+  const int k_steps = (S + 3) / 4;
+  std::vector<double> &eff_frag = hb->eff_frag;
+  eff_frag.assign((size_t)std::max(n_mb, 1) * k_steps * 32, 0.0);
+  for (int nt = 0; nt < n_mb; ++nt)
+    for (int ks = 0; ks < k_steps; ++ks)
+      for (int lane = 0; lane < 32; ++lane) {
+        const int k = 4 * ks + lane % 4, s_row = 8 * nt + lane / 4;
+        if (k < S && s_row < n_m)
+          eff_frag[((size_t)nt * k_steps + ks) * 32 + lane] =
+              d->eff ? d->eff[(size_t)k * R + m_rows[s_row]] : 1.0;
+      }
+  spec.inv_W = inv_W; spec.range_T = range_T; spec.thermo = thermo; spec.falloff = falloff;
   if (falloff.empty()) falloff.resize(ck::kFalloffStride, 0.0);
   if (range_T.empty()) range_T.push_back(0.0);
+
+  spec.n_m = n_m;
+  spec.n_fo = hb->n_lindemann + hb->n_troe;
+  hb->n_ranges = n_ranges; hb->n_m = n_m; hb->n_mb = n_mb;
+}
+
+// B200 (sm_100a) per-SM resources, used when the launch shape has to be chosen without a
+// device (ck_mech_jit_source on a build box)
+constexpr size_t kSmemPerSm = 233472, kSmemPerBlock = 232448;
+
+// Launch shape of the specialised kernel: as many resident threads as registers
+// (2 per species accumulator + ~48) and shared memory (ln C columns + rate tables) allow.
+// Returns "" and fills spec.threads / min_blocks / tab_in_smem, or the reason it cannot.
+std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk, size_t *smem_out) {
+  const int S = spec.S, R = spec.R;
+  const int regs_needed = 2 * S + 48;
+  if (regs_needed > 255) return "too many species for register-resident accumulators";
+  const size_t tab_bytes = (size_t)spec.n_ranges * R * 10 * sizeof(double);
+  int best_nt = 0, best_b = 0;
+  bool best_tab = false;
+  size_t best_smem = 0;
+  const char *nt_env = std::getenv("CK_JIT_NT");   // tuning knob: force the block size
+  const int nt_forced = nt_env ? std::atoi(nt_env) : 0;
+  for (int tab_smem = 1; tab_smem >= 0 && best_nt == 0; --tab_smem) {
+    for (int nt : {512, 448, 384, 320, 256, 192, 128}) {
+      if (nt_forced && nt != nt_forced) continue;
+      for (int b = 1; b <= 4; ++b) {
+        const int regcap = std::min(255, (65536 / (nt * b)) / 8 * 8);
+        if (regcap < regs_needed) continue;
+        const size_t smem = (size_t)S * (nt + 8) * 8 + 32 * 8 + (tab_smem ? tab_bytes : 0);
+        if (smem > smem_blk || b * (smem + 1024) > smem_sm) continue;
+        if (nt * b > best_nt * best_b || (nt * b == best_nt * best_b && nt > best_nt)) {
+          best_nt = nt; best_b = b; best_tab = tab_smem != 0; best_smem = smem;
+        }
+      }
+    }
+  }
+  if (best_nt == 0) return "no launch shape fits shared memory";
+  spec.threads = best_nt; spec.min_blocks = best_b; spec.tab_in_smem = best_tab;
+  // tuning knobs for A/B runs under ncu (defaults are the measured best)
+  if (const char *e = std::getenv("CK_JIT_M")) spec.m_dmma = std::string(e) != "dfma";
+  if (const char *e = std::getenv("CK_JIT_SYNC")) spec.sync_every = std::atoi(e);
+  *smem_out = best_smem;
+  return "";
+}
+
+// Decides whether to use the specialised kernel (env CK_KERNEL = auto | generic | jit),
+// compiles and loads it.  Returns CK_OK also when it falls back to the generic kernel in
+// auto mode (m->jit_note says why).
+int setup_jit(ck_mech *m, ck::JitSpec &spec, const cudaDeviceProp &prop) {
+  const char *mode_env = std::getenv("CK_KERNEL");
+  const std::string mode = mode_env ? mode_env : "auto";
+  if (mode == "generic") { m->jit_note = "CK_KERNEL=generic"; return CK_OK; }
+  if (mode != "auto" && mode != "jit") return fail(CK_EINVAL, "CK_KERNEL must be auto, generic or jit");
+  const bool required = (mode == "jit");
+  auto give_up = [&](const std::string &why) {
+    m->jit_note = why;
+    return required ? fail(CK_EUNSUPPORTED, "CK_KERNEL=jit but " + why) : (int)CK_OK;
+  };
+  size_t smem = 0;
+  const std::string why = choose_jit_shape(spec, (size_t)prop.sharedMemPerMultiprocessor,
+                                           (size_t)prop.sharedMemPerBlockOptin, &smem);
+  if (!why.empty()) return give_up(why);
+
+  const std::string src = ck::jit_generate_source(spec);
+  if (const char *e = std::getenv("CK_JIT_DUMP")) {
+    if (FILE *f = std::fopen(e, "w")) {
+      std::fwrite(src.data(), 1, src.size(), f);
+      std::fclose(f);
+    }
+  }
+  std::vector<char> cubin;
+  const std::string err = ck::jit_compile(src, &cubin);
+  if (!err.empty()) return give_up(err);
+  cudaError_t ce = cudaLibraryLoadData(&m->jit_lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
+  if (ce != cudaSuccess) return give_up(std::string("cudaLibraryLoadData: ") + cudaGetErrorString(ce));
+  ce = cudaLibraryGetKernel(&m->jit_kernel, m->jit_lib, "ck_source_terms_jit");
+  if (ce == cudaSuccess)
+    ce = cudaKernelSetAttributeForDevice(m->jit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)smem, m->device);
+  if (ce != cudaSuccess) {
+    cudaLibraryUnload(m->jit_lib);
+    m->jit_lib = nullptr; m->jit_kernel = nullptr;
+    return give_up(std::string("loading the specialised kernel: ") + cudaGetErrorString(ce));
+  }
+  m->jit_threads = spec.threads; m->jit_blocks_per_sm = spec.min_blocks; m->jit_smem = smem;
+  m->jit_grid_max = m->num_sms * spec.min_blocks;
+  const int n_mb = (spec.n_m + ck::kMBlock - 1) / ck::kMBlock;
+  const size_t elems = (size_t)m->jit_grid_max * std::max(n_mb, 1) * ck::kMBlock * spec.threads;
+  ce = cudaMalloc((void **)&m->d_jit_scratch, elems * sizeof(double));
+  if (ce != cudaSuccess) return fail(CK_ENOMEM, std::string("cudaMalloc scratch: ") + cudaGetErrorString(ce));
+  m->jit_params.m_scratch = m->d_jit_scratch;
+  return CK_OK;
+}
+
+}  // namespace
+
+extern "C" const char *ck_last_error(void) { return g_last_error.c_str(); }
+
+extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
+  if (!out) return fail(CK_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (int st = validate(d)) return st;
+  const int S = d->n_species, R = d->n_reactions;
+
+  ck_mech *m = new (std::nothrow) ck_mech();
+  if (!m) return fail(CK_ENOMEM, "host allocation failed");
+  cudaError_t ce = cudaGetDevice(&m->device);
+  if (ce != cudaSuccess) { delete m; return fail_cuda(ce, "cudaGetDevice"); }
+  cudaDeviceProp prop;
+  ce = cudaGetDeviceProperties(&prop, m->device);
+  if (ce != cudaSuccess) { delete m; return fail_cuda(ce, "cudaGetDeviceProperties"); }
+  m->num_sms = prop.multiProcessorCount;
+
+  // ---- launch shape: as many resident cells per SM as shared memory allows ----------
+  int best_threads = 0, best_bps = 0;
+  size_t best_smem = 0;
+  for (int threads : {128, 64, 32}) {
+    size_t smem = (size_t)2 * S * threads * sizeof(double);
+    if (smem > (size_t)prop.sharedMemPerBlockOptin) continue;
+    int bps = 0;
+    ce = ck::kernel_configure(threads, smem, &bps);
+    if (ce != cudaSuccess) { delete m; return fail_cuda(ce, "kernel_configure"); }
+    if (bps * threads > best_bps * best_threads) {
+      best_threads = threads; best_bps = bps; best_smem = smem;
+    }
+  }
+  if (best_threads == 0) {
+    delete m;
+    return fail(CK_EUNSUPPORTED, "n_species too large for the shared-memory resident kernel");
+  }
+  ce = ck::kernel_configure(best_threads, best_smem, &best_bps);   // leave the attribute set
+  if (ce != cudaSuccess) { delete m; return fail_cuda(ce, "kernel_configure"); }
+  m->blocks_per_sm = best_bps;
+  m->smem_bytes = best_smem;
+  m->grid_max = m->num_sms * best_bps;
+
+  HostBuild hb;
+  build_host(d, &hb);
+  const int n_ranges = hb.n_ranges, n_m = hb.n_m, n_mb = hb.n_mb;
+  m->nnz_reac = hb.nnz_reac; m->nnz_prod = hb.nnz_prod; m->nnz_net = hb.nnz_net; m->nnz_eff = hb.nnz_eff;
+  m->n_three_body = hb.n_three_body; m->n_lindemann = hb.n_lindemann; m->n_troe = hb.n_troe;
+  std::vector<double> &inv_W = hb.inv_W, &range_T = hb.range_T, &thermo = hb.thermo, &eff = hb.eff,
+                      &eff_frag = hb.eff_frag, &falloff = hb.falloff, &jit_tab = hb.jit_tab;
+  std::vector<unsigned char> &program = hb.program;
+  ck::JitSpec &spec = hb.spec;
 
   // ---- one device allocation for all tables -------------------------------------------
   Packer pk;
@@ -354,6 +426,7 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   const size_t o_fo = pk.append(falloff.data(), falloff.size() * sizeof(double));
   const size_t o_prog = pk.append(program.data(), program.size());
   const size_t o_jtab = pk.append(jit_tab.data(), jit_tab.size() * sizeof(double));
+  const size_t o_efrag = pk.append(eff_frag.data(), eff_frag.size() * sizeof(double));
   ce = cudaMalloc(&m->d_tables, pk.bytes.size());
   if (ce != cudaSuccess) { delete m; return fail(CK_ENOMEM, std::string("cudaMalloc tables: ") + cudaGetErrorString(ce)); }
   ce = cudaMemcpy(m->d_tables, pk.bytes.data(), pk.bytes.size(), cudaMemcpyHostToDevice);
@@ -375,10 +448,8 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   dm.m_scratch = m->d_scratch;
 
   // ---- mechanism-specialised kernel (ck_jit.cu); the generic kernel stays as fallback ---
-  spec.n_m = n_m;
-  spec.n_fo = m->n_lindemann + m->n_troe;
-  m->jit_params.inv_W = dm.inv_W; m->jit_params.range_T = dm.range_T; m->jit_params.thermo = dm.thermo;
-  m->jit_params.eff = dm.eff; m->jit_params.falloff = dm.falloff;
+  m->jit_params.eff = dm.eff;
+  m->jit_params.eff_frag = (const double *)(base + o_efrag);
   m->jit_params.tab = (const double *)(base + o_jtab);
   if (int st = setup_jit(m, spec, prop)) { ck_mech_destroy(m); return st; }
   *out = m;
@@ -470,6 +541,22 @@ extern "C" int64_t ck_mech_info(const ck_mech *m, int what) {
     case 14: return m->jit_kernel ? 1 : 0;
     default: return -1;
   }
+}
+
+extern "C" int64_t ck_mech_jit_source(const ck_mech_desc *d, char *buf, int64_t cap) {
+  if (validate(d)) return -1;
+  HostBuild hb;
+  build_host(d, &hb);
+  size_t smem = 0;
+  const std::string why = choose_jit_shape(hb.spec, kSmemPerSm, kSmemPerBlock, &smem);
+  if (!why.empty()) { fail(CK_EUNSUPPORTED, why); return -1; }
+  const std::string src = ck::jit_generate_source(hb.spec);
+  if (buf && cap > 0) {
+    const size_t n = std::min((size_t)cap - 1, src.size());
+    std::memcpy(buf, src.data(), n);
+    buf[n] = '\0';
+  }
+  return (int64_t)src.size() + 1;
 }
 
 extern "C" int ck_measure_fp64_peak(double *fma_per_s, void *stream) {

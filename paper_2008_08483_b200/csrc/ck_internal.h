@@ -15,7 +15,7 @@ namespace ck {
 // Kernel argument of the mechanism-specialised kernel; must match CkParams in
 // ck_jit_kernel.cuh field for field.
 struct JitParams {
-  const double *inv_W, *range_T, *thermo, *eff, *falloff, *tab;
+  const double *eff, *eff_frag, *tab;
   double *m_scratch;
   const double *T, *P, *Y;
   double *wdot, *dTdt;
@@ -30,7 +30,10 @@ struct JitReaction {
 struct JitSpec {
   int S = 0, R = 0, threads = 0, min_blocks = 1, n_ranges = 1, n_m = 0, n_fo = 0;
   bool tab_in_smem = true;
+  bool m_dmma = true;          // M = C E on DMMA.8x8x4 (else register-tiled DFMA)
+  int sync_every = 8;          // block barrier every n reactions (0 = never)
   std::vector<JitReaction> rxn;
+  std::vector<double> inv_W, range_T, thermo, falloff;   // constant-bank tables
 };
 
 std::string jit_generate_source(const JitSpec &spec);

@@ -105,7 +105,18 @@ std::string jit_generate_source(const JitSpec &s) {
   o << "#define CK_S " << s.S << "\n#define CK_R " << s.R << "\n#define CK_NT " << s.threads
     << "\n#define CK_MINB " << s.min_blocks << "\n#define CK_NRANGES " << s.n_ranges
     << "\n#define CK_NM " << s.n_m << "\n#define CK_NMB " << (s.n_m + kMBlock - 1) / kMBlock
-    << "\n#define CK_NFO " << s.n_fo << "\n#define CK_TAB_SMEM " << (s.tab_in_smem ? 1 : 0) << "\n";
+    << "\n#define CK_NFO " << s.n_fo << "\n#define CK_TAB_SMEM " << (s.tab_in_smem ? 1 : 0)
+    << "\n#define CK_M_DMMA " << (s.m_dmma ? 1 : 0) << "\n#define CK_SYNC_EVERY " << s.sync_every << "\n";
+  auto emit = [&](const char *name, const std::vector<double> &v) {
+    o << "__constant__ double " << name << "[" << (v.empty() ? 1 : v.size()) << "] = {";
+    for (size_t i = 0; i < v.size(); ++i) o << (i ? "," : "") << (i % 6 == 0 ? "\n  " : " ") << lit(v[i]);
+    if (v.empty()) o << "0.0";
+    o << "};\n";
+  };
+  emit("ck_c_invW", s.inv_W);
+  emit("ck_c_rangeT", s.range_T);
+  emit("ck_c_thermo", s.thermo);
+  emit("ck_c_falloff", s.falloff);
   const std::string text(kKernelText);
   const std::string marker = "//@@CK_GENERATED_REACTIONS@@";
   const size_t at = text.find(marker);
@@ -134,6 +145,7 @@ std::string jit_generate_source(const JitSpec &s) {
       else o << "    w[" << k << "] = fma(" << lit(c) << ", q, w[" << k << "]);\n";
     }
     o << "  }\n";
+    if (s.sync_every > 0 && (j + 1) % s.sync_every == 0 && j + 1 < s.rxn.size()) o << "  CK_SYNC();\n";
   }
   o << "}\n";
   o << text.substr(at + marker.size());

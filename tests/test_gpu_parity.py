@@ -135,7 +135,7 @@ def test_single_reaction_mechanisms(ck, spec):
 
 # ---------------------------------------------------------------- edge cases
 
-@pytest.mark.parametrize("N", [1, 31, 127, 128, 129, 257])
+@pytest.mark.parametrize("N", [1, 31, 127, 128, 129, 257, 383, 384, 385, 769])
 def test_ragged_sizes(ck, N):
     cfg = ckgen.CONFIGS["tiny_1k"]
     mech = ckgen.mechanism(cfg.mech)
