@@ -111,11 +111,108 @@ void gibbs_feature_row(const double *a, double p_ref, long double out[7]) {
 struct HostBuild {
   int n_ranges = 1, n_m = 0, n_mb = 0;
   std::vector<double> range_T, inv_W, thermo, eff, eff_frag, falloff, jit_tab;
+  int jit_n_m = 0;            // rows of M in the specialised kernel's (padded) order
+  int n_ranges_tmp = 1;
+  std::vector<double> jit_eff;
   std::vector<unsigned char> program;
   ck::JitSpec spec;
   int64_t nnz_reac = 0, nnz_prod = 0, nnz_net = 0, nnz_eff = 0;
   int n_three_body = 0, n_lindemann = 0, n_troe = 0;
 };
+
+// The specialised kernel walks the reactions in blocks of kJitBlock that are homogeneous
+// in (type, reversible): a compact, instruction-cache resident "core" evaluates the rate
+// layers of a whole block (Eq. 4, 6, 7, 11 and Sec. 2.4), and only the gathers / scatters
+// of each block are unique generated code.  Here the reactions are sorted into those
+// (blocks of 4 reactions by default)
+// groups, every group is padded to whole blocks with null reactions (rate ~ 0, no species),
+// and the rate table, falloff table and efficiency fragments are laid out in that order.
+
+void finalize_jit(const ck_mech_desc *d, HostBuild *hb, const std::vector<double> &falloff_orig) {
+  const int S = d->n_species, R = d->n_reactions;
+  ck::JitSpec &spec = hb->spec;
+  const int n_ranges = hb->n_ranges_tmp;
+  std::vector<ck::JitReaction> orig;
+  orig.swap(spec.rxn);
+  const std::vector<double> tab_orig = hb->jit_tab;
+
+  int kJitBlock = 4;                      // tuning knob CK_JIT_B (2..8)
+  if (const char *e = std::getenv("CK_JIT_B")) kJitBlock = std::min(8, std::max(1, std::atoi(e)));
+  auto group_of = [](const ck::JitReaction &r) {
+    const int t = r.type == 0 ? 0 : (r.type == 1 ? 1 : 2);
+    return 2 * t + (r.reversible ? 0 : 1);
+  };
+  std::vector<int> order;                 // original reaction index, or -1 for a null reaction
+  spec.block = kJitBlock;
+  for (int g = 0; g < 6; ++g) {
+    for (int j = 0; j < R; ++j)
+      if (group_of(orig[j]) == g) order.push_back(j);
+    while (order.size() % kJitBlock) order.push_back(-1);
+    spec.group_end[g] = (int)order.size() / kJitBlock;
+  }
+  const int RP = (int)order.size();
+  spec.R = RP;
+  hb->jit_tab.assign((size_t)n_ranges * RP * 10, 0.0);
+  spec.falloff.clear();
+  std::vector<int> m_rows;                // original reaction of each M row (-1: null)
+  for (int jj = 0; jj < RP; ++jj) {
+    const int j = order[jj];
+    const int g = [&] { int gg = 0; while (jj / kJitBlock >= spec.group_end[gg]) ++gg; return gg; }();
+    ck::JitReaction r;
+    if (j >= 0) r = orig[j];
+    r.index = j;
+    r.type = g / 2 == 0 ? 0 : (g / 2 == 1 ? 1 : (j >= 0 ? orig[j].type : 2));
+    r.reversible = (g % 2 == 0);
+    for (int rg = 0; rg < n_ranges; ++rg) {
+      double *row = &hb->jit_tab[((size_t)rg * RP + jj) * 10];
+      if (j >= 0) {
+        const double *src = &tab_orig[((size_t)rg * R + j) * 10];
+        for (int i = 0; i < 10; ++i) row[i] = src[i];
+      } else {
+        row[0] = -5000.0;   // null reaction: ln q = -5000, the rate underflows to ~1e-307
+        row[3] = -5000.0;
+      }
+    }
+    if (g >= 2) {           // third-body and falloff reactions: a row of M each, in this order
+      r.m_slot = (int)m_rows.size();
+      m_rows.push_back(j);
+    }
+    if (g >= 4) {           // falloff rows in this order (null: Lindemann with k0 tiny)
+      r.fo_idx = (int)(spec.falloff.size() / ck::kFalloffStride);
+      if (j >= 0) {
+        const double *src = &falloff_orig[(size_t)orig[j].fo_idx * ck::kFalloffStride];
+        spec.falloff.insert(spec.falloff.end(), src, src + ck::kFalloffStride);
+      } else {
+        const double row[ck::kFalloffStride] = {-100.0, 0, 0, 0, 0, 0, 0, 2.0};
+        spec.falloff.insert(spec.falloff.end(), row, row + ck::kFalloffStride);
+      }
+    }
+    spec.rxn.push_back(std::move(r));
+  }
+  // E as DMMA.8x8x4 B fragments: [n-tile][k-step][lane], lane holds
+  // E[4 ks + lane%4][8 nt + lane/4], zero padded in both directions
+  const int n_m = (int)m_rows.size();
+  const int n_mb = (n_m + 7) / 8, k_steps = (S + 3) / 4;
+  hb->jit_n_m = n_m;
+  spec.n_m = n_m;
+  spec.n_fo = (int)(spec.falloff.size() / ck::kFalloffStride);
+  hb->eff_frag.assign((size_t)std::max(n_mb, 1) * k_steps * 32, 0.0);
+  for (int nt = 0; nt < n_mb; ++nt)
+    for (int ks = 0; ks < k_steps; ++ks)
+      for (int lane = 0; lane < 32; ++lane) {
+        const int k = 4 * ks + lane % 4, row = 8 * nt + lane / 4;
+        if (k < S && row < n_m && m_rows[row] >= 0)
+          hb->eff_frag[((size_t)nt * k_steps + ks) * 32 + lane] =
+              d->eff ? d->eff[(size_t)k * R + m_rows[row]] : 1.0;
+      }
+  // the DFMA variant's layout [block of 8 rows][species][8]
+  hb->jit_eff.assign((size_t)std::max(n_mb, 1) * S * 8, 0.0);
+  for (int row = 0; row < n_m; ++row)
+    if (m_rows[row] >= 0)
+      for (int k = 0; k < S; ++k)
+        hb->jit_eff[((size_t)(row / 8) * S + k) * 8 + row % 8] =
+            d->eff ? d->eff[(size_t)k * R + m_rows[row]] : 1.0;
+}
 
 void build_host(const ck_mech_desc *d, HostBuild *hb) {
   const int S = d->n_species, R = d->n_reactions;
@@ -254,25 +351,12 @@ void build_host(const ck_mech_desc *d, HostBuild *hb) {
       eff[((size_t)(s / ck::kMBlock) * S + k) * ck::kMBlock + (s % ck::kMBlock)] =
           d->eff ? d->eff[(size_t)k * R + j] : 1.0;
   }
-  // the same matrix as DMMA.8x8x4 B fragments: [n-tile][k-step][lane], lane holds
-  // E[4 ks + lane%4][8 nt + lane/4], zero padded in both directions
-  const int k_steps = (S + 3) / 4;
-  std::vector<double> &eff_frag = hb->eff_frag;
-  eff_frag.assign((size_t)std::max(n_mb, 1) * k_steps * 32, 0.0);
-  for (int nt = 0; nt < n_mb; ++nt)
-    for (int ks = 0; ks < k_steps; ++ks)
-      for (int lane = 0; lane < 32; ++lane) {
-        const int k = 4 * ks + lane % 4, s_row = 8 * nt + lane / 4;
-        if (k < S && s_row < n_m)
-          eff_frag[((size_t)nt * k_steps + ks) * 32 + lane] =
-              d->eff ? d->eff[(size_t)k * R + m_rows[s_row]] : 1.0;
-      }
-  spec.inv_W = inv_W; spec.range_T = range_T; spec.thermo = thermo; spec.falloff = falloff;
+  spec.inv_W = inv_W; spec.range_T = range_T; spec.thermo = thermo;
+  hb->n_ranges_tmp = n_ranges;
+  finalize_jit(d, hb, falloff);
   if (falloff.empty()) falloff.resize(ck::kFalloffStride, 0.0);
   if (range_T.empty()) range_T.push_back(0.0);
 
-  spec.n_m = n_m;
-  spec.n_fo = hb->n_lindemann + hb->n_troe;
   hb->n_ranges = n_ranges; hb->n_m = n_m; hb->n_mb = n_mb;
 }
 
@@ -287,7 +371,7 @@ std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk,
   const int S = spec.S, R = spec.R;
   const int regs_needed = 2 * S + 48;
   if (regs_needed > 255) return "too many species for register-resident accumulators";
-  const size_t tab_bytes = (size_t)spec.n_ranges * R * 10 * sizeof(double);
+  const size_t tab_bytes = (size_t)spec.n_ranges * R * 10 * sizeof(double);   // R includes padding
   int best_nt = 0, best_b = 0;
   bool best_tab = false;
   size_t best_smem = 0;
@@ -427,6 +511,7 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   const size_t o_prog = pk.append(program.data(), program.size());
   const size_t o_jtab = pk.append(jit_tab.data(), jit_tab.size() * sizeof(double));
   const size_t o_efrag = pk.append(eff_frag.data(), eff_frag.size() * sizeof(double));
+  const size_t o_jeff = pk.append(hb.jit_eff.data(), hb.jit_eff.size() * sizeof(double));
   ce = cudaMalloc(&m->d_tables, pk.bytes.size());
   if (ce != cudaSuccess) { delete m; return fail(CK_ENOMEM, std::string("cudaMalloc tables: ") + cudaGetErrorString(ce)); }
   ce = cudaMemcpy(m->d_tables, pk.bytes.data(), pk.bytes.size(), cudaMemcpyHostToDevice);
@@ -448,7 +533,7 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   dm.m_scratch = m->d_scratch;
 
   // ---- mechanism-specialised kernel (ck_jit.cu); the generic kernel stays as fallback ---
-  m->jit_params.eff = dm.eff;
+  m->jit_params.eff = (const double *)(base + o_jeff);
   m->jit_params.eff_frag = (const double *)(base + o_efrag);
   m->jit_params.tab = (const double *)(base + o_jtab);
   if (int st = setup_jit(m, spec, prop)) { ck_mech_destroy(m); return st; }

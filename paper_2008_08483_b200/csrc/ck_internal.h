@@ -31,7 +31,9 @@ struct JitSpec {
   int S = 0, R = 0, threads = 0, min_blocks = 1, n_ranges = 1, n_m = 0, n_fo = 0;
   bool tab_in_smem = true;
   bool m_dmma = true;          // M = C E on DMMA.8x8x4 (else register-tiled DFMA)
-  int sync_every = 8;          // block barrier every n reactions (0 = never)
+  int sync_every = 0;          // block barrier every n reaction blocks (0 = never)
+  int block = 4;               // reactions per block of the core
+  int group_end[6] = {0, 0, 0, 0, 0, 0};   // end block of (elementary, three-body, falloff) x (rev, irrev)
   std::vector<JitReaction> rxn;
   std::vector<double> inv_W, range_T, thermo, falloff;   // constant-bank tables
 };

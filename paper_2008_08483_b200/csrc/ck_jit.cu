@@ -73,11 +73,17 @@ std::string lit(double v) {
   return s;
 }
 
-void gather(std::ostringstream &o, const char *acc, int k, double c) {
-  if (c == 1.0)
-    o << "    " << acc << " += CK_LNC(" << k << ");\n";
-  else
-    o << "    " << acc << " = fma(" << lit(c) << ", CK_LNC(" << k << "), " << acc << ");\n";
+// nu^T ln C of one side of a reaction as an expression: sums and fmas of CK_LNC(k)
+std::string gather_expr(const std::vector<std::pair<int, double>> &side) {
+  if (side.empty()) return "0.0";
+  std::string e;
+  for (size_t i = 0; i < side.size(); ++i) {
+    const std::string c = "CK_LNC(" + std::to_string(side[i].first) + ")";
+    const double nu = side[i].second;
+    if (i == 0) e = (nu == 1.0) ? c : (lit(nu) + " * " + c);
+    else e = (nu == 1.0) ? (e + " + " + c) : ("fma(" + lit(nu) + ", " + c + ", " + e + ")");
+  }
+  return e;
 }
 
 uint64_t fnv1a(const std::string &s, uint64_t h) {
@@ -106,7 +112,9 @@ std::string jit_generate_source(const JitSpec &s) {
     << "\n#define CK_MINB " << s.min_blocks << "\n#define CK_NRANGES " << s.n_ranges
     << "\n#define CK_NM " << s.n_m << "\n#define CK_NMB " << (s.n_m + kMBlock - 1) / kMBlock
     << "\n#define CK_NFO " << s.n_fo << "\n#define CK_TAB_SMEM " << (s.tab_in_smem ? 1 : 0)
-    << "\n#define CK_M_DMMA " << (s.m_dmma ? 1 : 0) << "\n#define CK_SYNC_EVERY " << s.sync_every << "\n";
+    << "\n#define CK_M_DMMA " << (s.m_dmma ? 1 : 0) << "\n#define CK_SYNC_EVERY " << s.sync_every
+    << "\n#define CK_B " << s.block << "\n#define CK_NBLK " << (int)s.rxn.size() / s.block
+    << "\n#define CK_G_TB0 " << s.group_end[1] << "\n#define CK_G_FO0 " << s.group_end[3] << "\n";
   auto emit = [&](const char *name, const std::vector<double> &v) {
     o << "__constant__ double " << name << "[" << (v.empty() ? 1 : v.size()) << "] = {";
     for (size_t i = 0; i < v.size(); ++i) o << (i ? "," : "") << (i % 6 == 0 ? "\n  " : " ") << lit(v[i]);
@@ -121,33 +129,50 @@ std::string jit_generate_source(const JitSpec &s) {
   const std::string marker = "//@@CK_GENERATED_REACTIONS@@";
   const size_t at = text.find(marker);
   o << text.substr(0, at);
-  o << "__device__ __forceinline__ void ck_reactions(const CkCtx &x, double (&w)[CK_S]) {\n";
-  for (size_t j = 0; j < s.rxn.size(); ++j) {
-    const JitReaction &r = s.rxn[j];
-    o << "  {  // reaction " << r.index << "\n    const double lkf = CK_LNKF(" << j << ");\n    double lf = lkf;\n";
-    for (size_t e = 0; e < r.reac.size(); ++e) gather(o, "lf", r.reac[e].first, r.reac[e].second);
-    if (r.reversible) {
-      o << "    double lr = CK_LNKR(" << j << ");\n";
-      for (size_t e = 0; e < r.prod.size(); ++e) gather(o, "lr", r.prod[e].first, r.prod[e].second);
-      o << "    double q = CK_EXP(lf) - CK_EXP(lr);\n";
-    } else {
-      o << "    double q = CK_EXP(lf);\n";
+  const int B = s.block, nblk = (int)s.rxn.size() / B;
+  o << "__device__ __forceinline__ void ck_reactions(const CkCtx &x, double (&w)[CK_S]) {\n"
+    << "#pragma unroll 1\n  for (int blk = 0; blk < CK_NBLK; ++blk) {\n"
+    << "    double gf[CK_B], gr[CK_B], q[CK_B];\n    switch (blk) {  // gathers: nu'^T ln C, nu''^T ln C\n";
+  for (int k = 0; k < nblk; ++k) {
+    o << "      case " << k << ":\n";
+    for (int b = 0; b < B; ++b) {
+      const JitReaction &r = s.rxn[(size_t)k * B + b];
+      o << "        gf[" << b << "] = " << gather_expr(r.reac) << ";";
+      if (r.index >= 0) o << "  // reaction " << r.index;
+      o << "\n        gr[" << b << "] = " << (r.reversible ? gather_expr(r.prod) : std::string("0.0")) << ";\n";
     }
-    if (r.type == 1)
-      o << "    q *= CK_M(" << r.m_slot << ");\n";
-    else if (r.type >= 2)
-      o << "    q *= CK_FALLOFF(" << r.fo_idx << ", lkf, CK_M(" << r.m_slot << "));\n";
-    for (size_t e = 0; e < r.net.size(); ++e) {
-      const int k = r.net[e].first;
-      const double c = r.net[e].second;
-      if (c == 1.0) o << "    w[" << k << "] += q;\n";
-      else if (c == -1.0) o << "    w[" << k << "] -= q;\n";
-      else o << "    w[" << k << "] = fma(" << lit(c) << ", q, w[" << k << "]);\n";
-    }
-    o << "  }\n";
-    if (s.sync_every > 0 && (j + 1) % s.sync_every == 0 && j + 1 < s.rxn.size()) o << "  CK_SYNC();\n";
+    o << "        break;\n";
   }
-  o << "}\n";
+  o << "    }\n";
+  const char *names[6] = {"ck_core<0, 1>", "ck_core<0, 0>", "ck_core<1, 1>", "ck_core<1, 0>",
+                          "ck_core<2, 1>", "ck_core<2, 0>"};
+  bool first = true;
+  for (int g = 0; g < 6; ++g) {
+    const int lo = g ? s.group_end[g - 1] : 0;
+    if (s.group_end[g] == lo) continue;
+    o << "    " << (first ? "if" : "else if") << " (blk < " << s.group_end[g] << ") " << names[g]
+      << "(x, blk, gf, gr, q);\n";
+    first = false;
+  }
+  o << "    switch (blk) {  // scatters: w[k] += nu_k q (Eq. 2)\n";
+  for (int k = 0; k < nblk; ++k) {
+    o << "      case " << k << ":\n";
+    for (int b = 0; b < B; ++b) {
+      const JitReaction &r = s.rxn[(size_t)k * B + b];
+      for (size_t e = 0; e < r.net.size(); ++e) {
+        const int sp = r.net[e].first;
+        const double c = r.net[e].second;
+        if (c == 1.0) o << "        w[" << sp << "] += q[" << b << "];\n";
+        else if (c == -1.0) o << "        w[" << sp << "] -= q[" << b << "];\n";
+        else o << "        w[" << sp << "] = fma(" << lit(c) << ", q[" << b << "], w[" << sp << "]);\n";
+      }
+    }
+    o << "        break;\n";
+  }
+  o << "    }\n";
+  if (s.sync_every > 0)
+    o << "    if (blk % " << s.sync_every << " == " << s.sync_every - 1 << ") __syncthreads();\n";
+  o << "  }\n}\n";
   o << text.substr(at + marker.size());
   return o.str();
 }
