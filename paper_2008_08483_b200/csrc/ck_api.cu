@@ -114,6 +114,8 @@ struct HostBuild {
   int jit_n_m = 0;            // rows of M in the specialised kernel's (padded) order
   int n_ranges_tmp = 1;
   std::vector<double> jit_eff;
+  std::vector<double> jit_thermo;   // [n_ranges][S][12], the NASA-7 set holding in each range
+  std::vector<double> jit_logtab;   // [128][2]: 1/c_i, ln c_i (ck_log in ck_jit_kernel.cuh)
   std::vector<unsigned char> program;
   ck::JitSpec spec;
   int64_t nnz_reac = 0, nnz_prod = 0, nnz_net = 0, nnz_eff = 0;
@@ -192,9 +194,10 @@ void finalize_jit(const ck_mech_desc *d, HostBuild *hb, const std::vector<double
   // E as DMMA.8x8x4 B fragments: [n-tile][k-step][lane], lane holds
   // E[4 ks + lane%4][8 nt + lane/4], zero padded in both directions
   const int n_m = (int)m_rows.size();
-  const int n_mb = (n_m + 7) / 8, k_steps = (S + 3) / 4;
+  const int n_mb = ((n_m + 7) / 8 + 1) & ~1, k_steps = (S + 3) / 4;   // pairs of n-tiles
   hb->jit_n_m = n_m;
   spec.n_m = n_m;
+  spec.n_mb = n_mb;
   spec.n_fo = (int)(spec.falloff.size() / ck::kFalloffStride);
   hb->eff_frag.assign((size_t)std::max(n_mb, 1) * k_steps * 32, 0.0);
   for (int nt = 0; nt < n_mb; ++nt)
@@ -351,7 +354,30 @@ void build_host(const ck_mech_desc *d, HostBuild *hb) {
       eff[((size_t)(s / ck::kMBlock) * S + k) * ck::kMBlock + (s % ck::kMBlock)] =
           d->eff ? d->eff[(size_t)k * R + j] : 1.0;
   }
-  spec.inv_W = inv_W; spec.range_T = range_T; spec.thermo = thermo;
+  spec.inv_W = inv_W; spec.range_T = range_T;
+  // NASA-7 rows per temperature range: species k is on its high set in range r iff r > rank[k]
+  hb->jit_thermo.assign((size_t)n_ranges * S * 12, 0.0);
+  for (int r = 0; r < n_ranges; ++r)
+    for (int k = 0; k < S; ++k) {
+      const double *a = (r > rank[k]) ? d->nasa_hi + 7 * k : d->nasa_lo + 7 * k;
+      double *row = &hb->jit_thermo[((size_t)r * S + k) * 12];
+      for (int i = 0; i < 5; ++i) { row[i] = a[i]; row[6 + i] = a[i] / (i + 1); }
+      row[11] = a[5];
+    }
+  // ln table: interval i covers m in [lo_i, lo_i + width) on the hi-word grid from 0x3fe6a000
+  hb->jit_logtab.assign(256, 0.0);
+  for (int i = 0; i < 128; ++i) {
+    auto from_hi = [](uint32_t hi) {
+      const uint64_t bits = (uint64_t)hi << 32;
+      double v;
+      std::memcpy(&v, &bits, sizeof v);
+      return v;
+    };
+    const double lo = from_hi(0x3fe6a000u + (uint32_t)i * 8192u), hi = from_hi(0x3fe6a000u + (uint32_t)(i + 1) * 8192u);
+    const double inv_c = 1.0 / (0.5 * (lo + hi));
+    hb->jit_logtab[2 * i] = inv_c;
+    hb->jit_logtab[2 * i + 1] = (double)(-logl((long double)inv_c));
+  }
   hb->n_ranges_tmp = n_ranges;
   finalize_jit(d, hb, falloff);
   if (falloff.empty()) falloff.resize(ck::kFalloffStride, 0.0);
@@ -383,7 +409,8 @@ std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk,
       for (int b = 1; b <= 4; ++b) {
         const int regcap = std::min(255, (65536 / (nt * b)) / 8 * 8);
         if (regcap < regs_needed) continue;
-        const size_t smem = (size_t)S * (nt + 8) * 8 + 32 * 8 + (tab_smem ? tab_bytes : 0);
+        const size_t smem = (size_t)S * (nt + 8) * 8 + (32 + 256) * 8 +
+                            (size_t)spec.n_ranges * S * 12 * 8 + (tab_smem ? tab_bytes : 0);
         if (smem > smem_blk || b * (smem + 1024) > smem_sm) continue;
         if (nt * b > best_nt * best_b || (nt * b == best_nt * best_b && nt > best_nt)) {
           best_nt = nt; best_b = b; best_tab = tab_smem != 0; best_smem = smem;
@@ -441,8 +468,7 @@ int setup_jit(ck_mech *m, ck::JitSpec &spec, const cudaDeviceProp &prop) {
   }
   m->jit_threads = spec.threads; m->jit_blocks_per_sm = spec.min_blocks; m->jit_smem = smem;
   m->jit_grid_max = m->num_sms * spec.min_blocks;
-  const int n_mb = (spec.n_m + ck::kMBlock - 1) / ck::kMBlock;
-  const size_t elems = (size_t)m->jit_grid_max * std::max(n_mb, 1) * ck::kMBlock * spec.threads;
+  const size_t elems = (size_t)m->jit_grid_max * std::max(spec.n_mb, 1) * ck::kMBlock * spec.threads;
   ce = cudaMalloc((void **)&m->d_jit_scratch, elems * sizeof(double));
   if (ce != cudaSuccess) return fail(CK_ENOMEM, std::string("cudaMalloc scratch: ") + cudaGetErrorString(ce));
   m->jit_params.m_scratch = m->d_jit_scratch;
@@ -512,6 +538,8 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   const size_t o_jtab = pk.append(jit_tab.data(), jit_tab.size() * sizeof(double));
   const size_t o_efrag = pk.append(eff_frag.data(), eff_frag.size() * sizeof(double));
   const size_t o_jeff = pk.append(hb.jit_eff.data(), hb.jit_eff.size() * sizeof(double));
+  const size_t o_jthermo = pk.append(hb.jit_thermo.data(), hb.jit_thermo.size() * sizeof(double));
+  const size_t o_jlog = pk.append(hb.jit_logtab.data(), hb.jit_logtab.size() * sizeof(double));
   ce = cudaMalloc(&m->d_tables, pk.bytes.size());
   if (ce != cudaSuccess) { delete m; return fail(CK_ENOMEM, std::string("cudaMalloc tables: ") + cudaGetErrorString(ce)); }
   ce = cudaMemcpy(m->d_tables, pk.bytes.data(), pk.bytes.size(), cudaMemcpyHostToDevice);
@@ -536,6 +564,8 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   m->jit_params.eff = (const double *)(base + o_jeff);
   m->jit_params.eff_frag = (const double *)(base + o_efrag);
   m->jit_params.tab = (const double *)(base + o_jtab);
+  m->jit_params.thermo = (const double *)(base + o_jthermo);
+  m->jit_params.logtab = (const double *)(base + o_jlog);
   if (int st = setup_jit(m, spec, prop)) { ck_mech_destroy(m); return st; }
   *out = m;
   return CK_OK;

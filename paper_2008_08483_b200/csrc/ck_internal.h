@@ -15,7 +15,7 @@ namespace ck {
 // Kernel argument of the mechanism-specialised kernel; must match CkParams in
 // ck_jit_kernel.cuh field for field.
 struct JitParams {
-  const double *eff, *eff_frag, *tab;
+  const double *eff, *eff_frag, *tab, *thermo, *logtab;
   double *m_scratch;
   const double *T, *P, *Y;
   double *wdot, *dTdt;
@@ -29,13 +29,14 @@ struct JitReaction {
 
 struct JitSpec {
   int S = 0, R = 0, threads = 0, min_blocks = 1, n_ranges = 1, n_m = 0, n_fo = 0;
+  int n_mb = 0;                // blocks of 8 rows of M, padded to an even count
   bool tab_in_smem = true;
   bool m_dmma = true;          // M = C E on DMMA.8x8x4 (else register-tiled DFMA)
   int sync_every = 0;          // block barrier every n reaction blocks (0 = never)
   int block = 4;               // reactions per block of the core
   int group_end[6] = {0, 0, 0, 0, 0, 0};   // end block of (elementary, three-body, falloff) x (rev, irrev)
   std::vector<JitReaction> rxn;
-  std::vector<double> inv_W, range_T, thermo, falloff;   // constant-bank tables
+  std::vector<double> inv_W, range_T, falloff;   // constant-bank tables
 };
 
 std::string jit_generate_source(const JitSpec &spec);

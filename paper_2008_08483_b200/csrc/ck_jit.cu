@@ -110,7 +110,7 @@ std::string jit_generate_source(const JitSpec &s) {
   std::ostringstream o;
   o << "#define CK_S " << s.S << "\n#define CK_R " << s.R << "\n#define CK_NT " << s.threads
     << "\n#define CK_MINB " << s.min_blocks << "\n#define CK_NRANGES " << s.n_ranges
-    << "\n#define CK_NM " << s.n_m << "\n#define CK_NMB " << (s.n_m + kMBlock - 1) / kMBlock
+    << "\n#define CK_NM " << s.n_m << "\n#define CK_NMB " << s.n_mb
     << "\n#define CK_NFO " << s.n_fo << "\n#define CK_TAB_SMEM " << (s.tab_in_smem ? 1 : 0)
     << "\n#define CK_M_DMMA " << (s.m_dmma ? 1 : 0) << "\n#define CK_SYNC_EVERY " << s.sync_every
     << "\n#define CK_B " << s.block << "\n#define CK_NBLK " << (int)s.rxn.size() / s.block
@@ -123,24 +123,41 @@ std::string jit_generate_source(const JitSpec &s) {
   };
   emit("ck_c_invW", s.inv_W);
   emit("ck_c_rangeT", s.range_T);
-  emit("ck_c_thermo", s.thermo);
   emit("ck_c_falloff", s.falloff);
   const std::string text(kKernelText);
   const std::string marker = "//@@CK_GENERATED_REACTIONS@@";
   const size_t at = text.find(marker);
   o << text.substr(0, at);
   const int B = s.block, nblk = (int)s.rxn.size() / B;
+  // One switch case per loop trip: the scatters of the previous block (Eq. 2) and the
+  // gathers of this one (Eq. 4), so that the unique code is walked in address order with one
+  // indirect branch per block; trip CK_NBLK only scatters the last block.
   o << "__device__ __forceinline__ void ck_reactions(const CkCtx &x, double (&w)[CK_S]) {\n"
-    << "#pragma unroll 1\n  for (int blk = 0; blk < CK_NBLK; ++blk) {\n"
-    << "    double gf[CK_B], gr[CK_B], q[CK_B];\n    switch (blk) {  // gathers: nu'^T ln C, nu''^T ln C\n";
-  for (int k = 0; k < nblk; ++k) {
-    o << "      case " << k << ":\n";
+    << "  double gf[CK_B], gr[CK_B], q[CK_B];\n"
+    << "#pragma unroll 1\n  for (int blk = 0; blk <= CK_NBLK; ++blk) {\n"
+    << "    switch (blk) {\n";
+  auto scatters = [&](int k) {
     for (int b = 0; b < B; ++b) {
       const JitReaction &r = s.rxn[(size_t)k * B + b];
-      o << "        gf[" << b << "] = " << gather_expr(r.reac) << ";";
-      if (r.index >= 0) o << "  // reaction " << r.index;
-      o << "\n        gr[" << b << "] = " << (r.reversible ? gather_expr(r.prod) : std::string("0.0")) << ";\n";
+      for (size_t e = 0; e < r.net.size(); ++e) {
+        const int sp = r.net[e].first;
+        const double c = r.net[e].second;
+        if (c == 1.0) o << "        w[" << sp << "] += q[" << b << "];\n";
+        else if (c == -1.0) o << "        w[" << sp << "] -= q[" << b << "];\n";
+        else o << "        w[" << sp << "] = fma(" << lit(c) << ", q[" << b << "], w[" << sp << "]);\n";
+      }
     }
+  };
+  for (int k = 0; k <= nblk; ++k) {
+    o << "      case " << k << ":\n";
+    if (k > 0) scatters(k - 1);
+    if (k < nblk)
+      for (int b = 0; b < B; ++b) {
+        const JitReaction &r = s.rxn[(size_t)k * B + b];
+        o << "        gf[" << b << "] = " << gather_expr(r.reac) << ";";
+        if (r.index >= 0) o << "  // reaction " << r.index;
+        o << "\n        gr[" << b << "] = " << (r.reversible ? gather_expr(r.prod) : std::string("0.0")) << ";\n";
+      }
     o << "        break;\n";
   }
   o << "    }\n";
@@ -154,22 +171,6 @@ std::string jit_generate_source(const JitSpec &s) {
       << "(x, blk, gf, gr, q);\n";
     first = false;
   }
-  o << "    switch (blk) {  // scatters: w[k] += nu_k q (Eq. 2)\n";
-  for (int k = 0; k < nblk; ++k) {
-    o << "      case " << k << ":\n";
-    for (int b = 0; b < B; ++b) {
-      const JitReaction &r = s.rxn[(size_t)k * B + b];
-      for (size_t e = 0; e < r.net.size(); ++e) {
-        const int sp = r.net[e].first;
-        const double c = r.net[e].second;
-        if (c == 1.0) o << "        w[" << sp << "] += q[" << b << "];\n";
-        else if (c == -1.0) o << "        w[" << sp << "] -= q[" << b << "];\n";
-        else o << "        w[" << sp << "] = fma(" << lit(c) << ", q[" << b << "], w[" << sp << "]);\n";
-      }
-    }
-    o << "        break;\n";
-  }
-  o << "    }\n";
   if (s.sync_every > 0)
     o << "    if (blk % " << s.sync_every << " == " << s.sync_every - 1 << ") __syncthreads();\n";
   o << "  }\n}\n";
