@@ -362,6 +362,7 @@ void build_host(const ck_mech_desc *d, HostBuild *hb) {
       const double *a = (r > rank[k]) ? d->nasa_hi + 7 * k : d->nasa_lo + 7 * k;
       double *row = &hb->jit_thermo[((size_t)r * S + k) * 12];
       for (int i = 0; i < 5; ++i) { row[i] = a[i]; row[6 + i] = a[i] / (i + 1); }
+      row[5] = inv_W[k];
       row[11] = a[5];
     }
   // ln table: interval i covers m in [lo_i, lo_i + width) on the hi-word grid from 0x3fe6a000
@@ -430,6 +431,7 @@ std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk,
   // tuning knobs for A/B runs under ncu (defaults are the measured best)
   if (const char *e = std::getenv("CK_JIT_M")) spec.m_dmma = std::string(e) != "dfma";
   if (const char *e = std::getenv("CK_JIT_SYNC")) spec.sync_every = std::atoi(e);
+  if (const char *e = std::getenv("CK_JIT_KCONST")) spec.kconst = std::atoi(e) != 0;
   *smem_out = best_smem;
   return "";
 }

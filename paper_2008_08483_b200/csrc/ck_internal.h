@@ -34,6 +34,7 @@ struct JitSpec {
   bool m_dmma = true;          // M = C E on DMMA.8x8x4 (else register-tiled DFMA)
   int sync_every = 0;          // block barrier every n reaction blocks (0 = never)
   int block = 4;               // reactions per block of the core
+  bool kconst = false;         // polynomial coefficients as constant-bank operands (else literals)
   int group_end[6] = {0, 0, 0, 0, 0, 0};   // end block of (elementary, three-body, falloff) x (rev, irrev)
   std::vector<JitReaction> rxn;
   std::vector<double> inv_W, range_T, falloff;   // constant-bank tables
