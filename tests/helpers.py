@@ -118,3 +118,24 @@ def paper_matrix_form(mech, T, P, Y):
     cp_mass = (Yc * cp_R * RU / W).sum(1)
     dTdt = -(h_RT * RU * T[:, None] * Omega).sum(1) / (rho * cp_mass)
     return Omega, dTdt
+
+
+def tame(mech, seed=0):
+    """A copy of a generated mechanism with physically mild kinetics, for tests that follow a
+    state in time (input construction only, no kinetics): species enthalpies and entropies
+    proportional to their element counts plus a small random part (element-balanced
+    reactions then have |ln Kc| of order 10 instead of several hundred), one NASA-7 set for
+    both temperature ranges, pre-exponential factors lowered by 1e8 and temperature exponents
+    quartered, so that time scales are far longer than 1e-9 s."""
+    import dataclasses
+    rng = np.random.default_rng(seed)
+    S = mech.n_species
+    n_el = mech.elem_count.shape[1]
+    h_el = rng.uniform(-4000.0, 4000.0, n_el)
+    s_el = rng.uniform(5.0, 15.0, n_el)
+    nasa = mech.nasa_lo.copy()
+    nasa[:, 5] = mech.elem_count @ h_el + rng.uniform(-2000.0, 2000.0, S)
+    nasa[:, 6] = mech.elem_count @ s_el + rng.uniform(-2.0, 2.0, S)
+    return dataclasses.replace(mech, nasa_lo=nasa, nasa_hi=nasa.copy(),
+                               ln_A=mech.ln_A - np.log(1e8), b=mech.b / 4.0,
+                               ln_A0=mech.ln_A0 - np.log(1e8), b0=mech.b0 / 4.0)
