@@ -74,9 +74,10 @@ typedef struct ck_mech_desc {
  * equilibrium-layer coefficients, thermo tables, efficiency matrix) on the current CUDA
  * device and return an opaque handle in *out.  Synchronous.
  * Kernel variant: by default (environment CK_KERNEL unset or "auto") a kernel specialised
- * to the mechanism's structure is compiled with NVRTC for sm_100a when the species
- * accumulators fit in registers (S <= 103), falling back to the generic table-driven kernel
- * otherwise or if NVRTC is unavailable; CK_KERNEL=generic forces the generic kernel,
+ * to the mechanism's structure is compiled with NVRTC for sm_100a (species accumulators in
+ * registers for S <= 103, the most updated ones in registers and the rest in shared memory
+ * beyond that), falling back to the generic table-driven kernel if no launch shape fits or
+ * NVRTC is unavailable; CK_KERNEL=generic forces the generic kernel,
  * CK_KERNEL=jit makes a failed specialisation an error.  Compiled cubins are cached under
  * $CK_JIT_CACHE (default ~/.cache/ck_jit; empty string disables the cache).
  * Errors: CK_EINVAL (NULL pointers, S/R < 1, W <= 0, negative or non-finite nu, a reaction
@@ -105,6 +106,27 @@ int ck_source_terms(const ck_mech *m, const double *T, const double *P, const do
 int ck_source_terms_host(ck_mech *m, const double *T, const double *P, const double *Y,
                          int64_t N, double *wdot, double *dTdt, void *stream);
 
+/* The 0-D constant-pressure reactor use of the source term (BASELINE.json
+ * configs[4]): n_steps steps of the classic explicit 4-stage Runge-Kutta scheme with step dt
+ * [s] on y = (T, Y_1..Y_S) of N independent cells, in place, P[N] constant:
+ *   dT/dt = ck_source_terms' energy term,  dY_k/dt = wdot_k W_k / rho,
+ *   rho = P / (Ru T sum_k Y_k / W_k);
+ *   k1 = f(y), k2 = f(p(y + dt/2 k1)), k3 = f(p(y + dt/2 k2)), k4 = f(p(y + dt k3)),
+ *   y <- p(y + dt/6 (k1 + 2 k2 + 2 k3 + k4)),
+ * where p projects onto valid thermochemical states: Y <- max(Y, 0), Y <- Y / sum(Y),
+ * T <- min(max(T, 250 K), 5000 K) (reading Q14: BASELINE's dt = 1e-9 s is far
+ * outside explicit stability for its rate constants, so every state handed to the source
+ * term is projected).  ck_source_terms runs once per stage (4 per step); one more kernel per
+ * stage forms slopes, weighted sums, the next stage state and its projection.
+ * T, P, Y are DEVICE pointers laid out as for ck_source_terms; T and Y are updated in place.
+ * use_graph != 0: the step is captured once into a CUDA graph (re-captured when T, P, Y, N or
+ * dt change) and replayed n_steps times; use_graph == 0: plain launches.  Asynchronous on
+ * `stream`; the workspace ((3S+3) N doubles) is owned by the handle and grows on demand
+ * (that allocation synchronises).  N == 0 or n_steps == 0 is a successful no-op.
+ * Errors: CK_EINVAL (NULL handle/pointer, negative sizes, dt <= 0), CK_ENOMEM, CK_ECUDA. */
+int ck_rk4_integrate(ck_mech *m, double *T, const double *P, double *Y, int64_t N, double dt,
+                     int64_t n_steps, int use_graph, void *stream);
+
 /* Free the handle and its device memory.  NULL is a no-op. */
 void ck_mech_destroy(ck_mech *m);
 
@@ -116,7 +138,9 @@ const char *ck_last_error(void);
  *       7 #Troe, 8 #temperature ranges, 9 threads per block, 10 blocks per SM,
  *       11 dynamic shared memory per block (bytes), 12 kernels launched per
  *       ck_source_terms call, 13 nnz(E) counted over third-body and falloff columns,
- *       14 kernel variant in use (0 generic table-driven kernel, 1 mechanism-specialised).
+ *       14 kernel variant in use (0 generic table-driven kernel, 1 mechanism-specialised),
+ *       15 species whose accumulators the specialised kernel keeps in registers (the other
+ *       S - that many accumulate in shared memory; 0 for the generic kernel).
  * Returns -1 for a NULL handle or unknown `what`. */
 int64_t ck_mech_info(const ck_mech *m, int what);
 

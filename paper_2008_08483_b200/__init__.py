@@ -21,6 +21,7 @@ import numpy as np
 from . import _build
 
 __all__ = ["Mechanism", "CkError", "ck_mech_create", "ck_source_terms", "ck_source_terms_host",
+           "ck_rk4_integrate",
            "ck_mech_destroy", "ck_last_error", "ck_mech_info", "ck_measure_fp64_peak",
            "ck_mech_jit_source",
            "library_path", "RU", "INFO"]
@@ -28,7 +29,7 @@ __all__ = ["Mechanism", "CkError", "ck_mech_create", "ck_source_terms", "ck_sour
 RU = 8314.46261815324  # J/(kmol K), the constant compiled into the kernels
 INFO = {"S": 0, "R": 1, "nnz_reac": 2, "nnz_prod": 3, "nnz_net": 4, "n_three_body": 5,
         "n_lindemann": 6, "n_troe": 7, "n_ranges": 8, "threads": 9, "blocks_per_sm": 10,
-        "smem_bytes": 11, "launches_per_call": 12, "nnz_eff": 13, "jit": 14}
+        "smem_bytes": 11, "launches_per_call": 12, "nnz_eff": 13, "jit": 14, "s_reg": 15}
 
 _dp = C.POINTER(C.c_double)
 _bp = C.POINTER(C.c_uint8)
@@ -66,6 +67,8 @@ def _load():
     lib.ck_source_terms.argtypes = [C.c_void_p] * 4 + [C.c_int64] + [C.c_void_p] * 3
     lib.ck_source_terms_host.restype = C.c_int
     lib.ck_source_terms_host.argtypes = [C.c_void_p] * 4 + [C.c_int64] + [C.c_void_p] * 3
+    lib.ck_rk4_integrate.restype = C.c_int
+    lib.ck_rk4_integrate.argtypes = [C.c_void_p] * 4 + [C.c_int64, C.c_double, C.c_int64, C.c_int, C.c_void_p]
     lib.ck_mech_destroy.restype = None
     lib.ck_mech_destroy.argtypes = [C.c_void_p]
     lib.ck_last_error.restype = C.c_char_p
@@ -120,6 +123,11 @@ def ck_source_terms(handle, T, P, Y, N, wdot, dTdt, stream=0) -> None:
 def ck_source_terms_host(handle, T, P, Y, N, wdot, dTdt, stream=0) -> None:
     _check(_lib.ck_source_terms_host(handle, _addr(T), _addr(P), _addr(Y), int(N), _addr(wdot),
                                      _addr(dTdt), stream or None))
+
+
+def ck_rk4_integrate(handle, T, P, Y, N, dt, n_steps, use_graph=True, stream=0) -> None:
+    _check(_lib.ck_rk4_integrate(handle, _addr(T), _addr(P), _addr(Y), int(N), float(dt), int(n_steps),
+                                 1 if use_graph else 0, stream or None))
 
 
 def ck_mech_destroy(handle) -> None:
@@ -210,6 +218,13 @@ class Mechanism:
             dTdt = np.empty(N)
         ck_source_terms_host(self.handle, T, P, Y, N, wdot, dTdt, stream)
         return wdot, dTdt
+
+    def rk4_integrate(self, T, P, Y, dt, n_steps, N=None, use_graph=True, stream=0) -> None:
+        """n_steps explicit RK4 steps of the constant-pressure reactor, in place on the device
+        buffers T[N], Y[S][N]; asynchronous on `stream`."""
+        if N is None:
+            N = T.shape[0]
+        ck_rk4_integrate(self.handle, T, P, Y, N, dt, n_steps, use_graph, stream)
 
     def close(self) -> None:
         if getattr(self, "handle", None):

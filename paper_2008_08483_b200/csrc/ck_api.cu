@@ -118,9 +118,90 @@ struct HostBuild {
   std::vector<double> jit_logtab;   // [128][2]: 1/c_i, ln c_i (ck_log in ck_jit_kernel.cuh)
   std::vector<unsigned char> program;
   ck::JitSpec spec;
+  std::string jit_why;        // why the mechanism cannot be specialised ("" if it can)
+  size_t jit_smem = 0;        // dynamic shared memory of the specialised kernel
   int64_t nnz_reac = 0, nnz_prod = 0, nnz_net = 0, nnz_eff = 0;
   int n_three_body = 0, n_lindemann = 0, n_troe = 0;
 };
+
+// B200 (sm_100a) per-SM resources, used when the launch shape has to be chosen without a
+// device (ck_mech_jit_source on a build box)
+constexpr size_t kSmemPerSm = 233472, kSmemPerBlock = 232448;
+
+int env_int(const char *name, int dflt) {
+  const char *e = std::getenv(name);
+  return (e && *e) ? std::atoi(e) : dflt;
+}
+
+// Launch shape of the specialised kernel.  The kernel wants registers before threads: the
+// species accumulators (2 registers per species), the DMMA fragments of M = C E and the
+// interleaved exp chains of a reaction block (about 144 registers, "rest"); measured at S=53,
+// 256 threads x 255 registers beat 384 x 168 by 14 %.
+//  * All accumulators in registers (S <= 103): the most resident threads whose register cap
+//    reaches 2 S + rest (or 255), else the largest cap.
+//  * Otherwise hot/cold: the s_reg most scattered-to species accumulate in registers, the
+//    rest in per-thread columns of shared memory (read-modify-write, no FP64-pipe cost);
+//    the most resident threads, then the most register accumulators.
+// Shared memory (ln C columns + cold accumulators + tables) must fit.  Fills spec.threads /
+// min_blocks / tab_in_smem / s_reg and returns "", or returns the reason it cannot.
+std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk, size_t *smem_out) {
+  const int S = spec.S, R = spec.R;
+  const bool fits = 2 * S + 48 <= 255;
+  const int rest = std::max(48, env_int("CK_JIT_REST", fits ? 144 : 166));
+  const int sreg_forced = std::min(S, env_int("CK_JIT_SREG", -1));   // tuning / test knob
+  const size_t tab_bytes = (size_t)spec.n_ranges * R * 10 * sizeof(double);   // R includes padding
+  const int nt_forced = env_int("CK_JIT_NT", 0), b_forced = env_int("CK_JIT_MINB", 0);
+  int best_nt = 0, best_b = 0, best_cap = 0, best_sreg = 0;
+  bool best_tab = false;
+  size_t best_smem = 0;
+  auto smem_of = [&](int nt, int s_reg, bool tab_smem) {
+    return (size_t)(S + (S - s_reg)) * (nt + 8) * 8 + (32 + 256) * 8 + (size_t)spec.n_ranges * S * 12 * 8 +
+           (tab_smem ? tab_bytes : (size_t)(nt / 32) * 2 * spec.n_ranges * spec.block * 10 * 8) + 16;
+  };
+  const bool all_regs = sreg_forced < 0 ? fits : (sreg_forced == S);
+  if (all_regs) {
+    const int regs_wanted = std::min(255, 2 * S + rest);
+    for (int tab_smem = 1; tab_smem >= 0 && best_nt == 0; --tab_smem)
+      for (int nt : {512, 448, 384, 320, 256, 192, 128, 64}) {
+        if (nt_forced && nt != nt_forced) continue;
+        for (int b = 1; b <= 4; ++b) {
+          if (b_forced && b != b_forced) continue;
+          const int regcap = std::min(255, (65536 / (nt * b)) / 8 * 8);
+          if (regcap < 2 * S + 48) continue;
+          const size_t smem = smem_of(nt, S, tab_smem != 0);
+          if (smem > smem_blk || b * (smem + 1024) > smem_sm) continue;
+          const int cap = std::min(regcap, regs_wanted);
+          const bool better = cap > best_cap || (cap == best_cap && nt * b > best_nt * best_b) ||
+                              (cap == best_cap && nt * b == best_nt * best_b && nt > best_nt);
+          if (better) { best_nt = nt; best_b = b; best_cap = cap; best_tab = tab_smem != 0; best_smem = smem; best_sreg = S; }
+        }
+      }
+  } else {
+    for (int nt : {512, 448, 384, 320, 256, 192, 128, 64})
+      for (int b = 1; b <= 2; ++b)
+        for (int tab_smem = 1; tab_smem >= 0; --tab_smem) {
+          if ((nt_forced && nt != nt_forced) || (b_forced && b != b_forced)) continue;
+          const int regcap = std::min(255, (65536 / (nt * b)) / 8 * 8);
+          const int s_reg = sreg_forced >= 0 ? sreg_forced : std::min(S, (regcap - rest) / 2);
+          if (s_reg < 0 || 2 * s_reg + 48 > regcap) continue;
+          if (sreg_forced < 0 && s_reg < S / 4) continue;
+          const size_t smem = smem_of(nt, s_reg, tab_smem != 0);
+          if (smem > smem_blk || b * (smem + 1024) > smem_sm) continue;
+          const bool better = nt * b > best_nt * best_b ||
+                              (nt * b == best_nt * best_b && (tab_smem != 0) > best_tab) ||
+                              (nt * b == best_nt * best_b && (tab_smem != 0) == best_tab && s_reg > best_sreg);
+          if (better) { best_nt = nt; best_b = b; best_tab = tab_smem != 0; best_smem = smem; best_sreg = s_reg; }
+        }
+  }
+  if (best_nt == 0) return "no launch shape fits registers and shared memory";
+  spec.threads = best_nt; spec.min_blocks = best_b; spec.tab_in_smem = best_tab; spec.s_reg = best_sreg;
+  // tuning knobs for A/B runs under ncu (defaults are the measured best, DESIGN.md)
+  if (const char *e = std::getenv("CK_JIT_M")) spec.m_dmma = std::string(e) != "dfma";
+  if (const char *e = std::getenv("CK_JIT_SYNC")) spec.sync_every = std::atoi(e);
+  if (const char *e = std::getenv("CK_JIT_KCONST")) spec.kconst = std::atoi(e) != 0;
+  *smem_out = best_smem;
+  return "";
+}
 
 // The specialised kernel walks the reactions in blocks of kJitBlock that are homogeneous
 // in (type, reversible): a compact, instruction-cache resident "core" evaluates the rate
@@ -130,7 +211,8 @@ struct HostBuild {
 // groups, every group is padded to whole blocks with null reactions (rate ~ 0, no species),
 // and the rate table, falloff table and efficiency fragments are laid out in that order.
 
-void finalize_jit(const ck_mech_desc *d, HostBuild *hb, const std::vector<double> &falloff_orig) {
+void finalize_jit(const ck_mech_desc *d, HostBuild *hb, const std::vector<double> &falloff_orig,
+                  size_t smem_sm, size_t smem_blk) {
   const int S = d->n_species, R = d->n_reactions;
   ck::JitSpec &spec = hb->spec;
   const int n_ranges = hb->n_ranges_tmp;
@@ -138,7 +220,9 @@ void finalize_jit(const ck_mech_desc *d, HostBuild *hb, const std::vector<double
   orig.swap(spec.rxn);
   const std::vector<double> tab_orig = hb->jit_tab;
 
-  int kJitBlock = 4;                      // tuning knob CK_JIT_B (2..8)
+  // blocks of 4 reactions; 6 when the accumulators do not all fit in registers: that shape has
+  // one warp per scheduler and needs the longer independent chains (measured)
+  int kJitBlock = (2 * S + 48 > 255) ? 6 : 4;   // tuning knob CK_JIT_B (1..8)
   if (const char *e = std::getenv("CK_JIT_B")) kJitBlock = std::min(8, std::max(1, std::atoi(e)));
   auto group_of = [](const ck::JitReaction &r) {
     const int t = r.type == 0 ? 0 : (r.type == 1 ? 1 : 2);
@@ -191,8 +275,35 @@ void finalize_jit(const ck_mech_desc *d, HostBuild *hb, const std::vector<double
     }
     spec.rxn.push_back(std::move(r));
   }
+  // ---- launch shape, and which accumulators live in registers --------------------------
+  hb->jit_why = choose_jit_shape(spec, smem_sm, smem_blk, &hb->jit_smem);
+  if (!hb->jit_why.empty()) spec.s_reg = S;
+  // Internal species order: by the number of scatters into the species (Eq. 2), descending,
+  // so that the register accumulators serve the most updates; identity if all are in registers.
+  std::vector<int> perm(S), inv(S);
+  for (int k = 0; k < S; ++k) perm[k] = k;
+  if (spec.s_reg < S) {
+    std::vector<int> hits(S, 0);
+    for (const ck::JitReaction &r : spec.rxn)
+      for (const auto &e : r.net) hits[e.first]++;
+    std::stable_sort(perm.begin(), perm.end(), [&](int a, int b) { return hits[a] > hits[b]; });
+    spec.perm = perm;
+  }
+  for (int k = 0; k < S; ++k) inv[perm[k]] = k;
+  for (ck::JitReaction &r : spec.rxn) {
+    for (auto &e : r.reac) e.first = inv[e.first];
+    for (auto &e : r.prod) e.first = inv[e.first];
+    for (auto &e : r.net) e.first = inv[e.first];
+  }
+  {
+    const std::vector<double> th = hb->jit_thermo;
+    for (int r = 0; r < n_ranges; ++r)
+      for (int k = 0; k < S; ++k)
+        std::copy(&th[((size_t)r * S + perm[k]) * 12], &th[((size_t)r * S + perm[k]) * 12] + 12,
+                  &hb->jit_thermo[((size_t)r * S + k) * 12]);
+  }
   // E as DMMA.8x8x4 B fragments: [n-tile][k-step][lane], lane holds
-  // E[4 ks + lane%4][8 nt + lane/4], zero padded in both directions
+  // E[4 ks + lane%4][8 nt + lane/4] (species in internal order), zero padded in both directions
   const int n_m = (int)m_rows.size();
   const int n_mb = ((n_m + 7) / 8 + 1) & ~1, k_steps = (S + 3) / 4;   // pairs of n-tiles
   hb->jit_n_m = n_m;
@@ -206,7 +317,7 @@ void finalize_jit(const ck_mech_desc *d, HostBuild *hb, const std::vector<double
         const int k = 4 * ks + lane % 4, row = 8 * nt + lane / 4;
         if (k < S && row < n_m && m_rows[row] >= 0)
           hb->eff_frag[((size_t)nt * k_steps + ks) * 32 + lane] =
-              d->eff ? d->eff[(size_t)k * R + m_rows[row]] : 1.0;
+              d->eff ? d->eff[(size_t)perm[k] * R + m_rows[row]] : 1.0;
       }
   // the DFMA variant's layout [block of 8 rows][species][8]
   hb->jit_eff.assign((size_t)std::max(n_mb, 1) * S * 8, 0.0);
@@ -214,10 +325,10 @@ void finalize_jit(const ck_mech_desc *d, HostBuild *hb, const std::vector<double
     if (m_rows[row] >= 0)
       for (int k = 0; k < S; ++k)
         hb->jit_eff[((size_t)(row / 8) * S + k) * 8 + row % 8] =
-            d->eff ? d->eff[(size_t)k * R + m_rows[row]] : 1.0;
+            d->eff ? d->eff[(size_t)perm[k] * R + m_rows[row]] : 1.0;
 }
 
-void build_host(const ck_mech_desc *d, HostBuild *hb) {
+void build_host(const ck_mech_desc *d, HostBuild *hb, size_t smem_sm = kSmemPerSm, size_t smem_blk = kSmemPerBlock) {
   const int S = d->n_species, R = d->n_reactions;
   HostBuild *m = hb;   // statistics are accumulated on the same names as in ck_mech
   // ---- temperature ranges from the distinct T_mid values --------------
@@ -380,66 +491,17 @@ void build_host(const ck_mech_desc *d, HostBuild *hb) {
     hb->jit_logtab[2 * i + 1] = (double)(-logl((long double)inv_c));
   }
   hb->n_ranges_tmp = n_ranges;
-  finalize_jit(d, hb, falloff);
+  finalize_jit(d, hb, falloff, smem_sm, smem_blk);
   if (falloff.empty()) falloff.resize(ck::kFalloffStride, 0.0);
   if (range_T.empty()) range_T.push_back(0.0);
 
   hb->n_ranges = n_ranges; hb->n_m = n_m; hb->n_mb = n_mb;
 }
 
-// B200 (sm_100a) per-SM resources, used when the launch shape has to be chosen without a
-// device (ck_mech_jit_source on a build box)
-constexpr size_t kSmemPerSm = 233472, kSmemPerBlock = 232448;
-
-// Launch shape of the specialised kernel.  The kernel wants registers before threads: the
-// species accumulators (2 per species), the DMMA fragments of M = C E and the interleaved
-// exp chains of a reaction block; measured at S=53, 256 threads x 255 registers beat
-// 384 x 168 by 14 %.  So: the most resident threads whose register cap reaches
-// 2 S + 144 (or 255), else the largest cap; shared memory (ln C columns + tables) must fit.
-// Returns "" and fills spec.threads / min_blocks / tab_in_smem, or the reason it cannot.
-std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk, size_t *smem_out) {
-  const int S = spec.S, R = spec.R;
-  if (2 * S + 48 > 255) return "too many species for register-resident accumulators";
-  const int regs_wanted = std::min(255, 2 * S + 144);
-  const size_t tab_bytes = (size_t)spec.n_ranges * R * 10 * sizeof(double);   // R includes padding
-  int best_nt = 0, best_b = 0, best_cap = 0;
-  bool best_tab = false;
-  size_t best_smem = 0;
-  const char *nt_env = std::getenv("CK_JIT_NT");   // tuning knobs: force the block size / blocks per SM
-  const int nt_forced = nt_env ? std::atoi(nt_env) : 0;
-  const char *b_env = std::getenv("CK_JIT_MINB");
-  const int b_forced = b_env ? std::atoi(b_env) : 0;
-  for (int tab_smem = 1; tab_smem >= 0 && best_nt == 0; --tab_smem) {
-    for (int nt : {512, 448, 384, 320, 256, 192, 128, 64}) {
-      if (nt_forced && nt != nt_forced) continue;
-      for (int b = 1; b <= 4; ++b) {
-        if (b_forced && b != b_forced) continue;
-        const int regcap = std::min(255, (65536 / (nt * b)) / 8 * 8);
-        if (regcap < 2 * S + 48) continue;
-        const size_t smem = (size_t)S * (nt + 8) * 8 + (32 + 256) * 8 +
-                            (size_t)spec.n_ranges * S * 12 * 8 + (tab_smem ? tab_bytes : 0) + 16;
-        if (smem > smem_blk || b * (smem + 1024) > smem_sm) continue;
-        const int cap = std::min(regcap, regs_wanted);
-        const bool better = cap > best_cap || (cap == best_cap && nt * b > best_nt * best_b) ||
-                            (cap == best_cap && nt * b == best_nt * best_b && nt > best_nt);
-        if (better) { best_nt = nt; best_b = b; best_cap = cap; best_tab = tab_smem != 0; best_smem = smem; }
-      }
-    }
-  }
-  if (best_nt == 0) return "no launch shape fits registers and shared memory";
-  spec.threads = best_nt; spec.min_blocks = best_b; spec.tab_in_smem = best_tab;
-  // tuning knobs for A/B runs under ncu (defaults are the measured best, DESIGN.md)
-  if (const char *e = std::getenv("CK_JIT_M")) spec.m_dmma = std::string(e) != "dfma";
-  if (const char *e = std::getenv("CK_JIT_SYNC")) spec.sync_every = std::atoi(e);
-  if (const char *e = std::getenv("CK_JIT_KCONST")) spec.kconst = std::atoi(e) != 0;
-  *smem_out = best_smem;
-  return "";
-}
-
 // Decides whether to use the specialised kernel (env CK_KERNEL = auto | generic | jit),
 // compiles and loads it.  Returns CK_OK also when it falls back to the generic kernel in
 // auto mode (m->jit_note says why).
-int setup_jit(ck_mech *m, ck::JitSpec &spec, const cudaDeviceProp &prop) {
+int setup_jit(ck_mech *m, ck::JitSpec &spec, const std::string &why, size_t smem) {
   const char *mode_env = std::getenv("CK_KERNEL");
   const std::string mode = mode_env ? mode_env : "auto";
   if (mode == "generic") { m->jit_note = "CK_KERNEL=generic"; return CK_OK; }
@@ -449,9 +511,6 @@ int setup_jit(ck_mech *m, ck::JitSpec &spec, const cudaDeviceProp &prop) {
     m->jit_note = why;
     return required ? fail(CK_EUNSUPPORTED, "CK_KERNEL=jit but " + why) : (int)CK_OK;
   };
-  size_t smem = 0;
-  const std::string why = choose_jit_shape(spec, (size_t)prop.sharedMemPerMultiprocessor,
-                                           (size_t)prop.sharedMemPerBlockOptin, &smem);
   if (!why.empty()) return give_up(why);
 
   const std::string src = ck::jit_generate_source(spec);
@@ -527,7 +586,7 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   m->grid_max = m->num_sms * best_bps;
 
   HostBuild hb;
-  build_host(d, &hb);
+  build_host(d, &hb, (size_t)prop.sharedMemPerMultiprocessor, (size_t)prop.sharedMemPerBlockOptin);
   const int n_ranges = hb.n_ranges, n_m = hb.n_m, n_mb = hb.n_mb;
   m->nnz_reac = hb.nnz_reac; m->nnz_prod = hb.nnz_prod; m->nnz_net = hb.nnz_net; m->nnz_eff = hb.nnz_eff;
   m->n_three_body = hb.n_three_body; m->n_lindemann = hb.n_lindemann; m->n_troe = hb.n_troe;
@@ -575,7 +634,8 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   m->jit_params.tab = (const double *)(base + o_jtab);
   m->jit_params.thermo = (const double *)(base + o_jthermo);
   m->jit_params.logtab = (const double *)(base + o_jlog);
-  if (int st = setup_jit(m, spec, prop)) { ck_mech_destroy(m); return st; }
+  if (int st = setup_jit(m, spec, hb.jit_why, hb.jit_smem)) { ck_mech_destroy(m); return st; }
+  m->jit_s_reg = spec.s_reg;
   *out = m;
   return CK_OK;
 }
@@ -586,6 +646,8 @@ extern "C" void ck_mech_destroy(ck_mech *m) {
   if (m->d_scratch) cudaFree(m->d_scratch);
   if (m->d_stage) cudaFree(m->d_stage);
   if (m->d_jit_scratch) cudaFree(m->d_jit_scratch);
+  if (m->rk4_graph) cudaGraphExecDestroy(m->rk4_graph);
+  if (m->d_rk4) cudaFree(m->d_rk4);
   if (m->jit_lib) cudaLibraryUnload(m->jit_lib);
   delete m;
 }
@@ -645,6 +707,73 @@ extern "C" int ck_source_terms_host(ck_mech *m, const double *T, const double *P
   return CK_OK;
 }
 
+namespace {
+
+// one RK4 step on `st`: 4 x (source terms at the current stage state + stage kernel)
+int rk4_enqueue_step(ck_mech *m, double *T, const double *P, double *Y, int64_t N, double dt, cudaStream_t st) {
+  const int64_t S = m->dev.S;
+  double *Ts = m->d_rk4, *Ys = Ts + N, *wd = Ys + S * N, *dT = wd + S * N, *aT = dT + N, *aY = aT + N;
+  for (int stage = 1; stage <= 4; ++stage) {
+    const double *Tin = stage == 1 ? T : Ts, *Yin = stage == 1 ? Y : Ys;
+    if (int rc = ck_source_terms(m, Tin, P, Yin, N, wd, dT, (void *)st)) return rc;
+    cudaError_t ce = ck::launch_rk4_stage(stage, m, P, T, Y, Ts, Ys, wd, dT, aT, aY, N, dt, st);
+    if (ce != cudaSuccess) return fail_cuda(ce, "rk4 stage kernel launch");
+  }
+  return CK_OK;
+}
+
+}  // namespace
+
+extern "C" int ck_rk4_integrate(ck_mech *m, double *T, const double *P, double *Y, int64_t N, double dt,
+                                int64_t n_steps, int use_graph, void *stream) {
+  if (!m) return fail(CK_EINVAL, "mechanism handle is NULL");
+  if (N < 0 || n_steps < 0) return fail(CK_EINVAL, "N and n_steps must be >= 0");
+  if (!(dt > 0.0) || !std::isfinite(dt)) return fail(CK_EINVAL, "dt must be finite and > 0");
+  if (N == 0 || n_steps == 0) return CK_OK;
+  if (!T || !P || !Y) return fail(CK_EINVAL, "a state pointer is NULL");
+  if (((uintptr_t)T | (uintptr_t)P | (uintptr_t)Y) & 7u) return fail(CK_EINVAL, "pointers must be 8-byte aligned");
+  const int64_t S = m->dev.S;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t ce;
+  if (m->rk4_cells < N) {
+    if (m->rk4_graph) { cudaGraphExecDestroy(m->rk4_graph); m->rk4_graph = nullptr; }
+    if (m->d_rk4) { cudaFree(m->d_rk4); m->d_rk4 = nullptr; m->rk4_cells = 0; }
+    // N even keeps every row 16-byte aligned for the bulk loads of the source-term kernel
+    ce = cudaMalloc((void **)&m->d_rk4, (size_t)(3 * S + 3) * N * sizeof(double));
+    if (ce != cudaSuccess) return fail(CK_ENOMEM, std::string("cudaMalloc rk4 workspace: ") + cudaGetErrorString(ce));
+    m->rk4_cells = N;
+  }
+  if (!use_graph) {
+    for (int64_t s = 0; s < n_steps; ++s)
+      if (int rc = rk4_enqueue_step(m, T, P, Y, N, dt, st)) return rc;
+    return CK_OK;
+  }
+  const bool same = m->rk4_graph && m->rk4_key[0] == T && m->rk4_key[1] == P && m->rk4_key[2] == Y &&
+                    m->rk4_key_N == N && m->rk4_key_dt == dt;
+  if (!same) {
+    if (m->rk4_graph) { cudaGraphExecDestroy(m->rk4_graph); m->rk4_graph = nullptr; }
+    // capture on a private stream so that a legacy/default `stream` argument also works
+    cudaStream_t cap = nullptr;
+    if ((ce = cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking)) != cudaSuccess) return fail_cuda(ce, "cudaStreamCreate");
+    cudaGraph_t graph = nullptr;
+    ce = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+    int rc = CK_OK;
+    if (ce == cudaSuccess) {
+      rc = rk4_enqueue_step(m, T, P, Y, N, dt, cap);
+      ce = cudaStreamEndCapture(cap, &graph);
+    }
+    if (ce == cudaSuccess && rc == CK_OK) ce = cudaGraphInstantiate(&m->rk4_graph, graph, 0);
+    if (graph) cudaGraphDestroy(graph);
+    cudaStreamDestroy(cap);
+    if (rc != CK_OK) return rc;
+    if (ce != cudaSuccess) { m->rk4_graph = nullptr; return fail_cuda(ce, "capturing the RK4 step"); }
+    m->rk4_key[0] = T; m->rk4_key[1] = P; m->rk4_key[2] = Y; m->rk4_key_N = N; m->rk4_key_dt = dt;
+  }
+  for (int64_t s = 0; s < n_steps; ++s)
+    if ((ce = cudaGraphLaunch(m->rk4_graph, st)) != cudaSuccess) return fail_cuda(ce, "cudaGraphLaunch");
+  return CK_OK;
+}
+
 extern "C" int64_t ck_mech_info(const ck_mech *m, int what) {
   if (!m) return -1;
   switch (what) {
@@ -663,6 +792,7 @@ extern "C" int64_t ck_mech_info(const ck_mech *m, int what) {
     case 12: return 1;
     case 13: return m->nnz_eff;
     case 14: return m->jit_kernel ? 1 : 0;
+    case 15: return m->jit_kernel ? m->jit_s_reg : 0;
     default: return -1;
   }
 }
@@ -671,9 +801,7 @@ extern "C" int64_t ck_mech_jit_source(const ck_mech_desc *d, char *buf, int64_t 
   if (validate(d)) return -1;
   HostBuild hb;
   build_host(d, &hb);
-  size_t smem = 0;
-  const std::string why = choose_jit_shape(hb.spec, kSmemPerSm, kSmemPerBlock, &smem);
-  if (!why.empty()) { fail(CK_EUNSUPPORTED, why); return -1; }
+  if (!hb.jit_why.empty()) { fail(CK_EUNSUPPORTED, hb.jit_why); return -1; }
   const std::string src = ck::jit_generate_source(hb.spec);
   if (buf && cap > 0) {
     const size_t n = std::min((size_t)cap - 1, src.size());

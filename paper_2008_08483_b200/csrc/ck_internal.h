@@ -34,6 +34,8 @@ struct JitSpec {
   bool m_dmma = true;          // M = C E on DMMA.8x8x4 (else register-tiled DFMA)
   int sync_every = 0;          // block barrier every n reaction blocks (0 = never)
   int block = 4;               // reactions per block of the core
+  int s_reg = 0;               // species with register accumulators (internal order); rest in smem
+  std::vector<int> perm;       // internal species -> row of Y / wdot; empty = identity
   bool kconst = false;         // polynomial coefficients as constant-bank operands (else literals)
   int group_end[6] = {0, 0, 0, 0, 0, 0};   // end block of (elementary, three-body, falloff) x (rev, irrev)
   std::vector<JitReaction> rxn;
@@ -63,13 +65,20 @@ struct ck_mech {
   cudaLibrary_t jit_lib = nullptr;
   cudaKernel_t jit_kernel = nullptr;
   ck::JitParams jit_params{};
-  int jit_threads = 0, jit_blocks_per_sm = 0, jit_grid_max = 0;
+  int jit_threads = 0, jit_blocks_per_sm = 0, jit_grid_max = 0, jit_s_reg = 0;
   size_t jit_smem = 0;
   double *d_jit_scratch = nullptr;
   std::string jit_note;       // why the specialised kernel is not in use, if so
   // staging for ck_source_terms_host
   double *d_stage = nullptr;
   int64_t stage_cells = 0;
+  // ck_rk4_integrate: workspace (stage state, slopes, weighted slope sums) and the captured step
+  double *d_rk4 = nullptr;
+  int64_t rk4_cells = 0;
+  cudaGraphExec_t rk4_graph = nullptr;
+  const void *rk4_key[3] = {nullptr, nullptr, nullptr};   // T, P, Y the graph was captured for
+  int64_t rk4_key_N = 0;
+  double rk4_key_dt = 0.0;
 };
 
 namespace ck {
@@ -81,6 +90,11 @@ cudaError_t kernel_configure(int threads, size_t smem_bytes, int *blocks_per_sm)
 cudaError_t launch_source_terms(const ck_mech *m, const double *T, const double *P,
                                 const double *Y, int64_t N, double *wdot, double *dTdt,
                                 cudaStream_t stream);
+
+// One RK4 stage's update kernel (ck_rk4.cu); stage = 1..4.
+cudaError_t launch_rk4_stage(int stage, const ck_mech *m, const double *P, double *T0, double *Y0, double *Ts,
+                             double *Ys, const double *wdot, const double *dTdt, double *accT, double *accY,
+                             int64_t N, double dt, cudaStream_t stream);
 
 // DFMA throughput microbenchmark (thread-level FMA instructions per second).
 cudaError_t measure_fp64_peak(double *fma_per_s, cudaStream_t stream);

@@ -114,7 +114,13 @@ std::string jit_generate_source(const JitSpec &s) {
     << "\n#define CK_NFO " << s.n_fo << "\n#define CK_TAB_SMEM " << (s.tab_in_smem ? 1 : 0)
     << "\n#define CK_M_DMMA " << (s.m_dmma ? 1 : 0) << "\n#define CK_KCONST " << (s.kconst ? 1 : 0) << "\n#define CK_SYNC_EVERY " << s.sync_every
     << "\n#define CK_B " << s.block << "\n#define CK_NBLK " << (int)s.rxn.size() / s.block
-    << "\n#define CK_G_TB0 " << s.group_end[1] << "\n#define CK_G_FO0 " << s.group_end[3] << "\n";
+    << "\n#define CK_G_TB0 " << s.group_end[1] << "\n#define CK_G_FO0 " << s.group_end[3]
+    << "\n#define CK_SREG " << s.s_reg << "\n#define CK_PERM " << (s.perm.empty() ? 0 : 1) << "\n";
+  if (!s.perm.empty()) {
+    o << "__constant__ int ck_c_perm[" << s.perm.size() << "] = {";
+    for (size_t i = 0; i < s.perm.size(); ++i) o << (i ? "," : "") << (i % 16 == 0 ? "\n  " : " ") << s.perm[i];
+    o << "};\n";
+  }
   auto emit = [&](const char *name, const std::vector<double> &v) {
     o << "__constant__ double " << name << "[" << (v.empty() ? 1 : v.size()) << "] = {";
     for (size_t i = 0; i < v.size(); ++i) o << (i ? "," : "") << (i % 6 == 0 ? "\n  " : " ") << lit(v[i]);
@@ -131,9 +137,11 @@ std::string jit_generate_source(const JitSpec &s) {
   // One switch case per loop trip: the scatters of the previous block (Eq. 2) and the
   // gathers of this one (Eq. 4), so that the unique code is walked in address order with one
   // indirect branch per block; trip CK_NBLK only scatters the last block.
-  o << "__device__ __forceinline__ void ck_reactions(const CkCtx &x, double (&w)[CK_S]) {\n"
+  o << "__device__ __forceinline__ void ck_reactions(const CkCtx &x, double (&w)[CK_SREG > 0 ? CK_SREG : 1]) {\n"
     << "  double gf[CK_B], gr[CK_B], q[CK_B];\n"
+    << "#if !CK_TAB_SMEM\n  ck_ring_issue(x, 0);\n#endif\n"
     << "#pragma unroll 1\n  for (int blk = 0; blk <= CK_NBLK; ++blk) {\n"
+    << "#if !CK_TAB_SMEM\n    ck_ring_issue(x, blk + 1);\n#endif\n"
     << "    switch (blk) {\n";
   auto scatters = [&](int k) {
     for (int b = 0; b < B; ++b) {
@@ -141,9 +149,12 @@ std::string jit_generate_source(const JitSpec &s) {
       for (size_t e = 0; e < r.net.size(); ++e) {
         const int sp = r.net[e].first;
         const double c = r.net[e].second;
-        if (c == 1.0) o << "        w[" << sp << "] += q[" << b << "];\n";
-        else if (c == -1.0) o << "        w[" << sp << "] -= q[" << b << "];\n";
-        else o << "        w[" << sp << "] = fma(" << lit(c) << ", q[" << b << "], w[" << sp << "]);\n";
+        // register accumulator, or the cold species' column in shared memory
+        const std::string acc = sp < s.s_reg ? "w[" + std::to_string(sp) + "]"
+                                             : "CK_WC(" + std::to_string(sp - s.s_reg) + ")";
+        if (c == 1.0) o << "        " << acc << " += q[" << b << "];\n";
+        else if (c == -1.0) o << "        " << acc << " -= q[" << b << "];\n";
+        else o << "        " << acc << " = fma(" << lit(c) << ", q[" << b << "], " << acc << ");\n";
       }
     }
   };
@@ -159,7 +170,7 @@ std::string jit_generate_source(const JitSpec &s) {
       }
     o << "        break;\n";
   }
-  o << "    }\n";
+  o << "    }\n#if !CK_TAB_SMEM\n    ck_ring_wait();\n#endif\n";
   const char *names[6] = {"ck_core<0, 1>", "ck_core<0, 0>", "ck_core<1, 1>", "ck_core<1, 0>",
                           "ck_core<2, 1>", "ck_core<2, 0>"};
   bool first = true;

@@ -32,9 +32,27 @@ def kernel_variant(request, monkeypatch):
 
 
 def test_variant_selection(ck, kernel_variant):
-    for spec in (ckgen.MECH_TINY, ckgen.MECH_MID):
+    for spec in (ckgen.MECH_TINY, ckgen.MECH_MID, ckgen.MECH_LARGE):
         with ck.Mechanism(ckgen.mechanism(spec)) as gm:
             assert gm.info("jit") == (1 if kernel_variant == "auto" else 0)
+            if kernel_variant == "auto":
+                # S=111 does not fit 2 registers per species: hot/cold accumulator split
+                assert (gm.info("s_reg") < spec.S) == (spec is ckgen.MECH_LARGE)
+
+
+@pytest.mark.parametrize("s_reg", [0, 7, 30])
+def test_cold_accumulators_on_small_mechanisms(ck, monkeypatch, kernel_variant, s_reg):
+    """The shared-memory (cold) accumulator path and the species permutation that comes with
+    it, forced on mechanisms that would otherwise keep every accumulator in registers."""
+    if kernel_variant != "auto":
+        pytest.skip("specialised kernel only")
+    monkeypatch.setenv("CK_JIT_SREG", str(s_reg))
+    for cfg_name, N in (("tiny_1k", 1024), ("mid_1m", 777)):
+        cfg = ckgen.CONFIGS[cfg_name]
+        mech = ckgen.mechanism(cfg.mech)
+        with ck.Mechanism(mech) as gm:
+            assert gm.info("jit") == 1 and gm.info("s_reg") == min(s_reg, mech.n_species)
+        assert_parity(ck, mech, *ckgen.states(cfg, N=N), label="%s s_reg=%d" % (cfg_name, s_reg))
 
 
 def gpu_run(ck, mech, T, P, Y, gm=None):
