@@ -18,6 +18,13 @@ _dp = C.POINTER(C.c_double)
 _bp = C.POINTER(C.c_uint8)
 
 
+class _Ann(C.Structure):
+    _fields_ = [("n_in", C.c_int32), ("n_layers", C.c_int32), ("n_hidden", C.c_int32),
+                ("activation", C.c_int32), ("in_mean", _dp), ("in_std", _dp), ("W_in", _dp),
+                ("B", _dp), ("W_hid", _dp), ("W_out", _dp), ("B_out", _dp), ("out_mean", _dp),
+                ("out_std", _dp)]
+
+
 class _Mech(C.Structure):
     _fields_ = [
         ("S", C.c_int32), ("R", C.c_int32),
@@ -25,7 +32,7 @@ class _Mech(C.Structure):
         ("ln_A", _dp), ("b", _dp), ("Ea_over_R", _dp), ("reversible", _bp),
         ("nasa_lo", _dp), ("nasa_hi", _dp), ("T_mid", _dp), ("rxn_type", _bp),
         ("eff", _dp), ("ln_A0", _dp), ("b0", _dp), ("Ea0_over_R", _dp), ("troe", _dp),
-        ("p_ref", C.c_double),
+        ("p_ref", C.c_double), ("kc_ann", C.POINTER(_Ann)),
     ]
 
 
@@ -57,7 +64,9 @@ def _u8(a):
 class OracleMechanism:
     """Holds C-contiguous copies of a ckgen.Mechanism's arrays and the C struct."""
 
-    def __init__(self, mech):
+    def __init__(self, mech, kc_ann=None):
+        """kc_ann: None (exact Kc) or an object with ckgen.KcAnn's attributes (approximate ANN
+        for log Kc)."""
         self.S, self.R = mech.n_species, mech.n_reactions
         self._keep = dict(
             W=_f64(mech.mol_weight), nu_reac=_f64(mech.nu_reac), nu_prod=_f64(mech.nu_prod),
@@ -75,6 +84,20 @@ class OracleMechanism:
         for name, arr in k.items():
             ptr_t = _bp if arr.dtype == np.uint8 else _dp
             setattr(s, name, arr.ctypes.data_as(ptr_t))
+        if kc_ann is not None:
+            NL, NH, NI = int(kc_ann.n_layers), int(kc_ann.n_hidden), int(kc_ann.n_in)
+            ka = dict(in_mean=_f64(kc_ann.in_mean), in_std=_f64(kc_ann.in_std), W_in=_f64(kc_ann.W_in),
+                      B=_f64(kc_ann.B), W_hid=_f64(kc_ann.W_hid), W_out=_f64(kc_ann.W_out),
+                      B_out=_f64(kc_ann.B_out), out_mean=_f64(kc_ann.out_mean), out_std=_f64(kc_ann.out_std))
+            assert ka["W_in"].shape == (NI, NH) and ka["B"].shape == (NL, NH)
+            assert ka["W_hid"].shape == (NL - 1, NH, NH) and ka["W_out"].shape == (NH, self.R)
+            assert ka["in_mean"].shape == (NI,) and ka["out_std"].shape == (self.R,)
+            a = _Ann()
+            a.n_in, a.n_layers, a.n_hidden, a.activation = NI, NL, NH, int(kc_ann.activation)
+            for name, arr in ka.items():
+                setattr(a, name, arr.ctypes.data_as(_dp))
+            self._keep_ann, self._ann = ka, a
+            s.kc_ann = C.pointer(a)
         self.c = s
 
 

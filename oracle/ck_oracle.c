@@ -47,10 +47,47 @@ static double troe_F(const double *tp, double T, double Pr) {
   return pow(10.0, lF);
 }
 
+/* Approximate ANN for log Kc, Eq. 12-14, one cell: lnKc[R] from T.
+ * xa, xb: scratch of N_H doubles each. */
+static double activation(int kind, double x) {
+  if (kind == 0) return x > 0.0 ? x : 0.0;          /* relu, Eq. 13 */
+  return x >= 0.0 ? x : exp(x) - 1.0;               /* elu, Eq. 14 */
+}
+
+static void ann_log_Kc(const ck_oracle_kc_ann *a, int R, double T, double *xa, double *xb,
+                       double *lnKc) {
+  const int NH = a->n_hidden;
+  const double feat[6] = {log(T), T, T * T, T * T * T, T * T * T * T, 1.0 / T};
+  /* X_1 = sigma(X_0 W_0 + B_0), X_0 = standardised features */
+  for (int h = 0; h < NH; ++h) {
+    double z = a->B[h];
+    for (int i = 0; i < a->n_in; ++i)
+      z += ((feat[i] - a->in_mean[i]) / a->in_std[i]) * a->W_in[i * NH + h];
+    xa[h] = activation(a->activation, z);
+  }
+  /* X_{l+1} = sigma(X_l W_l + B_l), l = 1 .. N_L - 1 */
+  for (int l = 1; l < a->n_layers; ++l) {
+    const double *W = a->W_hid + (size_t)(l - 1) * NH * NH;
+    for (int h = 0; h < NH; ++h) {
+      double z = a->B[l * NH + h];
+      for (int g = 0; g < NH; ++g) z += xa[g] * W[g * NH + h];
+      xb[h] = activation(a->activation, z);
+    }
+    for (int h = 0; h < NH; ++h) xa[h] = xb[h];
+  }
+  /* linear output layer, then de-standardisation */
+  for (int j = 0; j < R; ++j) {
+    double y = a->B_out[j];
+    for (int h = 0; h < NH; ++h) y += xa[h] * a->W_out[h * R + j];
+    lnKc[j] = y * a->out_std[j] + a->out_mean[j];
+  }
+}
+
 /* workspace: per-species and per-reaction scratch for one cell */
 typedef struct {
   double *C, *cp_R, *h_RT, *s_R, *g_RT;          /* [S] */
   double *kf, *Kc, *kr, *M, *qf, *qr, *Q, *wdot; /* [R], wdot [S] */
+  double *ann_lnKc, *ann_x;                      /* [R], [2 N_H] (approximate ANN only) */
 } cell_ws;
 
 static void one_cell(const ck_oracle_mech *m, double T, double P, const double *Y,
@@ -81,6 +118,10 @@ static void one_cell(const ck_oracle_mech *m, double T, double P, const double *
 
   for (int k = 0; k < S; ++k) w->wdot[k] = 0.0;
 
+  /* 2b. approximate ANN in place of the exact equilibrium layer */
+  if (m->kc_ann)
+    ann_log_Kc(m->kc_ann, R, T, w->ann_x, w->ann_x + m->kc_ann->n_hidden, w->ann_lnKc);
+
   for (int j = 0; j < R; ++j) {
     /* 3. forward constant, Eq. 5; equilibrium constant, Eq. 8:
      *    Kc = (p_ref/(Ru T))^(sum_k nu_kj) exp(-sum_k nu_kj g_k/RT)  */
@@ -92,6 +133,7 @@ static void one_cell(const ck_oracle_mech *m, double T, double P, const double *
       dG += nu * w->g_RT[k];
     }
     double Kc = exp(-dG) * pow(m->p_ref / (Ru * T), dnu_sum);
+    if (m->kc_ann) Kc = exp(w->ann_lnKc[j]);
 
     /* 4. third bodies and falloff */
     const int type = m->rxn_type ? m->rxn_type[j] : 0;
@@ -142,14 +184,14 @@ static void one_cell(const ck_oracle_mech *m, double T, double P, const double *
   *dTdt_out = -hw / (rho * cp);
 }
 
-static int ws_alloc(cell_ws *w, int S, int R) {
-  double *p = (double *)malloc(sizeof(double) * (size_t)(6 * S + 7 * R));
+static int ws_alloc(cell_ws *w, int S, int R, int NH) {
+  double *p = (double *)malloc(sizeof(double) * (size_t)(6 * S + 8 * R + 2 * NH));
   if (!p) return -1;
   w->C = p; w->cp_R = p + S; w->h_RT = p + 2 * S; w->s_R = p + 3 * S; w->g_RT = p + 4 * S;
   w->wdot = p + 5 * S;
   double *q = p + 6 * S;
   w->kf = q; w->Kc = q + R; w->kr = q + 2 * R; w->M = q + 3 * R; w->qf = q + 4 * R;
-  w->qr = q + 5 * R; w->Q = q + 6 * R;
+  w->qr = q + 5 * R; w->Q = q + 6 * R; w->ann_lnKc = q + 7 * R; w->ann_x = q + 8 * R;
   return 0;
 }
 
@@ -165,7 +207,7 @@ int ck_oracle_source_terms(const ck_oracle_mech *m, const double *T, const doubl
 #endif
   {
     cell_ws w;
-    if (ws_alloc(&w, S, R) == 0) {
+    if (ws_alloc(&w, S, R, m->kc_ann ? m->kc_ann->n_hidden : 0) == 0) {
 #ifdef _OPENMP
 #pragma omp for schedule(static)
 #endif
@@ -191,7 +233,7 @@ void ck_oracle_cell_detail(const ck_oracle_mech *m, double T, double P, const do
                            double *kf, double *Kc, double *kr, double *M, double *qf,
                            double *qr, double *Q, double *wdot, double *dTdt) {
   cell_ws w;
-  if (ws_alloc(&w, m->S, m->R) != 0) return;
+  if (ws_alloc(&w, m->S, m->R, m->kc_ann ? m->kc_ann->n_hidden : 0) != 0) return;
   double r, c, d;
   one_cell(m, T, P, Y, ldY, &w, &r, &c, &d);
   if (rho) *rho = r;

@@ -31,6 +31,25 @@
 extern "C" {
 #endif
 
+/* Approximate ANN for log Kc (Eq. 12-14, Fig. 2): a drop-in replacement of
+ * the exact equilibrium layer.  X_0 = standardised input features of temperature,
+ * X_{l+1} = sigma(X_l W_l + B_l) for the N_L hidden layers of N_H neurons (Eq. 12), a linear
+ * output layer of width R giving the standardised log Kc~, which is then de-standardised
+ * (PAPER.md:141).  n_in = 1: X_0 = [ln T] (Architecture 2); n_in = 6: X_0 = the exact layer's
+ * features [ln T, T, T^2, T^3, T^4, 1/T] (Architecture 1).  sigma = relu (Eq. 13) or elu
+ * (Eq. 14).  Pins: tests/test_oracle_ann.py (a 50-digit worked example; a network built to
+ * reproduce the exact layer; a numpy matrix restatement of Eq. 12). */
+typedef struct ck_oracle_kc_ann {
+  int32_t n_in, n_layers, n_hidden, activation;  /* activation: 0 relu, 1 elu */
+  const double *in_mean, *in_std;  /* [n_in] */
+  const double *W_in;              /* [n_in][N_H] */
+  const double *B;                 /* [N_L][N_H] */
+  const double *W_hid;             /* [N_L-1][N_H (from)][N_H (to)] */
+  const double *W_out;             /* [N_H][R] */
+  const double *B_out;             /* [R] */
+  const double *out_mean, *out_std;/* [R] */
+} ck_oracle_kc_ann;
+
 typedef struct ck_oracle_mech {
   int32_t S, R;
   const double *W;          /* [S] kg/kmol */
@@ -48,6 +67,7 @@ typedef struct ck_oracle_mech {
   const double *ln_A0, *b0, *Ea0_over_R; /* [R] low-pressure limit */
   const double *troe;       /* [R*4] alpha, T***, T*, T** */
   double p_ref;             /* Pa */
+  const ck_oracle_kc_ann *kc_ann; /* NULL: exact Kc (Eq. 8); else Kc = exp(ANN(T)) */
 } ck_oracle_mech;
 
 /* wdot[S][N] (kmol/m^3/s) and dTdt[N] (K/s) from T[N] (K), P[N] (Pa), Y[S][N].

@@ -139,3 +139,55 @@ def tame(mech, seed=0):
     return dataclasses.replace(mech, nasa_lo=nasa, nasa_hi=nasa.copy(),
                                ln_A=mech.ln_A - np.log(1e8), b=mech.b / 4.0,
                                ln_A0=mech.ln_A0 - np.log(1e8), b0=mech.b0 / 4.0)
+
+
+def ann_forward_matrix_form(ann, T):
+    """Eq. 12 literally, batch dimension leading: X_{l+1} = sigma(X_l W_l +
+    B_l), standardised input features and de-standardised linear output.
+    Returns log Kc~ [N, R]."""
+    import ckgen
+    act = (lambda z: np.maximum(z, 0.0)) if ann.activation == ckgen.RELU else \
+        (lambda z: np.where(z >= 0.0, z, np.expm1(np.minimum(z, 0.0))))
+    X = (ckgen.temperature_features(T)[:, :ann.n_in] - ann.in_mean) / ann.in_std
+    X = act(X @ ann.W_in + ann.B[0])
+    for l in range(1, ann.n_layers):
+        X = act(X @ ann.W_hid[l - 1] + ann.B[l])
+    return (X @ ann.W_out + ann.B_out) * ann.out_std + ann.out_mean
+
+
+def exact_layer_as_ann(mech, n_layers=1, activation=1, seed=0):
+    """A KcAnn that reproduces the exact equilibrium layer of a mechanism whose two NASA sets
+    coincide (input construction from Eq. 10-11 of the paper): Architecture 1
+    features pass through the hidden layers unchanged (they are all positive, so relu and elu
+    act as the identity; a second hidden layer permutes them) and the output layer carries
+    ln Kc_j = -sum_k nu_kj (g_k/RT - ln(p_ref/(Ru T))) on [ln T, T, T^2, T^3, T^4, 1/T].
+    Standardisations are non-trivial and undone by the weights."""
+    import ckgen
+    rng = np.random.default_rng(seed)
+    a = mech.nasa_hi
+    S, R = mech.n_species, mech.n_reactions
+    nu = mech.nu_prod - mech.nu_reac                                     # [S, R]
+    # g'_k = g_k/RT - ln(p_ref/(Ru T)) = coef_k . X_G + bias_k
+    coef = np.stack([1.0 - a[:, 0], -a[:, 1] / 2, -a[:, 2] / 6, -a[:, 3] / 12, -a[:, 4] / 20, a[:, 5]], axis=0)  # [6, S]
+    bias = a[:, 0] - a[:, 6] - np.log(mech.p_ref / RU)                   # [S]
+    Wk = -(coef @ nu)                                                    # [6, R]  ln Kc on the features
+    bk = -(bias @ nu)                                                    # [R]
+    in_mean = rng.uniform(0.5, 2.0, 6) * np.array([7.0, 1e3, 1e6, 1e9, 1e12, 1e-3])
+    in_std = rng.uniform(0.5, 2.0, 6) * np.array([0.3, 5e2, 1e6, 1e9, 1e12, 3e-4])
+    out_mean, out_std = rng.uniform(-20, 20, R), rng.uniform(1, 10, R)
+    W_in, B0 = np.diag(in_std), in_mean.copy()                           # hidden 1 = raw features
+    B = np.zeros((n_layers, 6))
+    B[0] = B0
+    perm = np.arange(6)
+    W_hid = np.zeros((n_layers - 1, 6, 6))
+    for l in range(n_layers - 1):
+        p = rng.permutation(6)
+        W_hid[l][np.arange(6), p] = 1.0                                  # neuron `from` -> neuron p[from]
+        new = np.empty(6, dtype=int)
+        new[p] = perm
+        perm = new                                                       # hidden[to] holds feature perm[to]
+    W_out = (Wk[perm] / out_std[None, :])
+    B_out = (bk - out_mean) / out_std
+    return ckgen.KcAnn(n_in=6, n_layers=n_layers, n_hidden=6, activation=activation, in_mean=in_mean,
+                       in_std=in_std, W_in=W_in, B=B, W_hid=W_hid, W_out=W_out, B_out=B_out,
+                       out_mean=out_mean, out_std=out_std)
