@@ -251,6 +251,65 @@ def run_rk4(args):
     gm.close()
 
 
+def run_ann(args):
+    """The paper's Fig. 10 on this implementation: time of the source term
+    with the approximate ANN for log Kc (Architecture 2, elu; N_L = 1..3 hidden layers of N_H
+    neurons, random weights -- timing needs no trained ones) against the exact equilibrium
+    layer, at N_C = 1e5 cells, for the three mechanism shapes.  The kernel is fused, so the
+    layer's own cost is measured by ablation: t_none is the same kernel with the equilibrium
+    layer removed (CK_JIT_KC=none, a measurement-only variant).  One JSON line."""
+    import torch
+    import ckgen
+    import paper_2008_08483_b200 as ck
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    stream = torch.cuda.current_stream().cuda_stream
+    N = args.cells or 100000
+    out = {"ann": "Fig. 10 analogue: ck_source_terms at N=%d cells, exact vs approximate-ANN log Kc "
+                  "(Architecture 2, elu, random weights); ms per call" % N, "mechanisms": []}
+
+    def timed(gm, bufs):
+        Td, Pd, Yd, w, d = bufs
+        for _ in range(5):
+            gm.source_terms(Td, Pd, Yd, w, d, stream=stream)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(20):
+            gm.source_terms(Td, Pd, Yd, w, d, stream=stream)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / 20
+
+    for name in ("tiny_1m", "mid_1m", "large_256k"):
+        cfg = ckgen.CONFIGS[name]
+        mech = ckgen.mechanism(cfg.mech)
+        S, R = mech.n_species, mech.n_reactions
+        T, P, Y = ckgen.states(cfg, N=N)
+        bufs = [torch.from_numpy(a).to(dev) for a in (T, P, Y)]
+        bufs += [torch.empty((S, N), dtype=torch.float64, device=dev), torch.empty(N, dtype=torch.float64, device=dev)]
+        with ck.Mechanism(mech) as gm:
+            t_exact = timed(gm, bufs)
+        os.environ["CK_JIT_KC"] = "none"
+        try:
+            with ck.Mechanism(mech) as gm:
+                t_none = timed(gm, bufs)
+        finally:
+            del os.environ["CK_JIT_KC"]
+        rows = []
+        for n_layers in (1, 2, 3):
+            for n_hidden in (2, 4, 8, 16, 32):
+                ann = ckgen.random_kc_ann(R, n_layers, n_hidden, seed=n_layers * 100 + n_hidden, T_range=cfg.T_range)
+                with ck.Mechanism(mech, kc_ann=ann) as gm:
+                    t_ann = timed(gm, bufs)
+                rows.append({"N_L": n_layers, "N_H": n_hidden, "N_H_over_N_S": n_hidden / S, "ms": t_ann,
+                             "speedup_source_term": t_exact / t_ann,
+                             "speedup_kc_layer": (t_exact - t_none) / max(t_ann - t_none, 1e-9)})
+        out["mechanisms"].append({"S": S, "R": R, "ms_exact": t_exact, "ms_without_kc_layer": t_none,
+                                  "kc_share_of_source_term": (t_exact - t_none) / t_exact, "rows": rows})
+    print(json.dumps(out))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -264,12 +323,15 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="configs[4]: saturation sweep over N (1 GPU)")
     ap.add_argument("--rk4", action="store_true", help="configs[4]: explicit RK4 reactor run (1 GPU)")
     ap.add_argument("--rk4-steps", type=int, default=1000)
+    ap.add_argument("--ann", action="store_true", help="Fig. 10 analogue: approximate-ANN vs exact log Kc (1 GPU)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     if args.sweep:
         return run_sweep(args)
     if args.rk4:
         return run_rk4(args)
+    if args.ann:
+        return run_ann(args)
 
     import ckgen
     cfg = ckgen.CONFIGS[args.workload]

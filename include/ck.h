@@ -43,6 +43,36 @@ enum { CK_ELEMENTARY = 0, CK_THREE_BODY = 1, CK_LINDEMANN = 2, CK_TROE = 3 };
 
 typedef struct ck_mech ck_mech; /* opaque; owns device memory on the device current at create */
 
+/* Approximate ANN for log Kc (Sec. 2.3, Eq. 12-14, Fig. 2): a drop-in
+ * replacement of the exact equilibrium layer (3).  X_0 = standardised input features of
+ * temperature, X_{l+1} = sigma(X_l W_l + B_l) for l = 0 .. N_L-1 (N_L hidden layers of N_H
+ * neurons), a linear output layer of width R giving the standardised log Kc~, then
+ * log Kc~_j = out_mean[j] + out_std[j] * y_j (standardisation: PAPER.md:141).
+ *   n_in = 1: X_0 = [ln T]                              (Architecture 2, the one the paper runs)
+ *   n_in = 6: X_0 = [ln T, T, T^2, T^3, T^4, 1/T]       (Architecture 1, the exact layer's features)
+ * standardised as (x - in_mean) / in_std.  All arrays are HOST pointers, row-major, copied.
+ * The hidden layers' weights (everything but W_out, B_out, out_*) must fit 40 KB (they are
+ * constant-bank operands of the kernel): e.g. 3 layers of 50 neurons; else CK_EUNSUPPORTED.
+ * The weights come from the caller (the paper trains them; training is not part
+ * of this library).  Everything else of the path is unchanged: k_r = k_f / Kc~ (Eq. 7). */
+enum { CK_ANN_RELU = 0 /* Eq. 13 */, CK_ANN_ELU = 1 /* Eq. 14 */ };
+typedef struct ck_kc_ann {
+  int32_t n_in;           /* 1 or 6 */
+  int32_t n_layers;       /* N_L hidden layers, 1..8 */
+  int32_t n_hidden;       /* N_H neurons per hidden layer, 1..64 */
+  int32_t activation;     /* CK_ANN_RELU or CK_ANN_ELU */
+  const double *in_mean;  /* [n_in] */
+  const double *in_std;   /* [n_in] > 0 */
+  const double *W_in;     /* [n_in][N_H]         input i -> neuron h at i*N_H + h */
+  const double *B;        /* [N_L][N_H]          bias of hidden layer l */
+  const double *W_hid;    /* [N_L-1][N_H][N_H]   layer l: neuron g -> neuron h at (l*N_H + g)*N_H + h;
+                                                  may be NULL if N_L == 1 */
+  const double *W_out;    /* [N_H][R]            neuron h -> reaction j at h*R + j */
+  const double *B_out;    /* [R] */
+  const double *out_mean; /* [R] */
+  const double *out_std;  /* [R] */
+} ck_kc_ann;
+
 /* Mechanism description.  All pointers are HOST pointers; the arrays are copied by
  * ck_mech_create and stay owned by the caller.  S = n_species, R = n_reactions.
  * Matrices are row-major with the species index first: element (k, j) at k*R + j. */
@@ -68,6 +98,9 @@ typedef struct ck_mech_desc {
   const double *troe;        /* [R*4] alpha, T***, T*, T** at j*4; T** = +INF gives the
                                       3-parameter form; read where rxn_type == CK_TROE */
   double p_ref;              /* Pa, standard-state pressure of the NASA data (Eq. 8) */
+  const ck_kc_ann *kc_ann;   /* NULL: exact equilibrium layer; else log Kc from this network.
+                                Needs the mechanism-specialised kernel (CK_EUNSUPPORTED if it
+                                cannot be built) */
 } ck_mech_desc;
 
 /* Validate `desc`, build the device-resident mechanism (sorted reaction program, folded

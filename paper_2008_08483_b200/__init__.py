@@ -35,6 +35,13 @@ _dp = C.POINTER(C.c_double)
 _bp = C.POINTER(C.c_uint8)
 
 
+class _Ann(C.Structure):
+    _fields_ = [("n_in", C.c_int32), ("n_layers", C.c_int32), ("n_hidden", C.c_int32),
+                ("activation", C.c_int32), ("in_mean", _dp), ("in_std", _dp), ("W_in", _dp),
+                ("B", _dp), ("W_hid", _dp), ("W_out", _dp), ("B_out", _dp), ("out_mean", _dp),
+                ("out_std", _dp)]
+
+
 class _Desc(C.Structure):
     _fields_ = [
         ("n_species", C.c_int32), ("n_reactions", C.c_int32),
@@ -42,7 +49,7 @@ class _Desc(C.Structure):
         ("ln_A", _dp), ("b", _dp), ("Ea_over_R", _dp), ("reversible", _bp),
         ("nasa_lo", _dp), ("nasa_hi", _dp), ("T_mid", _dp), ("rxn_type", _bp),
         ("eff", _dp), ("ln_A0", _dp), ("b0", _dp), ("Ea0_over_R", _dp), ("troe", _dp),
-        ("p_ref", C.c_double),
+        ("p_ref", C.c_double), ("kc_ann", C.POINTER(_Ann)),
     ]
 
 
@@ -138,9 +145,9 @@ def ck_mech_info(handle, what) -> int:
     return int(_lib.ck_mech_info(handle, INFO[what] if isinstance(what, str) else int(what)))
 
 
-def ck_mech_jit_source(mech) -> str:
+def ck_mech_jit_source(mech, kc_ann=None) -> str:
     """Generated CUDA source of the specialised kernel for `mech` (needs no GPU)."""
-    desc, keep = make_desc(mech)
+    desc, keep = make_desc(mech, kc_ann)
     n = _lib.ck_mech_jit_source(C.byref(desc), None, 0)
     if n < 0:
         raise CkError(4, _lib.ck_last_error().decode())
@@ -166,9 +173,10 @@ def _u8(a):
     return np.ascontiguousarray(a, dtype=np.uint8)
 
 
-def make_desc(mech):
-    """ck_mech_desc from any object with ckgen.Mechanism's array attributes.
-    Returns (desc, keepalive) -- keepalive owns the host arrays the desc points to."""
+def make_desc(mech, kc_ann=None):
+    """ck_mech_desc from any object with ckgen.Mechanism's array attributes (and, optionally,
+    a ck_kc_ann from one with ckgen.KcAnn's).  Returns (desc, keepalive) -- keepalive owns the
+    host arrays the desc points to."""
     S, R = int(mech.nu_reac.shape[0]), int(mech.nu_reac.shape[1])
     keep = dict(
         mol_weight=_f64(mech.mol_weight), nu_reac=_f64(mech.nu_reac), nu_prod=_f64(mech.nu_prod),
@@ -187,14 +195,30 @@ def make_desc(mech):
     d.n_species, d.n_reactions, d.p_ref = S, R, float(mech.p_ref)
     for name, arr in keep.items():
         setattr(d, name, arr.ctypes.data_as(_bp if arr.dtype == np.uint8 else _dp))
+    if kc_ann is not None:
+        NL, NH, NI = int(kc_ann.n_layers), int(kc_ann.n_hidden), int(kc_ann.n_in)
+        ka = dict(in_mean=_f64(kc_ann.in_mean), in_std=_f64(kc_ann.in_std), W_in=_f64(kc_ann.W_in),
+                  B=_f64(kc_ann.B), W_hid=_f64(kc_ann.W_hid), W_out=_f64(kc_ann.W_out),
+                  B_out=_f64(kc_ann.B_out), out_mean=_f64(kc_ann.out_mean), out_std=_f64(kc_ann.out_std))
+        ann_shapes = dict(in_mean=(NI,), in_std=(NI,), W_in=(NI, NH), B=(NL, NH), W_hid=(NL - 1, NH, NH),
+                          W_out=(NH, R), B_out=(R,), out_mean=(R,), out_std=(R,))
+        for name, shp in ann_shapes.items():
+            if ka[name].shape != shp:
+                raise ValueError("kc_ann.%s has shape %s, expected %s" % (name, ka[name].shape, shp))
+        a = _Ann()
+        a.n_in, a.n_layers, a.n_hidden, a.activation = NI, NL, NH, int(kc_ann.activation)
+        for name, arr in ka.items():
+            setattr(a, name, arr.ctypes.data_as(_dp))
+        keep["_ann_arrays"], keep["_ann"] = ka, a
+        d.kc_ann = C.pointer(a)
     return d, keep
 
 
 class Mechanism:
     """Owns a ck_mech handle created from a mechanism's arrays."""
 
-    def __init__(self, mech):
-        desc, keep = make_desc(mech)
+    def __init__(self, mech, kc_ann=None):
+        desc, keep = make_desc(mech, kc_ann)
         self.handle = ck_mech_create(desc)
         del keep                      # the library copied everything it needs
         self.S = ck_mech_info(self.handle, "S")

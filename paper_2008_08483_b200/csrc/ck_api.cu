@@ -92,6 +92,29 @@ int validate(const ck_mech_desc *d) {
         return fail(CK_EINVAL, "Troe temperatures must be > 0 (T** may be +INF)");
     }
   }
+  if (const ck_kc_ann *a = d->kc_ann) {
+    if ((a->n_in != 1 && a->n_in != 6) || a->n_layers < 1 || a->n_layers > 8 || a->n_hidden < 1 ||
+        a->n_hidden > 64 || (a->activation != CK_ANN_RELU && a->activation != CK_ANN_ELU))
+      return fail(CK_EINVAL, "kc_ann: n_in must be 1 or 6, 1 <= n_layers <= 8, 1 <= n_hidden <= 64, activation 0 or 1");
+    if (!a->in_mean || !a->in_std || !a->W_in || !a->B || !a->W_out || !a->B_out || !a->out_mean ||
+        !a->out_std || (a->n_layers > 1 && !a->W_hid))
+      return fail(CK_EINVAL, "kc_ann: a weight array pointer is NULL");
+    auto finite = [](const double *p, size_t n) {
+      for (size_t i = 0; i < n; ++i) if (!std::isfinite(p[i])) return false;
+      return true;
+    };
+    const size_t NI = a->n_in, NH = a->n_hidden, NL = a->n_layers;
+    if (!finite(a->in_mean, NI) || !finite(a->in_std, NI) || !finite(a->W_in, NI * NH) || !finite(a->B, NL * NH) ||
+        (NL > 1 && !finite(a->W_hid, (NL - 1) * NH * NH)) || !finite(a->W_out, NH * R) || !finite(a->B_out, R) ||
+        !finite(a->out_mean, R) || !finite(a->out_std, R))
+      return fail(CK_EINVAL, "kc_ann: weights must be finite");
+    for (size_t i = 0; i < NI; ++i)
+      if (!(a->in_std[i] > 0.0)) return fail(CK_EINVAL, "kc_ann: in_std must be > 0");
+    // the hidden layers' weights are constant-bank operands of the kernel (64 KB bank, shared
+    // with the falloff table and the compiler's own constants)
+    if ((2 * NI + NI * NH + NL * NH + (NL - 1) * NH * NH) * sizeof(double) > 40960)
+      return fail(CK_EUNSUPPORTED, "kc_ann: hidden-layer weights exceed 40 KB (e.g. 3 layers of 50 neurons)");
+  }
   return CK_OK;
 }
 
@@ -149,33 +172,35 @@ std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk,
   const bool fits = 2 * S + 48 <= 255;
   const int rest = std::max(48, env_int("CK_JIT_REST", fits ? 144 : 166));
   const int sreg_forced = std::min(S, env_int("CK_JIT_SREG", -1));   // tuning / test knob
-  const size_t tab_bytes = (size_t)spec.n_ranges * R * 10 * sizeof(double);   // R includes padding
+  const size_t tab_bytes = (size_t)spec.tab_ranges * R * spec.row * sizeof(double);   // R includes padding
   const int nt_forced = env_int("CK_JIT_NT", 0), b_forced = env_int("CK_JIT_MINB", 0);
   int best_nt = 0, best_b = 0, best_cap = 0, best_sreg = 0;
   bool best_tab = false;
   size_t best_smem = 0;
   auto smem_of = [&](int nt, int s_reg, bool tab_smem) {
-    return (size_t)(S + (S - s_reg)) * (nt + 8) * 8 + (32 + 256) * 8 + (size_t)spec.n_ranges * S * 12 * 8 +
-           (tab_smem ? tab_bytes : (size_t)(nt / 32) * 2 * spec.n_ranges * spec.block * 10 * 8) + 16;
+    return (size_t)(S + (S - s_reg) + spec.ann_nhp) * (nt + 8) * 8 + (32 + 256) * 8 + (size_t)spec.n_ranges * S * 12 * 8 +
+           (tab_smem ? tab_bytes : (size_t)(nt / 32) * 2 * spec.tab_ranges * spec.block * spec.row * 8) + 16;
   };
   const bool all_regs = sreg_forced < 0 ? fits : (sreg_forced == S);
   if (all_regs) {
     const int regs_wanted = std::min(255, 2 * S + rest);
-    for (int tab_smem = 1; tab_smem >= 0 && best_nt == 0; --tab_smem)
-      for (int nt : {512, 448, 384, 320, 256, 192, 128, 64}) {
-        if (nt_forced && nt != nt_forced) continue;
-        for (int b = 1; b <= 4; ++b) {
+    for (int nt : {512, 448, 384, 320, 256, 192, 128, 64}) {
+      if (nt_forced && nt != nt_forced) continue;
+      for (int b = 1; b <= 4; ++b)
+        for (int tab_smem = 1; tab_smem >= 0; --tab_smem) {
           if (b_forced && b != b_forced) continue;
           const int regcap = std::min(255, (65536 / (nt * b)) / 8 * 8);
           if (regcap < 2 * S + 48) continue;
           const size_t smem = smem_of(nt, S, tab_smem != 0);
           if (smem > smem_blk || b * (smem + 1024) > smem_sm) continue;
           const int cap = std::min(regcap, regs_wanted);
+          // registers, then resident threads, then larger blocks, then the table resident in smem
           const bool better = cap > best_cap || (cap == best_cap && nt * b > best_nt * best_b) ||
-                              (cap == best_cap && nt * b == best_nt * best_b && nt > best_nt);
+                              (cap == best_cap && nt * b == best_nt * best_b && nt > best_nt) ||
+                              (cap == best_cap && nt == best_nt && b == best_b && (tab_smem != 0) > best_tab);
           if (better) { best_nt = nt; best_b = b; best_cap = cap; best_tab = tab_smem != 0; best_smem = smem; best_sreg = S; }
         }
-      }
+    }
   } else {
     for (int nt : {512, 448, 384, 320, 256, 192, 128, 64})
       for (int b = 1; b <= 2; ++b)
@@ -199,6 +224,7 @@ std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk,
   if (const char *e = std::getenv("CK_JIT_M")) spec.m_dmma = std::string(e) != "dfma";
   if (const char *e = std::getenv("CK_JIT_SYNC")) spec.sync_every = std::atoi(e);
   if (const char *e = std::getenv("CK_JIT_KCONST")) spec.kconst = std::atoi(e) != 0;
+  if (const char *e = std::getenv("CK_JIT_KC")) spec.kc_none = std::string(e) == "none";
   *smem_out = best_smem;
   return "";
 }
@@ -216,6 +242,7 @@ void finalize_jit(const ck_mech_desc *d, HostBuild *hb, const std::vector<double
   const int S = d->n_species, R = d->n_reactions;
   ck::JitSpec &spec = hb->spec;
   const int n_ranges = hb->n_ranges_tmp;
+  const int tab_ranges = spec.tab_ranges, ROW = spec.row;
   std::vector<ck::JitReaction> orig;
   orig.swap(spec.rxn);
   const std::vector<double> tab_orig = hb->jit_tab;
@@ -238,7 +265,7 @@ void finalize_jit(const ck_mech_desc *d, HostBuild *hb, const std::vector<double
   }
   const int RP = (int)order.size();
   spec.R = RP;
-  hb->jit_tab.assign((size_t)n_ranges * RP * 10, 0.0);
+  hb->jit_tab.assign((size_t)tab_ranges * RP * ROW, 0.0);
   spec.falloff.clear();
   std::vector<int> m_rows;                // original reaction of each M row (-1: null)
   for (int jj = 0; jj < RP; ++jj) {
@@ -249,14 +276,14 @@ void finalize_jit(const ck_mech_desc *d, HostBuild *hb, const std::vector<double
     r.index = j;
     r.type = g / 2 == 0 ? 0 : (g / 2 == 1 ? 1 : (j >= 0 ? orig[j].type : 2));
     r.reversible = (g % 2 == 0);
-    for (int rg = 0; rg < n_ranges; ++rg) {
-      double *row = &hb->jit_tab[((size_t)rg * RP + jj) * 10];
+    for (int rg = 0; rg < tab_ranges; ++rg) {
+      double *row = &hb->jit_tab[((size_t)rg * RP + jj) * ROW];
       if (j >= 0) {
-        const double *src = &tab_orig[((size_t)rg * R + j) * 10];
-        for (int i = 0; i < 10; ++i) row[i] = src[i];
+        const double *src = &tab_orig[((size_t)rg * R + j) * ROW];
+        for (int i = 0; i < ROW; ++i) row[i] = src[i];
       } else {
         row[0] = -5000.0;   // null reaction: ln q = -5000, the rate underflows to ~1e-307
-        row[3] = -5000.0;
+        if (!spec.kc_ann) row[3] = -5000.0;   // (with the ANN, ln k_r = ln k_f + row[3] + ...)
       }
     }
     if (g >= 2) {           // third-body and falloff reactions: a row of M each, in this order
@@ -365,8 +392,25 @@ void build_host(const ck_mech_desc *d, HostBuild *hb, size_t smem_sm = kSmemPerS
   std::vector<int> m_rows;       // reaction index of each row of M
   ck::JitSpec &spec = hb->spec;
   spec.S = S; spec.R = R; spec.n_ranges = n_ranges;
+  const ck_kc_ann *ann = d->kc_ann;
+  spec.kc_ann = ann != nullptr;
+  if (ann) {
+    spec.ann_nin = ann->n_in; spec.ann_nl = ann->n_layers; spec.ann_nh = ann->n_hidden;
+    spec.ann_act = ann->activation; spec.ann_nhp = (ann->n_hidden + 1) & ~1;
+    spec.tab_ranges = 1; spec.row = 4 + spec.ann_nhp;
+    // constant-bank block of the hidden layers: mean | 1/std | W_in | B | W_hid
+    const int NI = ann->n_in, NH = ann->n_hidden, NL = ann->n_layers;
+    spec.ann_const.assign(ann->in_mean, ann->in_mean + NI);
+    for (int i = 0; i < NI; ++i) spec.ann_const.push_back(1.0 / ann->in_std[i]);
+    spec.ann_const.insert(spec.ann_const.end(), ann->W_in, ann->W_in + (size_t)NI * NH);
+    spec.ann_const.insert(spec.ann_const.end(), ann->B, ann->B + (size_t)NL * NH);
+    spec.ann_const.insert(spec.ann_const.end(), ann->W_hid, ann->W_hid + (size_t)(NL - 1) * NH * NH);
+  } else {
+    spec.tab_ranges = n_ranges; spec.row = 10;
+  }
+  const int ROW = spec.row;
   std::vector<double> &jit_tab = hb->jit_tab;
-  jit_tab.assign((size_t)n_ranges * R * 10, 0.0);
+  jit_tab.assign((size_t)spec.tab_ranges * R * ROW, 0.0);
   for (int j = 0; j < R; ++j) {
     const int type = d->rxn_type ? d->rxn_type[j] : CK_ELEMENTARY;
     const int rev = d->reversible ? (d->reversible[j] != 0) : 1;
@@ -422,10 +466,19 @@ void build_host(const ck_mech_desc *d, HostBuild *hb, size_t smem_sm = kSmemPerS
       for (int i = 0; i < 7; ++i) dbl.push_back((double)f[i]);
       dbl.push_back(0.0);
       // row of the specialised kernel's rate table (ck_jit_kernel.cuh)
-      double *row = &jit_tab[((size_t)r * R + j) * 10];
+      if (ann) continue;
+      double *row = &jit_tab[((size_t)r * R + j) * ROW];
       row[0] = d->ln_A[j]; row[1] = d->b[j]; row[2] = -d->Ea_over_R[j];
       row[3] = (double)f[0]; row[4] = (double)f[1]; row[5] = (double)f[6];
       row[6] = (double)f[2]; row[7] = (double)f[3]; row[8] = (double)f[4]; row[9] = (double)f[5];
+    }
+    if (ann) {
+      // approximate ANN (Eq. 12): ln Kc~_j = mu_j + sigma_j (B_out,j + sum_h x_h W_out[h][j]);
+      // ln k_r = ln k_f - ln Kc~ (Eq. 7): output layer and de-standardisation folded into the row
+      double *row = &jit_tab[(size_t)j * ROW];
+      row[0] = d->ln_A[j]; row[1] = d->b[j]; row[2] = -d->Ea_over_R[j];
+      row[3] = -(ann->out_mean[j] + ann->out_std[j] * ann->B_out[j]);
+      for (int h = 0; h < ann->n_hidden; ++h) row[4 + h] = -ann->out_std[j] * ann->W_out[(size_t)h * R + j];
     }
     {
       ck::JitReaction jr;
@@ -503,7 +556,12 @@ void build_host(const ck_mech_desc *d, HostBuild *hb, size_t smem_sm = kSmemPerS
 // auto mode (m->jit_note says why).
 int setup_jit(ck_mech *m, ck::JitSpec &spec, const std::string &why, size_t smem) {
   const char *mode_env = std::getenv("CK_KERNEL");
-  const std::string mode = mode_env ? mode_env : "auto";
+  std::string mode = mode_env ? mode_env : "auto";
+  if (spec.kc_ann) {
+    // the approximate-ANN layer exists only in the specialised kernel
+    if (mode == "generic") return fail(CK_EUNSUPPORTED, "kc_ann needs the specialised kernel (CK_KERNEL=generic)");
+    mode = "jit";
+  }
   if (mode == "generic") { m->jit_note = "CK_KERNEL=generic"; return CK_OK; }
   if (mode != "auto" && mode != "jit") return fail(CK_EINVAL, "CK_KERNEL must be auto, generic or jit");
   const bool required = (mode == "jit");

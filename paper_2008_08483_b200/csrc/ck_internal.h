@@ -8,6 +8,7 @@
 #include <utility>
 #include <vector>
 
+#include "../../include/ck.h"
 #include "ck_program.h"
 
 namespace ck {
@@ -36,6 +37,11 @@ struct JitSpec {
   int block = 4;               // reactions per block of the core
   int s_reg = 0;               // species with register accumulators (internal order); rest in smem
   std::vector<int> perm;       // internal species -> row of Y / wdot; empty = identity
+  int tab_ranges = 1, row = 10;  // rate table: ranges and doubles per row
+  bool kc_none = false;        // measurement-only ablation: no equilibrium layer (CK_JIT_KC=none)
+  bool kc_ann = false;         // approximate ANN for ln Kc in place of the exact layer
+  int ann_nin = 0, ann_nl = 0, ann_nh = 0, ann_nhp = 0, ann_act = 0;
+  std::vector<double> ann_const;   // mean | 1/std | W_in | B | W_hid
   bool kconst = false;         // polynomial coefficients as constant-bank operands (else literals)
   int group_end[6] = {0, 0, 0, 0, 0, 0};   // end block of (elementary, three-body, falloff) x (rev, irrev)
   std::vector<JitReaction> rxn;

@@ -115,6 +115,8 @@ std::string jit_generate_source(const JitSpec &s) {
     << "\n#define CK_M_DMMA " << (s.m_dmma ? 1 : 0) << "\n#define CK_KCONST " << (s.kconst ? 1 : 0) << "\n#define CK_SYNC_EVERY " << s.sync_every
     << "\n#define CK_B " << s.block << "\n#define CK_NBLK " << (int)s.rxn.size() / s.block
     << "\n#define CK_G_TB0 " << s.group_end[1] << "\n#define CK_G_FO0 " << s.group_end[3]
+    << "\n#define CK_TAB_NRANGES " << s.tab_ranges << "\n#define CK_ROW " << s.row
+    << "\n#define CK_KC_ANN " << (s.kc_ann ? 1 : 0) << "\n#define CK_KC_NONE " << (s.kc_none ? 1 : 0)
     << "\n#define CK_SREG " << s.s_reg << "\n#define CK_PERM " << (s.perm.empty() ? 0 : 1) << "\n";
   if (!s.perm.empty()) {
     o << "__constant__ int ck_c_perm[" << s.perm.size() << "] = {";
@@ -127,6 +129,11 @@ std::string jit_generate_source(const JitSpec &s) {
     if (v.empty()) o << "0.0";
     o << "};\n";
   };
+  if (s.kc_ann) {
+    o << "#define CK_ANN_NIN " << s.ann_nin << "\n#define CK_ANN_NL " << s.ann_nl << "\n#define CK_ANN_NH "
+      << s.ann_nh << "\n#define CK_ANN_NHP " << s.ann_nhp << "\n#define CK_ANN_ACT " << s.ann_act << "\n";
+    emit("ck_c_ann", s.ann_const);
+  }
   emit("ck_c_rangeT", s.range_T);
   emit("ck_c_falloff", s.falloff);
   const std::string text(kKernelText);
