@@ -723,7 +723,17 @@ extern "C" int ck_source_terms(const ck_mech *m, const double *T, const double *
   if (m->jit_kernel) {
     ck::JitParams prm = m->jit_params;
     prm.T = T; prm.P = P; prm.Y = Y; prm.wdot = wdot; prm.dTdt = dTdt; prm.N = N;
-    const int64_t n_tiles = (N + m->jit_threads - 1) / m->jit_threads;
+    // Balanced tiles: the fewest waves of full tiles the grid needs, then the tile size that
+    // spreads the cells evenly over grid x waves (a multiple of the warp size), so that a batch
+    // just past a multiple of the grid does not pay for a nearly empty last wave and a small
+    // batch uses every SM.
+    const int64_t nt = m->jit_threads;
+    const int64_t waves = ((N + nt - 1) / nt + m->jit_grid_max - 1) / m->jit_grid_max;
+    int64_t tc = (N + m->jit_grid_max * waves - 1) / (m->jit_grid_max * waves);
+    tc = std::min<int64_t>(nt, (tc + 31) / 32 * 32);
+    if (const char *e = std::getenv("CK_JIT_TILE")) tc = std::min<int64_t>(nt, std::max(32, std::atoi(e) / 32 * 32));
+    prm.tile_cells = (int)tc;
+    const int64_t n_tiles = (N + tc - 1) / tc;
     const int grid = (int)std::min<int64_t>(n_tiles, m->jit_grid_max);
     void *args[] = {&prm};
     ce = cudaLaunchKernel((const void *)m->jit_kernel, dim3(grid), dim3(m->jit_threads), args,

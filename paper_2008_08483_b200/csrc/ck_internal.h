@@ -21,6 +21,7 @@ struct JitParams {
   const double *T, *P, *Y;
   double *wdot, *dTdt;
   long long N;
+  int tile_cells;
 };
 
 struct JitReaction {
