@@ -317,6 +317,8 @@ void finalize_jit(const ck_mech_desc *d, HostBuild *hb, const std::vector<double
     spec.perm = perm;
   }
   for (int k = 0; k < S; ++k) inv[perm[k]] = k;
+  spec.mol_weight.resize(S);
+  for (int k = 0; k < S; ++k) spec.mol_weight[k] = d->mol_weight[perm[k]];
   for (ck::JitReaction &r : spec.rxn) {
     for (auto &e : r.reac) e.first = inv[e.first];
     for (auto &e : r.prod) e.first = inv[e.first];
@@ -593,6 +595,7 @@ int setup_jit(ck_mech *m, ck::JitSpec &spec, const std::string &why, size_t smem
     return give_up(std::string("loading the specialised kernel: ") + cudaGetErrorString(ce));
   }
   m->jit_threads = spec.threads; m->jit_blocks_per_sm = spec.min_blocks; m->jit_smem = smem;
+  m->jit_spec = spec;
   m->jit_grid_max = m->num_sms * spec.min_blocks;
   const size_t elems = (size_t)m->jit_grid_max * std::max(spec.n_mb, 1) * ck::kMBlock * spec.threads;
   ce = cudaMalloc((void **)&m->d_jit_scratch, elems * sizeof(double));
@@ -705,9 +708,14 @@ extern "C" void ck_mech_destroy(ck_mech *m) {
   if (m->d_stage) cudaFree(m->d_stage);
   if (m->d_jit_scratch) cudaFree(m->d_jit_scratch);
   if (m->rk4_graph) cudaGraphExecDestroy(m->rk4_graph);
+  if (m->rk4_lib) cudaLibraryUnload(m->rk4_lib);
   if (m->d_rk4) cudaFree(m->d_rk4);
   if (m->jit_lib) cudaLibraryUnload(m->jit_lib);
   delete m;
+}
+
+namespace {
+int jit_tiling(const ck_mech *m, int64_t N, int *tile_cells);
 }
 
 extern "C" int ck_source_terms(const ck_mech *m, const double *T, const double *P,
@@ -727,14 +735,7 @@ extern "C" int ck_source_terms(const ck_mech *m, const double *T, const double *
     // spreads the cells evenly over grid x waves (a multiple of the warp size), so that a batch
     // just past a multiple of the grid does not pay for a nearly empty last wave and a small
     // batch uses every SM.
-    const int64_t nt = m->jit_threads;
-    const int64_t waves = ((N + nt - 1) / nt + m->jit_grid_max - 1) / m->jit_grid_max;
-    int64_t tc = (N + m->jit_grid_max * waves - 1) / (m->jit_grid_max * waves);
-    tc = std::min<int64_t>(nt, (tc + 31) / 32 * 32);
-    if (const char *e = std::getenv("CK_JIT_TILE")) tc = std::min<int64_t>(nt, std::max(32, std::atoi(e) / 32 * 32));
-    prm.tile_cells = (int)tc;
-    const int64_t n_tiles = (N + tc - 1) / tc;
-    const int grid = (int)std::min<int64_t>(n_tiles, m->jit_grid_max);
+    const int grid = jit_tiling(m, N, &prm.tile_cells);
     void *args[] = {&prm};
     ce = cudaLaunchKernel((const void *)m->jit_kernel, dim3(grid), dim3(m->jit_threads), args,
                           m->jit_smem, (cudaStream_t)stream);
@@ -777,10 +778,61 @@ extern "C" int ck_source_terms_host(ck_mech *m, const double *T, const double *P
 
 namespace {
 
-// one RK4 step on `st`: 4 x (source terms at the current stage state + stage kernel)
+// The explicit-RK4 stage variant of the specialised kernel (CK_RK4 in ck_jit_kernel.cuh),
+// compiled on first use.  Leaves m->rk4_kernel NULL if there is no specialised kernel, if
+// CK_RK4_FUSED=0, or if the compilation fails (the separate stage kernels are used then).
+void ensure_rk4_kernel(ck_mech *m) {
+  if (m->rk4_tried) return;
+  m->rk4_tried = true;
+  if (!m->jit_kernel) return;
+  if (const char *e = std::getenv("CK_RK4_FUSED")) if (std::atoi(e) == 0) return;
+  ck::JitSpec spec = m->jit_spec;
+  spec.rk4 = true;
+  std::vector<char> cubin;
+  if (!ck::jit_compile(ck::jit_generate_source(spec), &cubin).empty()) return;
+  if (cudaLibraryLoadData(&m->rk4_lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0) != cudaSuccess) {
+    m->rk4_lib = nullptr;
+    return;
+  }
+  if (cudaLibraryGetKernel(&m->rk4_kernel, m->rk4_lib, "ck_source_terms_jit") != cudaSuccess ||
+      cudaKernelSetAttributeForDevice(m->rk4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m->jit_smem,
+                                      m->device) != cudaSuccess) {
+    cudaLibraryUnload(m->rk4_lib);
+    m->rk4_lib = nullptr; m->rk4_kernel = nullptr;
+  }
+  cudaGetLastError();
+}
+
+// tile size and grid of a launch of the specialised kernel (balanced tiles, see ck_source_terms)
+int jit_tiling(const ck_mech *m, int64_t N, int *tile_cells) {
+  const int64_t nt = m->jit_threads;
+  const int64_t waves = ((N + nt - 1) / nt + m->jit_grid_max - 1) / m->jit_grid_max;
+  int64_t tc = (N + m->jit_grid_max * waves - 1) / (m->jit_grid_max * waves);
+  tc = std::min<int64_t>(nt, (tc + 31) / 32 * 32);
+  if (const char *e = std::getenv("CK_JIT_TILE")) tc = std::min<int64_t>(nt, std::max(32, std::atoi(e) / 32 * 32));
+  *tile_cells = (int)tc;
+  return (int)std::min<int64_t>((N + tc - 1) / tc, m->jit_grid_max);
+}
+
+// one RK4 step on `st`: 4 fused stage launches, or 4 x (source terms + stage kernel)
 int rk4_enqueue_step(ck_mech *m, double *T, const double *P, double *Y, int64_t N, double dt, cudaStream_t st) {
   const int64_t S = m->dev.S;
   double *Ts = m->d_rk4, *Ys = Ts + N, *wd = Ys + S * N, *dT = wd + S * N, *aT = dT + N, *aY = aT + N;
+  if (m->rk4_kernel) {
+    for (int stage = 1; stage <= 4; ++stage) {
+      ck::JitParams prm = m->jit_params;
+      prm.T = stage == 1 ? T : Ts; prm.P = P; prm.Y = stage == 1 ? Y : Ys; prm.N = N;
+      prm.wdot = nullptr; prm.dTdt = nullptr;
+      prm.rk_stage = stage; prm.rk_dt = dt; prm.rk_T0 = T; prm.rk_Y0 = Y; prm.rk_accT = aT; prm.rk_accY = aY;
+      prm.rk_Tout = stage == 4 ? T : Ts; prm.rk_Yout = stage == 4 ? Y : Ys;
+      const int grid = jit_tiling(m, N, &prm.tile_cells);
+      void *args[] = {&prm};
+      cudaError_t ce = cudaLaunchKernel((const void *)m->rk4_kernel, dim3(grid), dim3(m->jit_threads), args,
+                                        m->jit_smem, st);
+      if (ce != cudaSuccess) return fail_cuda(ce, "rk4 fused stage launch");
+    }
+    return CK_OK;
+  }
   for (int stage = 1; stage <= 4; ++stage) {
     const double *Tin = stage == 1 ? T : Ts, *Yin = stage == 1 ? Y : Ys;
     if (int rc = ck_source_terms(m, Tin, P, Yin, N, wd, dT, (void *)st)) return rc;
@@ -811,6 +863,7 @@ extern "C" int ck_rk4_integrate(ck_mech *m, double *T, const double *P, double *
     if (ce != cudaSuccess) return fail(CK_ENOMEM, std::string("cudaMalloc rk4 workspace: ") + cudaGetErrorString(ce));
     m->rk4_cells = N;
   }
+  ensure_rk4_kernel(m);
   if (!use_graph) {
     for (int64_t s = 0; s < n_steps; ++s)
       if (int rc = rk4_enqueue_step(m, T, P, Y, N, dt, st)) return rc;

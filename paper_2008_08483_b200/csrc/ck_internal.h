@@ -22,6 +22,11 @@ struct JitParams {
   double *wdot, *dTdt;
   long long N;
   int tile_cells;
+  int rk_stage;
+  double rk_dt;
+  const double *rk_T0, *rk_Y0;
+  double *rk_accT, *rk_accY;
+  double *rk_Tout, *rk_Yout;
 };
 
 struct JitReaction {
@@ -39,6 +44,8 @@ struct JitSpec {
   int s_reg = 0;               // species with register accumulators (internal order); rest in smem
   std::vector<int> perm;       // internal species -> row of Y / wdot; empty = identity
   int tab_ranges = 1, row = 10;  // rate table: ranges and doubles per row
+  bool rk4 = false;            // the explicit-RK4 stage variant of the kernel (ck_rk4_integrate)
+  std::vector<double> mol_weight;  // [S], internal order (RK4 variant)
   bool kc_none = false;        // measurement-only ablation: no equilibrium layer (CK_JIT_KC=none)
   bool kc_ann = false;         // approximate ANN for ln Kc in place of the exact layer
   int ann_nin = 0, ann_nl = 0, ann_nh = 0, ann_nhp = 0, ann_act = 0;
@@ -75,6 +82,10 @@ struct ck_mech {
   int jit_threads = 0, jit_blocks_per_sm = 0, jit_grid_max = 0, jit_s_reg = 0;
   size_t jit_smem = 0;
   double *d_jit_scratch = nullptr;
+  ck::JitSpec jit_spec;       // kept to compile the RK4 stage variant on first use
+  cudaLibrary_t rk4_lib = nullptr;
+  cudaKernel_t rk4_kernel = nullptr;
+  bool rk4_tried = false;
   std::string jit_note;       // why the specialised kernel is not in use, if so
   // staging for ck_source_terms_host
   double *d_stage = nullptr;

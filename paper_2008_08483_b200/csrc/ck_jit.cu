@@ -116,7 +116,7 @@ std::string jit_generate_source(const JitSpec &s) {
     << "\n#define CK_B " << s.block << "\n#define CK_NBLK " << (int)s.rxn.size() / s.block
     << "\n#define CK_G_TB0 " << s.group_end[1] << "\n#define CK_G_FO0 " << s.group_end[3]
     << "\n#define CK_TAB_NRANGES " << s.tab_ranges << "\n#define CK_ROW " << s.row
-    << "\n#define CK_KC_ANN " << (s.kc_ann ? 1 : 0) << "\n#define CK_KC_NONE " << (s.kc_none ? 1 : 0)
+    << "\n#define CK_RK4 " << (s.rk4 ? 1 : 0) << "\n#define CK_KC_ANN " << (s.kc_ann ? 1 : 0) << "\n#define CK_KC_NONE " << (s.kc_none ? 1 : 0)
     << "\n#define CK_SREG " << s.s_reg << "\n#define CK_PERM " << (s.perm.empty() ? 0 : 1) << "\n";
   if (!s.perm.empty()) {
     o << "__constant__ int ck_c_perm[" << s.perm.size() << "] = {";
@@ -134,6 +134,7 @@ std::string jit_generate_source(const JitSpec &s) {
       << s.ann_nh << "\n#define CK_ANN_NHP " << s.ann_nhp << "\n#define CK_ANN_ACT " << s.ann_act << "\n";
     emit("ck_c_ann", s.ann_const);
   }
+  if (s.rk4) emit("ck_c_W", s.mol_weight);
   emit("ck_c_rangeT", s.range_T);
   emit("ck_c_falloff", s.falloff);
   const std::string text(kKernelText);

@@ -26,12 +26,21 @@ def ck():
     return ck
 
 
+@pytest.fixture(autouse=True, params=["fused", "separate"])
+def stage_variant(request, monkeypatch):
+    """Every test runs with the RK stage update fused into the specialised source-term kernel's
+    epilogue (the default) and with the separate stage kernels (CK_RK4_FUSED=0, also what the
+    generic kernel uses)."""
+    monkeypatch.setenv("CK_RK4_FUSED", "1" if request.param == "fused" else "0")
+    return request.param
+
+
 def to_dev(*arrays):
     return [torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0") for a in arrays]
 
 
 @pytest.mark.parametrize("use_graph", [False, True])
-@pytest.mark.parametrize("cfg_name,N,steps", [("tiny_1k", 1000, 25), ("mid_rk4", 600, 6)])
+@pytest.mark.parametrize("cfg_name,N,steps", [("tiny_1k", 1000, 25), ("mid_rk4", 600, 6), ("mid_rk4", 333, 2)])
 def test_trajectory_parity_on_tamed_mechanism(ck, cfg_name, N, steps, use_graph):
     cfg = ckgen.CONFIGS[cfg_name]
     mech = tame(ckgen.mechanism(cfg.mech))
@@ -103,3 +112,19 @@ def test_config5_stagewise_parity_on_the_synthetic_mechanism(ck):
             wr, dr, _ = oracle.source_terms(om, Th[idx], P[idx], np.ascontiguousarray(Yh[:, idx]))
             rw, rt = parity_violations(w[:, idx].cpu().numpy(), d[idx].cpu().numpy(), wr, dr)
             assert rw <= 1.0 and rt <= 1.0, (upto, rw, rt)
+
+
+def test_large_mechanism_one_step(ck):
+    """S=111: cold accumulators and the species permutation through the fused stage epilogue."""
+    cfg = ckgen.CONFIGS["large_256k"]
+    mech = tame(ckgen.mechanism(cfg.mech))
+    T, P, Y = ckgen.states(cfg, N=300)
+    Tr, Yr = reactor.integrate(oracle.OracleMechanism(mech), mech.mol_weight, T, P, Y, 1e-9, 2)
+    Td, Pd, Yd = to_dev(T, P, Y)
+    with ck.Mechanism(mech) as gm:
+        gm.rk4_integrate(Td, Pd, Yd, 1e-9, 2, stream=torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+    dY, dYr = Yd.cpu().numpy() - Y, Yr - Y
+    assert np.abs(dYr).max() > 1e-8
+    assert (np.abs(dY - dYr) <= 1e-9 * np.abs(dYr).max(0, keepdims=True) + 4e-16).all()
+    assert np.abs((Td.cpu().numpy() - T) - (Tr - T)).max() <= 1e-9 * np.abs(Tr - T).max() + 1e-13 * T.max()
