@@ -133,7 +133,12 @@ int ck_source_terms(const ck_mech *m, const double *T, const double *P, const do
                     int64_t N, double *wdot, double *dTdt, void *stream);
 
 /* Same computation with HOST buffers: copies T, P, Y to the device, runs
- * ck_source_terms and copies wdot, dTdt back, all on `stream`, then synchronises it.
+ * ck_source_terms and copies wdot, dTdt back, then synchronises `stream`.  Batches of
+ * 2^17 cells or more are split into up to 16 chunks of cells that are pipelined: a chunk's
+ * rows are copied up on a stream owned by the handle while the previous chunk computes on
+ * `stream` and the one before is copied back on a second owned stream; the work starts
+ * after everything queued on `stream` at the call and `stream` ends after the last copy
+ * (environment CK_HOST_CHUNKS=n overrides the chunk count, 1 = everything on `stream`).
  * Pinned host memory makes the copies asynchronous; pageable memory also works.
  * Device staging buffers are owned by the handle and grow on demand. */
 int ck_source_terms_host(ck_mech *m, const double *T, const double *P, const double *Y,

@@ -706,6 +706,9 @@ extern "C" void ck_mech_destroy(ck_mech *m) {
   if (m->d_tables) cudaFree(m->d_tables);
   if (m->d_scratch) cudaFree(m->d_scratch);
   if (m->d_stage) cudaFree(m->d_stage);
+  if (m->host_in) cudaStreamDestroy(m->host_in);
+  if (m->host_out) cudaStreamDestroy(m->host_out);
+  for (cudaEvent_t e : m->host_ev) if (e) cudaEventDestroy(e);
   if (m->d_jit_scratch) cudaFree(m->d_jit_scratch);
   if (m->rk4_graph) cudaGraphExecDestroy(m->rk4_graph);
   if (m->rk4_lib) cudaLibraryUnload(m->rk4_lib);
@@ -762,16 +765,59 @@ extern "C" int ck_source_terms_host(ck_mech *m, const double *T, const double *P
     if (ce != cudaSuccess) return fail(CK_ENOMEM, std::string("cudaMalloc staging: ") + cudaGetErrorString(ce));
     m->stage_cells = N;
   }
-  double *dT = m->d_stage, *dP = dT + N, *dY = dP + N, *dW = dY + S * N, *dD = dW + S * N;
-  const size_t col = (size_t)N * sizeof(double);
-  if ((ce = cudaMemcpyAsync(dT, T, col, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-      (ce = cudaMemcpyAsync(dP, P, col, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-      (ce = cudaMemcpyAsync(dY, Y, col * S, cudaMemcpyHostToDevice, st)) != cudaSuccess)
-    return fail_cuda(ce, "host to device copy");
-  if (int rc = ck_source_terms(m, dT, dP, dY, N, dW, dD, stream)) return rc;
-  if ((ce = cudaMemcpyAsync(wdot, dW, col * S, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
-      (ce = cudaMemcpyAsync(dTdt, dD, col, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
-    return fail_cuda(ce, "device to host copy");
+  // Chunks of cells pipelined over three streams: chunk c's rows go up on the handle's
+  // copy-in stream while chunk c-1 computes on `stream` and chunk c-2's results come down on
+  // the copy-out stream (PCIe is full duplex, so the two copy directions overlap as well).
+  // Each chunk has its own compact SoA region of the staging buffer: T | P | Y[S] | wdot[S] | dTdt.
+  int64_t n_chunks = N / 65536;
+  if (n_chunks > CK_HOST_CHUNKS) n_chunks = CK_HOST_CHUNKS;
+  if (const char *e = std::getenv("CK_HOST_CHUNKS")) n_chunks = std::atoi(e);
+  if (n_chunks < 1) n_chunks = 1;
+  if (n_chunks > CK_HOST_CHUNKS) n_chunks = CK_HOST_CHUNKS;
+  if (n_chunks > 1 && !m->host_in) {
+    if ((ce = cudaStreamCreateWithFlags(&m->host_in, cudaStreamNonBlocking)) != cudaSuccess ||
+        (ce = cudaStreamCreateWithFlags(&m->host_out, cudaStreamNonBlocking)) != cudaSuccess)
+      return fail_cuda(ce, "cudaStreamCreate (host pipeline)");
+    for (int i = 0; i < 2 * CK_HOST_CHUNKS + 2; ++i)
+      if ((ce = cudaEventCreateWithFlags(&m->host_ev[i], cudaEventDisableTiming)) != cudaSuccess)
+        return fail_cuda(ce, "cudaEventCreate (host pipeline)");
+  }
+  const int64_t per = ((N + n_chunks - 1) / n_chunks + 255) & ~(int64_t)255;   // keeps rows 16-byte aligned
+  const size_t pitch = (size_t)N * sizeof(double);
+  cudaStream_t s_in = n_chunks > 1 ? m->host_in : st, s_out = n_chunks > 1 ? m->host_out : st;
+  if (n_chunks > 1) {
+    // the copies start after whatever the caller has queued on `stream`
+    cudaEvent_t e0 = m->host_ev[2 * CK_HOST_CHUNKS];
+    if ((ce = cudaEventRecord(e0, st)) != cudaSuccess || (ce = cudaStreamWaitEvent(s_in, e0, 0)) != cudaSuccess ||
+        (ce = cudaStreamWaitEvent(s_out, e0, 0)) != cudaSuccess)
+      return fail_cuda(ce, "host pipeline start");
+  }
+  int c = 0;
+  for (int64_t c0 = 0; c0 < N; c0 += per, ++c) {
+    const int64_t n = (N - c0 < per) ? (N - c0) : per;
+    double *dT = m->d_stage + (size_t)(2 * S + 3) * c0, *dP = dT + n, *dY = dP + n, *dW = dY + S * n, *dD = dW + S * n;
+    const size_t w = (size_t)n * sizeof(double);
+    if ((ce = cudaMemcpyAsync(dT, T + c0, w, cudaMemcpyHostToDevice, s_in)) != cudaSuccess ||
+        (ce = cudaMemcpyAsync(dP, P + c0, w, cudaMemcpyHostToDevice, s_in)) != cudaSuccess ||
+        (ce = cudaMemcpy2DAsync(dY, w, Y + c0, pitch, w, (size_t)S, cudaMemcpyHostToDevice, s_in)) != cudaSuccess)
+      return fail_cuda(ce, "host to device copy");
+    if (n_chunks > 1 && ((ce = cudaEventRecord(m->host_ev[2 * c], s_in)) != cudaSuccess ||
+                         (ce = cudaStreamWaitEvent(st, m->host_ev[2 * c], 0)) != cudaSuccess))
+      return fail_cuda(ce, "host pipeline (copy-in event)");
+    if (int rc = ck_source_terms(m, dT, dP, dY, n, dW, dD, stream)) return rc;
+    if (n_chunks > 1 && ((ce = cudaEventRecord(m->host_ev[2 * c + 1], st)) != cudaSuccess ||
+                         (ce = cudaStreamWaitEvent(s_out, m->host_ev[2 * c + 1], 0)) != cudaSuccess))
+      return fail_cuda(ce, "host pipeline (kernel event)");
+    if ((ce = cudaMemcpy2DAsync(wdot + c0, pitch, dW, w, w, (size_t)S, cudaMemcpyDeviceToHost, s_out)) != cudaSuccess ||
+        (ce = cudaMemcpyAsync(dTdt + c0, dD, w, cudaMemcpyDeviceToHost, s_out)) != cudaSuccess)
+      return fail_cuda(ce, "device to host copy");
+  }
+  if (n_chunks > 1) {
+    // `stream` ends after the last copy-out, so that the caller's later work is ordered behind it
+    cudaEvent_t e1 = m->host_ev[2 * CK_HOST_CHUNKS + 1];
+    if ((ce = cudaEventRecord(e1, s_out)) != cudaSuccess || (ce = cudaStreamWaitEvent(st, e1, 0)) != cudaSuccess)
+      return fail_cuda(ce, "host pipeline end");
+  }
   if ((ce = cudaStreamSynchronize(st)) != cudaSuccess) return fail_cuda(ce, "cudaStreamSynchronize");
   return CK_OK;
 }

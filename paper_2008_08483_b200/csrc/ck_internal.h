@@ -11,6 +11,8 @@
 #include "../../include/ck.h"
 #include "ck_program.h"
 
+#define CK_HOST_CHUNKS 16   // most chunks ck_source_terms_host splits a batch into
+
 namespace ck {
 
 // Kernel argument of the mechanism-specialised kernel; must match CkParams in
@@ -90,6 +92,10 @@ struct ck_mech {
   // staging for ck_source_terms_host
   double *d_stage = nullptr;
   int64_t stage_cells = 0;
+  // ... and its copy/compute pipeline: copy-in and copy-out streams, per chunk one event after
+  // the copy-in and one after the kernel, plus a start and an end event
+  cudaStream_t host_in = nullptr, host_out = nullptr;
+  cudaEvent_t host_ev[2 * CK_HOST_CHUNKS + 2] = {};
   // ck_rk4_integrate: workspace (stage state, slopes, weighted slope sums) and the captured step
   double *d_rk4 = nullptr;
   int64_t rk4_cells = 0;
