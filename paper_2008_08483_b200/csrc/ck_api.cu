@@ -174,11 +174,12 @@ std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk,
   const int sreg_forced = std::min(S, env_int("CK_JIT_SREG", -1));   // tuning / test knob
   const size_t tab_bytes = (size_t)spec.tab_ranges * R * spec.row * sizeof(double);   // R includes padding
   const int nt_forced = env_int("CK_JIT_NT", 0), b_forced = env_int("CK_JIT_MINB", 0);
+  spec.lut_rep = std::max(1, env_int("CK_JIT_LUTREP", 1));
   int best_nt = 0, best_b = 0, best_cap = 0, best_sreg = 0;
   bool best_tab = false;
   size_t best_smem = 0;
   auto smem_of = [&](int nt, int s_reg, bool tab_smem) {
-    return (size_t)(S + (S - s_reg) + spec.ann_nhp) * (nt + 8) * 8 + (32 + 256) * 8 + (size_t)spec.n_ranges * S * 12 * 8 +
+    return (size_t)(S + (S - s_reg) + spec.ann_nhp) * (nt + 8) * 8 + (128 * spec.lut_rep + 256) * 8 + (size_t)spec.n_ranges * S * 12 * 8 +
            (tab_smem ? tab_bytes : (size_t)(nt / 32) * 2 * spec.tab_ranges * spec.block * spec.row * 8) + 16;
   };
   const bool all_regs = sreg_forced < 0 ? fits : (sreg_forced == S);
@@ -258,8 +259,11 @@ void finalize_jit(const ck_mech_desc *d, HostBuild *hb, const std::vector<double
   std::vector<int> order;                 // original reaction index, or -1 for a null reaction
   spec.block = kJitBlock;
   for (int g = 0; g < 6; ++g) {
-    for (int j = 0; j < R; ++j)
-      if (group_of(orig[j]) == g) order.push_back(j);
+    // within a falloff group the Troe reactions first: the kernel decides Troe / Lindemann per
+    // block from its first reaction
+    for (int pass = 0; pass < 2; ++pass)
+      for (int j = 0; j < R; ++j)
+        if (group_of(orig[j]) == g && (orig[j].type == 3) == (pass == 0)) order.push_back(j);
     while (order.size() % kJitBlock) order.push_back(-1);
     spec.group_end[g] = (int)order.size() / kJitBlock;
   }

@@ -52,6 +52,7 @@ struct JitSpec {
   bool kc_ann = false;         // approximate ANN for ln Kc in place of the exact layer
   int ann_nin = 0, ann_nl = 0, ann_nh = 0, ann_nhp = 0, ann_act = 0;
   std::vector<double> ann_const;   // mean | 1/std | W_in | B | W_hid
+  int lut_rep = 1;             // interleaved copies of the exp table (16: conflict-free lookups)
   bool kconst = false;         // polynomial coefficients as constant-bank operands (else literals)
   int group_end[6] = {0, 0, 0, 0, 0, 0};   // end block of (elementary, three-body, falloff) x (rev, irrev)
   std::vector<JitReaction> rxn;

@@ -117,7 +117,7 @@ std::string jit_generate_source(const JitSpec &s) {
     << "\n#define CK_G_TB0 " << s.group_end[1] << "\n#define CK_G_FO0 " << s.group_end[3]
     << "\n#define CK_TAB_NRANGES " << s.tab_ranges << "\n#define CK_ROW " << s.row
     << "\n#define CK_RK4 " << (s.rk4 ? 1 : 0) << "\n#define CK_KC_ANN " << (s.kc_ann ? 1 : 0) << "\n#define CK_KC_NONE " << (s.kc_none ? 1 : 0)
-    << "\n#define CK_SREG " << s.s_reg << "\n#define CK_PERM " << (s.perm.empty() ? 0 : 1) << "\n";
+    << "\n#define CK_LUT_REP " << s.lut_rep << "\n#define CK_SREG " << s.s_reg << "\n#define CK_PERM " << (s.perm.empty() ? 0 : 1) << "\n";
   if (!s.perm.empty()) {
     o << "__constant__ int ck_c_perm[" << s.perm.size() << "] = {";
     for (size_t i = 0; i < s.perm.size(); ++i) o << (i ? "," : "") << (i % 16 == 0 ? "\n  " : " ") << s.perm[i];
