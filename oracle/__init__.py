@@ -49,6 +49,8 @@ def _load():
         lib.ck_oracle_cell_detail.restype = None
         lib.ck_oracle_cell_detail.argtypes = ([C.POINTER(_Mech), C.c_double, C.c_double, _dp,
                                                C.c_int64] + [_dp] * 16)
+        lib.ck_oracle_jacobian.restype = C.c_int
+        lib.ck_oracle_jacobian.argtypes = [C.POINTER(_Mech), _dp, _dp, _dp, C.c_int64, _dp, C.c_int]
         _lib = lib
     return _lib
 
@@ -133,3 +135,18 @@ def cell_detail(omech: OracleMechanism, T: float, P: float, Y):
     out.update(per_s)
     out.update(per_r)
     return out
+
+
+def jacobian(omech: OracleMechanism, T, P, Y, nthreads: int = 0):
+    """J[N, S+1, S+1] = d(wdot_0..wdot_{S-1}, dT/dt) / d(Y_0..Y_{S-1}, T) at constant P
+    (ck_oracle_jac.c), for T[N], P[N], Y[S,N]."""
+    T, P, Y = _f64(T), _f64(P), _f64(Y)
+    N = T.shape[0]
+    assert P.shape == (N,) and Y.shape == (omech.S, N)
+    J = np.empty((N, omech.S + 1, omech.S + 1))
+    used = _load().ck_oracle_jacobian(
+        C.byref(omech.c), T.ctypes.data_as(_dp), P.ctypes.data_as(_dp), Y.ctypes.data_as(_dp),
+        N, J.ctypes.data_as(_dp), int(nthreads))
+    if used < 0:
+        raise ValueError("the oracle Jacobian does not support the approximate-ANN Kc")
+    return J

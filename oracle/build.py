@@ -9,16 +9,17 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "ck_oracle.c")
+SRC_JAC = os.path.join(HERE, "ck_oracle_jac.c")
 HDR = os.path.join(HERE, "ck_oracle.h")
 LIB = os.path.join(HERE, "libck_oracle.so")
 
 
 def build(force: bool = False) -> str:
-    newest = max(os.path.getmtime(SRC), os.path.getmtime(HDR))
+    newest = max(os.path.getmtime(SRC), os.path.getmtime(SRC_JAC), os.path.getmtime(HDR))
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
         return LIB
     cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra",
-           "-o", LIB + ".tmp", SRC, "-lm"]
+           "-o", LIB + ".tmp", SRC, SRC_JAC, "-lm"]
     subprocess.run(cmd, check=True, cwd=HERE)
     os.replace(LIB + ".tmp", LIB)
     return LIB

@@ -84,6 +84,13 @@ void ck_oracle_cell_detail(const ck_oracle_mech *m, double T, double P, const do
                            double *kf, double *Kc, double *kr, double *M, double *qf,
                            double *qr, double *Q, double *wdot, double *dTdt);
 
+/* Analytic Jacobian of (wdot, dT/dt) with respect to (Y, T) at constant P (ck_oracle_jac.c,
+ * which states the formulas, the reading and the pins): J[N][S+1][S+1], cell-major; row i < S
+ * is wdot_i, row S is dT/dt; column l < S is Y_l, column S is T.  Returns the number of
+ * threads used, or -1 if the mechanism carries the approximate-ANN Kc (not supported). */
+int ck_oracle_jacobian(const ck_oracle_mech *m, const double *T, const double *P, const double *Y,
+                       int64_t N, double *J, int nthreads);
+
 #ifdef __cplusplus
 }
 #endif
