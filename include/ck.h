@@ -165,6 +165,27 @@ int ck_source_terms_host(ck_mech *m, const double *T, const double *P, const dou
 int ck_rk4_integrate(ck_mech *m, double *T, const double *P, double *Y, int64_t N, double dt,
                      int64_t n_steps, int use_graph, void *stream);
 
+/* Analytic Jacobian of the source term (the prerequisite of
+ * the GPU stiff integrator PAPER.md:277 names): for each of N cells the (S+1) x (S+1) matrix
+ *   J = d(wdot_0 .. wdot_{S-1}, dT/dt) / d(Y_0 .. Y_{S-1}, T)      at constant P,
+ * the Y_l taken as S independent variables (the source term is defined for any Y > 0 and is
+ * homogeneous of degree 0 in Y, so sum_l Y_l J_il = 0).  It is the chain rule applied to the
+ * paper's layers: Eq. 4 dq/dC_l = nu_lj q/C_l; Eq. 6
+ * d ln k_f/dT = (b + (Ea/R)/T)/T; Eq. 11 d ln Kc/dT = (dnu^T h/RT - sum dnu)/T;
+ * third bodies and falloff through M and Pr; Eq. 2; then
+ * C_k = rho Y_k / W_k with rho = P/(Ru T sum_j Y_j/W_j) and the quotient rule on
+ * dT/dt = -sum_k h_k wdot_k/(rho cp).  The floor on C, the clamp on Pr and the NASA-7 range
+ * switch are not differentiated (reading Q18): T, P and every Y_k must be > 0.
+ * T, P, Y: DEVICE pointers laid out as for ck_source_terms.  J: DEVICE, [N][S+1][S+1]
+ * doubles, cell-major and row-major per cell (a strided batch of matrices, lda = S+1); row
+ * i < S is wdot_i, row S is dT/dt; column l < S is Y_l, column S is T; every entry is written.
+ * Asynchronous on `stream`, allocates nothing, deterministic run to run (no atomics).
+ * N == 0 is a successful no-op.  Errors: CK_EINVAL (NULL handle or pointer with N > 0, N < 0,
+ * misaligned pointer), CK_EUNSUPPORTED (mechanism with the approximate-ANN Kc, S > 127, or
+ * a tile that does not fit shared memory), CK_ECUDA. */
+int ck_jacobian(const ck_mech *m, const double *T, const double *P, const double *Y, int64_t N,
+                double *J, void *stream);
+
 /* Free the handle and its device memory.  NULL is a no-op. */
 void ck_mech_destroy(ck_mech *m);
 
@@ -178,7 +199,8 @@ const char *ck_last_error(void);
  *       ck_source_terms call, 13 nnz(E) counted over third-body and falloff columns,
  *       14 kernel variant in use (0 generic table-driven kernel, 1 mechanism-specialised),
  *       15 species whose accumulators the specialised kernel keeps in registers (the other
- *       S - that many accumulate in shared memory; 0 for the generic kernel).
+ *       S - that many accumulate in shared memory; 0 for the generic kernel),
+ *       16 cells per tile of the Jacobian kernel (0 if ck_jacobian is unsupported here).
  * Returns -1 for a NULL handle or unknown `what`. */
 int64_t ck_mech_info(const ck_mech *m, int what);
 

@@ -21,7 +21,7 @@ import numpy as np
 from . import _build
 
 __all__ = ["Mechanism", "CkError", "ck_mech_create", "ck_source_terms", "ck_source_terms_host",
-           "ck_rk4_integrate",
+           "ck_rk4_integrate", "ck_jacobian",
            "ck_mech_destroy", "ck_last_error", "ck_mech_info", "ck_measure_fp64_peak",
            "ck_mech_jit_source",
            "library_path", "RU", "INFO"]
@@ -29,7 +29,7 @@ __all__ = ["Mechanism", "CkError", "ck_mech_create", "ck_source_terms", "ck_sour
 RU = 8314.46261815324  # J/(kmol K), the constant compiled into the kernels
 INFO = {"S": 0, "R": 1, "nnz_reac": 2, "nnz_prod": 3, "nnz_net": 4, "n_three_body": 5,
         "n_lindemann": 6, "n_troe": 7, "n_ranges": 8, "threads": 9, "blocks_per_sm": 10,
-        "smem_bytes": 11, "launches_per_call": 12, "nnz_eff": 13, "jit": 14, "s_reg": 15}
+        "smem_bytes": 11, "launches_per_call": 12, "nnz_eff": 13, "jit": 14, "s_reg": 15, "jac_cells": 16}
 
 _dp = C.POINTER(C.c_double)
 _bp = C.POINTER(C.c_uint8)
@@ -82,6 +82,8 @@ def _load():
     lib.ck_last_error.argtypes = []
     lib.ck_mech_info.restype = C.c_int64
     lib.ck_mech_info.argtypes = [C.c_void_p, C.c_int]
+    lib.ck_jacobian.restype = C.c_int
+    lib.ck_jacobian.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
     lib.ck_mech_jit_source.restype = C.c_int64
     lib.ck_mech_jit_source.argtypes = [C.POINTER(_Desc), C.c_char_p, C.c_int64]
     lib.ck_measure_fp64_peak.restype = C.c_int
@@ -130,6 +132,10 @@ def ck_source_terms(handle, T, P, Y, N, wdot, dTdt, stream=0) -> None:
 def ck_source_terms_host(handle, T, P, Y, N, wdot, dTdt, stream=0) -> None:
     _check(_lib.ck_source_terms_host(handle, _addr(T), _addr(P), _addr(Y), int(N), _addr(wdot),
                                      _addr(dTdt), stream or None))
+
+
+def ck_jacobian(handle, T, P, Y, N, J, stream=0) -> None:
+    _check(_lib.ck_jacobian(handle, _addr(T), _addr(P), _addr(Y), int(N), _addr(J), stream or None))
 
 
 def ck_rk4_integrate(handle, T, P, Y, N, dt, n_steps, use_graph=True, stream=0) -> None:
@@ -232,6 +238,12 @@ class Mechanism:
         if N is None:
             N = T.shape[0]
         ck_source_terms(self.handle, T, P, Y, N, wdot, dTdt, stream)
+
+    def jacobian(self, T, P, Y, J, N=None, stream=0) -> None:
+        """J[N, S+1, S+1] = d(wdot, dT/dt)/d(Y, T) at constant P; device buffers; asynchronous."""
+        if N is None:
+            N = T.shape[0]
+        ck_jacobian(self.handle, T, P, Y, N, J, stream)
 
     def source_terms_host(self, T, P, Y, wdot=None, dTdt=None, stream=0):
         """Host buffers (numpy or pinned torch CPU tensors); synchronous. Returns (wdot, dTdt)."""

@@ -701,6 +701,11 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   m->jit_params.logtab = (const double *)(base + o_jlog);
   if (int st = setup_jit(m, spec, hb.jit_why, hb.jit_smem)) { ck_mech_destroy(m); return st; }
   m->jit_s_reg = spec.s_reg;
+  // ---- tables of the Jacobian kernel (ck_jac.cu) ------------------------------------------
+  {
+    const std::string err = ck::jac_create(d, m->num_sms, (size_t)prop.sharedMemPerBlockOptin, &m->jac);
+    if (!err.empty()) { ck_mech_destroy(m); return fail(CK_ECUDA, err); }
+  }
   *out = m;
   return CK_OK;
 }
@@ -709,6 +714,7 @@ extern "C" void ck_mech_destroy(ck_mech *m) {
   if (!m) return;
   if (m->d_tables) cudaFree(m->d_tables);
   if (m->d_scratch) cudaFree(m->d_scratch);
+  ck::jac_destroy(m->jac);
   if (m->d_stage) cudaFree(m->d_stage);
   if (m->host_in) cudaStreamDestroy(m->host_in);
   if (m->host_out) cudaStreamDestroy(m->host_out);
@@ -750,6 +756,22 @@ extern "C" int ck_source_terms(const ck_mech *m, const double *T, const double *
     ce = ck::launch_source_terms(m, T, P, Y, N, wdot, dTdt, (cudaStream_t)stream);
   }
   if (ce != cudaSuccess) return fail_cuda(ce, "ck_source_terms launch");
+  return CK_OK;
+}
+
+extern "C" int ck_jacobian(const ck_mech *m, const double *T, const double *P, const double *Y,
+                           int64_t N, double *J, void *stream) {
+  if (!m) return fail(CK_EINVAL, "mechanism handle is NULL");
+  if (N < 0) return fail(CK_EINVAL, "N must be >= 0");
+  if (N == 0) return CK_OK;
+  if (!T || !P || !Y || !J) return fail(CK_EINVAL, "a state or result pointer is NULL");
+  if (((uintptr_t)T | (uintptr_t)P | (uintptr_t)Y | (uintptr_t)J) & 7u)
+    return fail(CK_EINVAL, "pointers must be 8-byte aligned");
+  if (!m->jac)
+    return fail(CK_EUNSUPPORTED, "ck_jacobian: not available for this mechanism (approximate-ANN Kc, S > 127, "
+                                 "or the tile does not fit shared memory)");
+  const cudaError_t ce = ck::jac_launch(m->jac, T, P, Y, N, J, (cudaStream_t)stream);
+  if (ce != cudaSuccess) return fail_cuda(ce, "ck_jacobian launch");
   return CK_OK;
 }
 
@@ -964,6 +986,7 @@ extern "C" int64_t ck_mech_info(const ck_mech *m, int what) {
     case 13: return m->nnz_eff;
     case 14: return m->jit_kernel ? 1 : 0;
     case 15: return m->jit_kernel ? m->jit_s_reg : 0;
+    case 16: return m->jac ? ck::jac_cells_per_tile(m->jac) : 0;
     default: return -1;
   }
 }

@@ -59,6 +59,14 @@ struct JitSpec {
   std::vector<double> inv_W, range_T, falloff;   // constant-bank tables
 };
 
+struct JacMech;   // device tables of the Jacobian kernel (ck_jac.cu)
+// Builds them; returns "" (with *out NULL if the mechanism is unsupported there) or an error text.
+std::string jac_create(const ck_mech_desc *d, int num_sms, size_t smem_block_max, JacMech **out);
+void jac_destroy(JacMech *jm);
+int jac_cells_per_tile(const JacMech *jm);
+cudaError_t jac_launch(const JacMech *jm, const double *T, const double *P, const double *Y, int64_t N,
+                       double *J, cudaStream_t stream);
+
 std::string jit_generate_source(const JitSpec &spec);
 // Compiles to a cubin for sm_100a with NVRTC; returns "" on success, else the error text.
 std::string jit_compile(const std::string &src, std::vector<char> *cubin);
@@ -90,6 +98,8 @@ struct ck_mech {
   cudaKernel_t rk4_kernel = nullptr;
   bool rk4_tried = false;
   std::string jit_note;       // why the specialised kernel is not in use, if so
+  // analytic Jacobian (ck_jacobian): NULL if unsupported for this mechanism
+  ck::JacMech *jac = nullptr;
   // staging for ck_source_terms_host
   double *d_stage = nullptr;
   int64_t stage_cells = 0;

@@ -1,0 +1,534 @@
+// ck_jac.cu -- analytic Jacobian of the source term, d(wdot, dT/dt)/d(Y, T) at constant P
+// (the prerequisite of the GPU stiff integrator the paper
+// names as future work).  Host table builder + one fused kernel for sm_100a.
+//
+// The paper prints no Jacobian; this is the chain rule applied to its layers (DESIGN.md
+// section 14 derives every term):
+//   Eq. 4  ln q_f = nu'^T ln C + ln k_f, ln q_r = nu''^T ln C + ln k_r
+//          =>  dq_f/dC_l = nu'_lj q_f / C_l,  dq_r/dC_l = nu''_lj q_r / C_l
+//   Eq. 6  d ln k_f/dT = (b + (Ea/R)/T)/T
+//   Eq. 11 d ln Kc/dT = (dnu^T (h/RT) - sum dnu)/T    (Gibbs-Helmholtz on Eq. 10)
+//   PAPER.md:157          three-body: dQ/dC_l += E_lj (q_f - q_r); falloff through Pr = k_0 M/k_inf
+//   Eq. 2  d wdot_i = sum_j dnu_ij dQ_j
+// followed by the change of variables C -> (Y, T) at constant P and the energy row.
+//
+// Output layout: J[N][S+1][S+1], cell-major and row-major per cell (what a batched linear
+// solver takes as a strided batch); row i < S is wdot_i, row S is dT/dt; column l < S is
+// Y_l, column S is T.  23 KB per cell at S=53: the kernel is bound by these HBM writes
+// (DESIGN.md section 14), so the mapping is chosen for coalesced row stores:
+//
+//   block = 8 warps, tile of CELLS cells (8, or 4 for big mechanisms), persistent grid.
+//   phase A  thread per (species, cell): C, 1/C, ln C, NASA-7 h/RT, cp/R, d(cp/R)/dT, g'.
+//   phase M  thread per (third-body or falloff reaction, cell): M = sum_k E_kj C_k.
+//   phase B  thread per (reaction, cell): the rate layers in log form and the five scalars
+//            every derivative of Q_j is made of:
+//              a = phi q_f, b = phi q_r        dQ/dC_l|sparse = (nu'_lj a - nu''_lj b)/C_l
+//              m                               dQ/dC_l|dense  = m E_lj
+//              t = dQ/dT at constant C,  Q,    e = sum_l C_l dQ/dC_l = ord' a - ord'' b + m M
+//   phase C  warp per row i (species), lanes = columns l, the tile's cells in registers:
+//            the row of d wdot_i/dC is gathered (never scattered: no atomics, fixed order)
+//            from three host-built lists -- the reactions of row i (diagonal, T column, wdot_i
+//            and g_i = sum_l C_l dwdot_i/dC_l, lanes = (cell, quarter of the list)), the
+//            off-diagonal sparse entries grouped by column, and the third-body reactions of
+//            the row (dense in l: coefficient x row of E) -- then mapped to (Y, T):
+//              dwdot_i/dY_l = rho/W_l dwdot_i/dC_l - g_i/(s W_l),  dwdot_i/dT = t-sum - g_i/T
+//            stored as one coalesced row per cell, and accumulated into the energy row.
+//   phase E  energy row: cross-warp sum of H_i x row i, then the quotient rule.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "ck_internal.h"
+
+namespace ck {
+
+constexpr int kJacWarps = 8;
+constexpr int kJacThreads = kJacWarps * 32;
+
+struct JacRowEnt {   // reaction j of row i: coefficients of a_j, b_j on the diagonal, dnu_ij
+  double dnu, cf, cr;   // dnu_ij, dnu_ij nu'_ij, dnu_ij nu''_ij
+  int j, tb;            // reaction, its row of E / M (or -1)
+};
+struct JacOffEnt {   // off-diagonal sparse entry (i, l): coefficients of a_j and b_j
+  double cf, cr;        // dnu_ij nu'_lj, dnu_ij nu''_lj
+  int j, pad;
+};
+struct JacRxn {      // per reaction, phase B
+  double lnA, b, EaR, lnA0, b0, Ea0R, troe[4];
+  double dn, ordf, ordr;   // sum dnu, sum nu', sum nu''
+  int type, rev, tb, s0, s1, pad;   // support list [s0, s1) of (species, nu', nu'')
+};
+struct JacSup { double nuf, nur; int k, pad; };
+
+struct JacTables {
+  int S, R, n_tb, SP;          // SP = padded row length of E (multiple of 32)
+  const double *invW, *nasa_lo, *nasa_hi, *T_mid;   // [S], [S][7], [S][7], [S]
+  const JacRxn *rxn;           // [R]
+  const JacSup *sup;           // support lists
+  const int *tb_rxn;           // [n_tb] reaction of each row of E
+  const double *E;             // [n_tb][SP] efficiencies, zero padded
+  const int *row_start;        // [S+1] into row_ent
+  const JacRowEnt *row_ent;
+  const int *off_start;        // [S][SP+1] into off_ent, segments by column
+  const JacOffEnt *off_ent;
+  double ln_pref_Ru;           // ln(p_ref / Ru)
+};
+
+struct JacMech {
+  JacTables t{};
+  void *d_blob = nullptr;
+  int cells = 8;               // cells per tile
+  size_t smem = 0;
+  int grid_max = 1;
+};
+
+}  // namespace ck
+
+namespace ck {
+namespace {
+
+constexpr double kLn10 = 2.302585092994045684;
+enum { SP_C = 0, SP_INVC, SP_LNC, SP_HRT, SP_CPR, SP_DCPR, SP_GP, SP_COUNT };
+enum { CS_T = 0, CS_RHO, CS_S, CS_INVT, CS_LNT, CS_D, CS_DDT, CS_COUNT = 8 };
+
+// doubles of dynamic shared memory
+inline size_t jac_smem_doubles(int S, int R, int n_tb, int cells, int cpl) {
+  const size_t rx = (size_t)6 * R * cells, red = (size_t)kJacWarps * cells * (32 * cpl + 2);
+  return (size_t)SP_COUNT * S * cells + (size_t)CS_COUNT * cells + (size_t)(n_tb > 0 ? n_tb : 1) * cells +
+         std::max(rx, red);
+}
+
+template <int CELLS, int CPL>
+__global__ void __launch_bounds__(kJacThreads, 1)
+jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *__restrict__ Pg,
+                const double *__restrict__ Yg, long long N, double *__restrict__ Jg) {
+  extern __shared__ __align__(16) double smem[];
+  const int S = t.S, R = t.R, n = S + 1, SP = t.SP;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  double *sp = smem;                                   // [SP_COUNT][S][CELLS]
+  double *cs = sp + (size_t)SP_COUNT * S * CELLS;      // [CELLS][CS_COUNT]
+  double *Mtb = cs + CS_COUNT * CELLS;                 // [n_tb][CELLS]
+  double *rx = Mtb + (size_t)(t.n_tb > 0 ? t.n_tb : 1) * CELLS;
+  double2 *AB = (double2 *)rx;                         // [R][CELLS]  (a, b)
+  double *Mm = rx + (size_t)2 * R * CELLS;             // [R][CELLS]  m
+  double *Tt = Mm + (size_t)R * CELLS;                 // t
+  double *Qq = Tt + (size_t)R * CELLS;                 // Q
+  double *Ee = Qq + (size_t)R * CELLS;                 // e
+  double *red = rx;                                    // phase E, aliases the reaction arrays
+  double *red2 = red + (size_t)kJacWarps * CELLS * 32 * CPL;
+#define SPV(a, k, c) sp[((size_t)(a) * S + (k)) * CELLS + (c)]
+  constexpr int PARTS = 32 / CELLS;
+
+  const long long n_tiles = (N + CELLS - 1) / CELLS;
+  for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    const long long cell0 = tile * CELLS;
+    // ---- cell scalars: s = sum_k Y_k/W_k, rho; warp c <-> cell c -----------
+    for (int c = warp; c < CELLS; c += kJacWarps) {
+      const long long cell = cell0 + c < N ? cell0 + c : N - 1;
+      double s = 0.0;
+      for (int k = lane; k < S; k += 32) s += Yg[(size_t)k * N + cell] * t.invW[k];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+      if (lane == 0) {
+        const double T = Tg[cell], P = Pg[cell];
+        cs[c * CS_COUNT + CS_T] = T;
+        cs[c * CS_COUNT + CS_S] = s;
+        cs[c * CS_COUNT + CS_RHO] = P / (kRu * T * s);
+        cs[c * CS_COUNT + CS_INVT] = 1.0 / T;
+        cs[c * CS_COUNT + CS_LNT] = log(T);
+      }
+    }
+    __syncthreads();
+    // ---- phase A: species layers, thread per (species, cell) -------------------------------
+    for (int idx = tid; idx < S * CELLS; idx += kJacThreads) {
+      const int k = idx / CELLS, c = idx - k * CELLS;
+      const long long cell = cell0 + c < N ? cell0 + c : N - 1;
+      const double T = cs[c * CS_COUNT + CS_T], lnT = cs[c * CS_COUNT + CS_LNT], invT = cs[c * CS_COUNT + CS_INVT];
+      const double C = fmax(cs[c * CS_COUNT + CS_RHO] * Yg[(size_t)k * N + cell] * t.invW[k], kCFloor);
+      SPV(SP_C, k, c) = C;
+      SPV(SP_INVC, k, c) = 1.0 / C;
+      SPV(SP_LNC, k, c) = log(C);
+      const double *a = (T <= t.T_mid[k] ? t.nasa_lo : t.nasa_hi) + 7 * k;
+      const double T2 = T * T, T3 = T2 * T, T4 = T3 * T;
+      const double cpR = a[0] + a[1] * T + a[2] * T2 + a[3] * T3 + a[4] * T4;
+      const double hRT = a[0] + a[1] * T * 0.5 + a[2] * T2 * (1.0 / 3.0) + a[3] * T3 * 0.25 + a[4] * T4 * 0.2 + a[5] * invT;
+      const double sR = a[0] * lnT + a[1] * T + a[2] * T2 * 0.5 + a[3] * T3 * (1.0 / 3.0) + a[4] * T4 * 0.25 + a[6];
+      SPV(SP_CPR, k, c) = cpR;
+      SPV(SP_DCPR, k, c) = a[1] + 2.0 * a[2] * T + 3.0 * a[3] * T2 + 4.0 * a[4] * T3;
+      SPV(SP_HRT, k, c) = hRT;
+      // g' = g/RT - ln(p_ref/(Ru T)): ln Kc = -dnu^T g' (Eq. 11 with PAPER.md:114's fold)
+      SPV(SP_GP, k, c) = hRT - sR - (t.ln_pref_Ru - lnT);
+    }
+    __syncthreads();
+    // D = rho cp = sum_k C_k Cp_k and dD/dT at constant C (+ the -D/T of dC/dT later)
+    for (int c = warp; c < CELLS; c += kJacWarps) {
+      double D = 0.0, dD = 0.0;
+      for (int k = lane; k < S; k += 32) {
+        D += SPV(SP_C, k, c) * SPV(SP_CPR, k, c);
+        dD += SPV(SP_C, k, c) * SPV(SP_DCPR, k, c);
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        D += __shfl_xor_sync(0xffffffffu, D, o);
+        dD += __shfl_xor_sync(0xffffffffu, dD, o);
+      }
+      if (lane == 0) {
+        cs[c * CS_COUNT + CS_D] = D * kRu;
+        cs[c * CS_COUNT + CS_DDT] = dD * kRu - D * kRu * cs[c * CS_COUNT + CS_INVT];
+      }
+    }
+    // ---- phase M: third-body layer M = C E, thread per (row of E, cell) -----
+    for (int idx = tid; idx < t.n_tb * CELLS; idx += kJacThreads) {
+      const int r = idx / CELLS, c = idx - r * CELLS;
+      const double *e = t.E + (size_t)r * SP;
+      double m0 = 0.0, m1 = 0.0;
+      int k = 0;
+      for (; k + 1 < S; k += 2) {
+        m0 = fma(__ldg(e + k), SPV(SP_C, k, c), m0);
+        m1 = fma(__ldg(e + k + 1), SPV(SP_C, k + 1, c), m1);
+      }
+      if (k < S) m0 = fma(__ldg(e + k), SPV(SP_C, k, c), m0);
+      Mtb[r * CELLS + c] = m0 + m1;
+    }
+    __syncthreads();
+    // ---- phase B: rate layers and the derivative scalars, thread per (reaction, cell) ------
+    for (int idx = tid; idx < R * CELLS; idx += kJacThreads) {
+      const int j = idx / CELLS, c = idx - j * CELLS;
+      const JacRxn &r = t.rxn[j];
+      const double lnT = cs[c * CS_COUNT + CS_LNT], invT = cs[c * CS_COUNT + CS_INVT], T = cs[c * CS_COUNT + CS_T];
+      // Arrhenius layer (Eq. 6) and its T-derivative
+      double lnkf = r.lnA + r.b * lnT - r.EaR * invT;
+      double dlnkf = (r.b + r.EaR * invT) * invT;
+      // log-rate layers (Eq. 4) and the equilibrium layer (Eq. 11) over the reaction's species
+      double sf = 0.0, sr = 0.0, dG = 0.0, dH = 0.0;
+      for (int e = r.s0; e < r.s1; ++e) {
+        const JacSup u = t.sup[e];
+        const double lc = SPV(SP_LNC, u.k, c), dnu = u.nur - u.nuf;
+        sf = fma(u.nuf, lc, sf);
+        sr = fma(u.nur, lc, sr);
+        dG = fma(dnu, SPV(SP_GP, u.k, c), dG);
+        dH = fma(dnu, SPV(SP_HRT, u.k, c), dH);
+      }
+      const double dlnKc = (dH - r.dn) * invT;
+      double M = 1.0, phi = 1.0, gam = 1.0, dlnG = 0.0;
+      if (r.type != 0) M = Mtb[r.tb * CELLS + c];
+      if (r.type == 1) phi = M;
+      if (r.type >= 2) {
+        // falloff (textbook forms): k = k_inf Pr/(1+Pr) F, Pr = k_0 M/k_inf
+        const double lnk0 = r.lnA0 + r.b0 * lnT - r.Ea0R * invT;
+        const double dlnk0 = (r.b0 + r.Ea0R * invT) * invT;
+        const double Pr = exp(lnk0 - lnkf) * M;
+        double F = 1.0, dlnF_dlnPr = 0.0, dlnF_dT = 0.0;
+        if (r.type == 3) {
+          const double alpha = r.troe[0], T3 = r.troe[1], T1 = r.troe[2], T2 = r.troe[3];
+          const double e3 = exp(-T / T3), e1 = exp(-T / T1), e2 = exp(-T2 * invT);
+          const double Fc = (1.0 - alpha) * e3 + alpha * e1 + e2;
+          const double dFc = -(1.0 - alpha) / T3 * e3 - alpha / T1 * e1 + (isinf(T2) ? 0.0 : T2 * invT * invT * e2);
+          const double lFc = log10(Fc), dlFc = dFc / (Fc * kLn10);
+          const double cc = -0.4 - 0.67 * lFc, nn = 0.75 - 1.27 * lFc;
+          const double A = log10(Pr) + cc, B = nn - 0.14 * A;
+          const double f1 = A / B, den = 1.0 + f1 * f1;
+          F = exp(kLn10 * lFc / den);
+          const double dlF_df1 = -2.0 * lFc * f1 / (den * den);
+          dlnF_dlnPr = dlF_df1 * nn / (B * B);
+          dlnF_dT = kLn10 * dlFc * (1.0 / den + dlF_df1 * ((-0.67 * B + A * (1.27 - 0.14 * 0.67)) / (B * B)));
+        }
+        dlnG = 1.0 / (1.0 + Pr) + dlnF_dlnPr;
+        dlnkf = dlnkf + dlnG * (dlnk0 - dlnkf) + dlnF_dT;
+        gam = Pr / (1.0 + Pr) * F;
+      }
+      const double qf = exp(lnkf + sf) * gam;
+      const double qr = r.rev ? exp(lnkf + dG + sr) * gam : 0.0;   // ln k_r = ln k_f - ln Kc, ln Kc = -dG
+      const double a = phi * qf, b = phi * qr;
+      double m = 0.0;
+      if (r.type == 1) m = qf - qr;
+      if (r.type >= 2) m = (qf - qr) * dlnG / M;
+      AB[idx] = make_double2(a, b);
+      Mm[idx] = m;
+      Tt[idx] = a * dlnkf - b * (dlnkf - dlnKc);
+      Qq[idx] = a - b;
+      Ee[idx] = r.ordf * a - r.ordr * b + (r.type != 0 ? m * M : 0.0);
+    }
+    __syncthreads();
+    // ---- phase C: one warp per row i; lanes = columns, the tile's cells in registers -------
+    double eacc[CELLS][CPL];       // energy row: sum_i H_i dwdot_i/dx, this warp's rows
+#pragma unroll
+    for (int c = 0; c < CELLS; ++c)
+#pragma unroll
+      for (int p = 0; p < CPL; ++p) eacc[c][p] = 0.0;
+    double hw_acc = 0.0, cpw_acc = 0.0;   // lane c < CELLS: sum_i H_i wdot_i, sum_i Cp_i wdot_i
+    const int my_c = lane % CELLS, my_part = lane / CELLS;
+    for (int i = warp; i < S; i += kJacWarps) {
+      const int r0 = t.row_start[i], r1 = t.row_start[i + 1];
+      // (1) the row's reaction list, lanes = (cell, part): diagonal of the sparse part, T column,
+      //     wdot_i, g_i = sum_l C_l dwdot_i/dC_l (Euler's relation reaction by reaction)
+      double diag = 0.0, tsum = 0.0, wd = 0.0, g = 0.0;
+      for (int e = r0 + my_part; e < r1; e += PARTS) {
+        const JacRowEnt u = t.row_ent[e];
+        const int at = u.j * CELLS + my_c;
+        const double2 ab = AB[at];
+        diag = fma(u.cf, ab.x, fma(-u.cr, ab.y, diag));
+        tsum = fma(u.dnu, Tt[at], tsum);
+        wd = fma(u.dnu, Qq[at], wd);
+        g = fma(u.dnu, Ee[at], g);
+      }
+#pragma unroll
+      for (int o = CELLS; o < 32; o <<= 1) {
+        diag += __shfl_xor_sync(0xffffffffu, diag, o);
+        tsum += __shfl_xor_sync(0xffffffffu, tsum, o);
+        wd += __shfl_xor_sync(0xffffffffu, wd, o);
+        g += __shfl_xor_sync(0xffffffffu, g, o);
+      }
+      const double Hi_mine = SPV(SP_HRT, i, my_c) * kRu * cs[my_c * CS_COUNT + CS_T];
+      hw_acc = fma(Hi_mine, wd, hw_acc);
+      cpw_acc = fma(SPV(SP_CPR, i, my_c) * kRu, wd, cpw_acc);
+
+      double accS[CELLS][CPL], accD[CELLS][CPL];
+#pragma unroll
+      for (int c = 0; c < CELLS; ++c)
+#pragma unroll
+        for (int p = 0; p < CPL; ++p) accS[c][p] = accD[c][p] = 0.0;
+      // (2) off-diagonal sparse entries of row i, grouped by column
+#pragma unroll
+      for (int p = 0; p < CPL; ++p) {
+        const int col = lane + 32 * p;
+        const int *seg = t.off_start + (size_t)i * (SP + 1) + col;
+        const int e0 = col < SP ? seg[0] : 0, e1 = col < SP ? seg[1] : 0;
+        for (int e = e0; e < e1; ++e) {
+          const JacOffEnt u = t.off_ent[e];
+          const double2 *ab = AB + (size_t)u.j * CELLS;
+#pragma unroll
+          for (int c = 0; c < CELLS; ++c) {
+            const double2 v = ab[c];
+            accS[c][p] = fma(u.cf, v.x, fma(-u.cr, v.y, accS[c][p]));
+          }
+        }
+      }
+      // (3) third-body / falloff reactions of the row (listed first): coefficient x row of E
+      for (int e = r0; e < r1; ++e) {
+        const int tb = t.row_ent[e].tb;
+        if (tb < 0) break;
+        const double dnu = t.row_ent[e].dnu;
+        const double *mm = Mm + (size_t)t.row_ent[e].j * CELLS;
+        double ev[CPL];
+#pragma unroll
+        for (int p = 0; p < CPL; ++p) ev[p] = (lane + 32 * p < SP) ? __ldg(t.E + (size_t)tb * SP + lane + 32 * p) : 0.0;
+#pragma unroll
+        for (int c = 0; c < CELLS; ++c) {
+          const double co = dnu * mm[c];
+#pragma unroll
+          for (int p = 0; p < CPL; ++p) accD[c][p] = fma(co, ev[p], accD[c][p]);
+        }
+      }
+      // (4) C -> (Y, T) at constant P, store the row, accumulate the energy row
+#pragma unroll
+      for (int c = 0; c < CELLS; ++c) {
+        const double diag_c = __shfl_sync(0xffffffffu, diag, c);
+        const double tsum_c = __shfl_sync(0xffffffffu, tsum, c);
+        const double g_c = __shfl_sync(0xffffffffu, g, c);
+        const double rho = cs[c * CS_COUNT + CS_RHO], inv_s = 1.0 / cs[c * CS_COUNT + CS_S];
+        const double Hi = SPV(SP_HRT, i, c) * kRu * cs[c * CS_COUNT + CS_T];
+        const long long cell = cell0 + c;
+#pragma unroll
+        for (int p = 0; p < CPL; ++p) {
+          const int col = lane + 32 * p;
+          double v = 0.0;
+          if (col < S) {
+            double jc = fma(accS[c][p] + (col == i ? diag_c : 0.0), SPV(SP_INVC, col, c), accD[c][p]);
+            const double iw = t.invW[col];
+            v = jc * (rho * iw) - g_c * (iw * inv_s);
+          } else if (col == S) {
+            v = tsum_c - g_c * cs[c * CS_COUNT + CS_INVT];
+          }
+          if (col <= S && cell < N) __stcs(Jg + ((size_t)cell * n + i) * n + col, v);
+          eacc[c][p] = fma(Hi, v, eacc[c][p]);
+        }
+      }
+    }
+    __syncthreads();   // the reaction arrays are dead: their memory becomes the reduction buffer
+    // ---- phase E: energy row dT/dt = -sum_k H_k wdot_k / D ---------------------------------
+#pragma unroll
+    for (int c = 0; c < CELLS; ++c)
+#pragma unroll
+      for (int p = 0; p < CPL; ++p) red[((size_t)warp * CELLS + c) * (32 * CPL) + lane + 32 * p] = eacc[c][p];
+    if (lane < CELLS) {
+      red2[(warp * CELLS + lane) * 2] = hw_acc;
+      red2[(warp * CELLS + lane) * 2 + 1] = cpw_acc;
+    }
+    __syncthreads();
+    for (int idx = tid; idx < CELLS * n; idx += kJacThreads) {
+      const int c = idx / n, col = idx - c * n;
+      double hj = 0.0, hw = 0.0, cpw = 0.0;
+#pragma unroll
+      for (int w = 0; w < kJacWarps; ++w) {
+        hj += red[((size_t)w * CELLS + c) * (32 * CPL) + col];
+        hw += red2[(w * CELLS + c) * 2];
+        cpw += red2[(w * CELLS + c) * 2 + 1];
+      }
+      const double D = cs[c * CS_COUNT + CS_D], invD = 1.0 / D, Tdot = -hw * invD;
+      double v;
+      if (col < S) {
+        const double iw = t.invW[col];
+        const double dD = cs[c * CS_COUNT + CS_RHO] * SPV(SP_CPR, col, c) * kRu * iw - D * iw / cs[c * CS_COUNT + CS_S];
+        v = -hj * invD - Tdot * dD * invD;
+      } else {
+        v = -(cpw + hj) * invD - Tdot * cs[c * CS_COUNT + CS_DDT] * invD;
+      }
+      const long long cell = cell0 + c;
+      if (cell < N) __stcs(Jg + ((size_t)cell * n + S) * n + col, v);
+    }
+    __syncthreads();
+  }
+#undef SPV
+}
+
+}  // namespace
+}  // namespace ck
+
+// ---- host: tables from the mechanism description ---------------------------------------------
+namespace ck {
+
+namespace {
+template <class T>
+size_t blob_add(std::vector<unsigned char> &blob, const std::vector<T> &v) {
+  const size_t off = (blob.size() + 255) / 256 * 256;
+  blob.resize(off + std::max<size_t>(v.size(), 1) * sizeof(T));
+  if (!v.empty()) std::memcpy(blob.data() + off, v.data(), v.size() * sizeof(T));
+  return off;
+}
+}  // namespace
+
+// Builds the device tables of the Jacobian kernel.  Returns "" or an error text; *out stays
+// NULL (with "") when the mechanism is not supported (approximate-ANN Kc) or does not fit.
+std::string jac_create(const ck_mech_desc *d, int num_sms, size_t smem_block_max, JacMech **out) {
+  *out = nullptr;
+  if (d->kc_ann) return "";
+  const int S = d->n_species, R = d->n_reactions;
+  const int cpl = (S + 1 + 31) / 32, SP = 32 * cpl;
+  if (cpl > 4) return "";   // S <= 127
+  std::vector<double> invW(S), lo(d->nasa_lo, d->nasa_lo + 7 * (size_t)S), hi(d->nasa_hi, d->nasa_hi + 7 * (size_t)S),
+      tmid(d->T_mid, d->T_mid + S);
+  for (int k = 0; k < S; ++k) invW[k] = 1.0 / d->mol_weight[k];
+  std::vector<JacRxn> rxn(R);
+  std::vector<JacSup> sup;
+  std::vector<int> tb_rxn;
+  std::vector<double> E;
+  for (int j = 0; j < R; ++j) {
+    JacRxn &r = rxn[j];
+    std::memset(&r, 0, sizeof r);
+    r.lnA = d->ln_A[j]; r.b = d->b[j]; r.EaR = d->Ea_over_R[j];
+    r.type = d->rxn_type ? d->rxn_type[j] : 0;
+    r.rev = d->reversible ? d->reversible[j] : 1;
+    r.tb = -1;
+    r.troe[1] = r.troe[2] = r.troe[3] = 1.0;
+    if (r.type >= 2) { r.lnA0 = d->ln_A0[j]; r.b0 = d->b0[j]; r.Ea0R = d->Ea0_over_R[j]; }
+    if (r.type == 3) for (int q = 0; q < 4; ++q) r.troe[q] = d->troe[4 * (size_t)j + q];
+    r.s0 = (int)sup.size();
+    for (int k = 0; k < S; ++k) {
+      const double f = d->nu_reac[(size_t)k * R + j], p = d->nu_prod[(size_t)k * R + j];
+      if (f == 0.0 && p == 0.0) continue;
+      sup.push_back(JacSup{f, p, k, 0});
+      r.dn += p - f; r.ordf += f; r.ordr += p;
+    }
+    r.s1 = (int)sup.size();
+    if (r.type != 0) {
+      r.tb = (int)tb_rxn.size();
+      tb_rxn.push_back(j);
+      E.resize(E.size() + SP, 0.0);
+      for (int k = 0; k < S; ++k) E[(size_t)r.tb * SP + k] = d->eff ? d->eff[(size_t)k * R + j] : 1.0;
+    }
+  }
+  // row lists: reactions with dnu_ij != 0, third-body / falloff ones first; off-diagonal
+  // entries (i, l != i) grouped by column l, reactions in ascending order (a fixed summation order)
+  std::vector<int> row_start(S + 1, 0), off_start((size_t)S * (SP + 1), 0);
+  std::vector<JacRowEnt> row_ent;
+  std::vector<JacOffEnt> off_ent;
+  for (int i = 0; i < S; ++i) {
+    row_start[i] = (int)row_ent.size();
+    for (int pass = 0; pass < 2; ++pass)
+      for (int j = 0; j < R; ++j) {
+        const double f = d->nu_reac[(size_t)i * R + j], p = d->nu_prod[(size_t)i * R + j], dnu = p - f;
+        if (dnu == 0.0 || (rxn[j].tb >= 0) != (pass == 0)) continue;
+        row_ent.push_back(JacRowEnt{dnu, dnu * f, dnu * p, j, rxn[j].tb});
+      }
+    for (int l = 0; l < SP; ++l) {
+      off_start[(size_t)i * (SP + 1) + l] = (int)off_ent.size();
+      if (l >= S || l == i) continue;
+      for (int j = 0; j < R; ++j) {
+        const double dnu = d->nu_prod[(size_t)i * R + j] - d->nu_reac[(size_t)i * R + j];
+        const double f = d->nu_reac[(size_t)l * R + j], p = d->nu_prod[(size_t)l * R + j];
+        if (dnu == 0.0 || (f == 0.0 && p == 0.0)) continue;
+        off_ent.push_back(JacOffEnt{dnu * f, dnu * p, j, 0});
+      }
+    }
+    off_start[(size_t)i * (SP + 1) + SP] = (int)off_ent.size();
+  }
+  row_start[S] = (int)row_ent.size();
+
+  JacMech *jm = new JacMech;
+  const int n_tb = (int)tb_rxn.size();
+  // cells per tile: 8 if the tile's shared memory fits, else 4
+  jm->cells = 8;
+  if (jac_smem_doubles(S, R, n_tb, 8, cpl) * 8 > smem_block_max) jm->cells = 4;
+  jm->smem = jac_smem_doubles(S, R, n_tb, jm->cells, cpl) * 8;
+  if (jm->smem > smem_block_max) { delete jm; return ""; }
+  jm->grid_max = num_sms;
+
+  std::vector<unsigned char> blob;
+  const size_t o_invW = blob_add(blob, invW), o_lo = blob_add(blob, lo), o_hi = blob_add(blob, hi),
+               o_tmid = blob_add(blob, tmid), o_rxn = blob_add(blob, rxn), o_sup = blob_add(blob, sup),
+               o_tbr = blob_add(blob, tb_rxn), o_E = blob_add(blob, E), o_rs = blob_add(blob, row_start),
+               o_re = blob_add(blob, row_ent), o_os = blob_add(blob, off_start), o_oe = blob_add(blob, off_ent);
+  cudaError_t ce = cudaMalloc(&jm->d_blob, blob.size());
+  if (ce == cudaSuccess) ce = cudaMemcpy(jm->d_blob, blob.data(), blob.size(), cudaMemcpyHostToDevice);
+  if (ce != cudaSuccess) {
+    if (jm->d_blob) cudaFree(jm->d_blob);
+    delete jm;
+    return std::string("Jacobian tables: ") + cudaGetErrorString(ce);
+  }
+  const unsigned char *b = (const unsigned char *)jm->d_blob;
+  JacTables &t = jm->t;
+  t.S = S; t.R = R; t.n_tb = n_tb; t.SP = SP;
+  t.invW = (const double *)(b + o_invW); t.nasa_lo = (const double *)(b + o_lo);
+  t.nasa_hi = (const double *)(b + o_hi); t.T_mid = (const double *)(b + o_tmid);
+  t.rxn = (const JacRxn *)(b + o_rxn); t.sup = (const JacSup *)(b + o_sup);
+  t.tb_rxn = (const int *)(b + o_tbr); t.E = (const double *)(b + o_E);
+  t.row_start = (const int *)(b + o_rs); t.row_ent = (const JacRowEnt *)(b + o_re);
+  t.off_start = (const int *)(b + o_os); t.off_ent = (const JacOffEnt *)(b + o_oe);
+  t.ln_pref_Ru = std::log(d->p_ref / kRu);
+  *out = jm;
+  return "";
+}
+
+void jac_destroy(JacMech *jm) {
+  if (!jm) return;
+  if (jm->d_blob) cudaFree(jm->d_blob);
+  delete jm;
+}
+
+int jac_cells_per_tile(const JacMech *jm) { return jm->cells; }
+
+cudaError_t jac_launch(const JacMech *jm, const double *T, const double *P, const double *Y, int64_t N,
+                       double *J, cudaStream_t stream) {
+  const int cpl = jm->t.SP / 32;
+  const long long tiles = (N + jm->cells - 1) / jm->cells;
+  const int grid = (int)std::min<long long>(tiles, jm->grid_max);
+#define CK_JAC_CASE(CE, CP)                                                                        \
+  if (jm->cells == CE && cpl == CP) {                                                              \
+    cudaError_t e = cudaFuncSetAttribute(jacobian_kernel<CE, CP>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                         (int)jm->smem);                                           \
+    if (e != cudaSuccess) return e;                                                                \
+    jacobian_kernel<CE, CP><<<grid, kJacThreads, jm->smem, stream>>>(jm->t, T, P, Y, (long long)N, J); \
+    return cudaGetLastError();                                                                     \
+  }
+  CK_JAC_CASE(8, 1) CK_JAC_CASE(8, 2) CK_JAC_CASE(8, 3) CK_JAC_CASE(8, 4)
+  CK_JAC_CASE(4, 1) CK_JAC_CASE(4, 2) CK_JAC_CASE(4, 3) CK_JAC_CASE(4, 4)
+#undef CK_JAC_CASE
+  return cudaErrorInvalidConfiguration;
+}
+
+}  // namespace ck

@@ -1,0 +1,167 @@
+"""Parity of ck_jacobian (through the C ABI) against the oracle's analytic Jacobian
+(oracle/ck_oracle_jac.c), entry by entry.
+
+Tolerance: the GPU forms every rate in log form (relative error of a
+rate ~1e-14 |ln q| ~ 1e-12) and each entry of a species row is a sum of such terms whose
+natural size is the largest entry of its column, so
+    |dJ_il| <= 1e-9 max_i |J_il| + 1e-11 |J_il|            (species rows, per cell and column)
+and the energy row, a sum over species that cancels like dT/dt itself, is measured against
+the sum of the absolute terms it is made of:
+    |dJ_Sl| <= 1e-9 (sum_k |H_k J_kl| / D + |J_Sl|),  H_k = (h_k/RT) Ru T, D = rho cp.
+"""
+import numpy as np
+import pytest
+
+import ckgen
+import oracle
+from helpers import RU
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def ck():
+    import paper_2008_08483_b200 as ck
+    assert torch.cuda.is_available()
+    return ck
+
+
+def gpu_jacobian(ck, gm, T, P, Y):
+    dev = torch.device("cuda:0")
+    N, S = T.shape[0], Y.shape[0]
+    Td, Pd, Yd = (torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (T, P, Y))
+    J = torch.full((N, S + 1, S + 1), float("nan"), dtype=torch.float64, device=dev)
+    gm.jacobian(Td, Pd, Yd, J, stream=torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    return J.cpu().numpy()
+
+
+def violations(mech, T, P, Y, J, Jr):
+    """Worst error/tolerance over the species rows and over the energy row."""
+    S = mech.n_species
+    om = oracle.OracleMechanism(mech)
+    assert np.isfinite(J).all()
+    col = np.abs(Jr[:, :S, :]).max(axis=1, keepdims=True)
+    tol = 1e-9 * col + 1e-11 * np.abs(Jr[:, :S, :])
+    rs = float((np.abs(J[:, :S, :] - Jr[:, :S, :]) / np.maximum(tol, 1e-300)).max())
+    re = 0.0
+    for i in range(T.shape[0]):
+        det = oracle.cell_detail(om, T[i], P[i], Y[:, i])
+        H = det["h_RT"] * RU * T[i]
+        D = det["rho"] * det["cp_mass"]
+        scale = (np.abs(H[:, None] * Jr[i, :S, :])).sum(0) / D + np.abs(Jr[i, S, :])
+        re = max(re, float((np.abs(J[i, S, :] - Jr[i, S, :]) / (1e-9 * scale)).max()))
+    return rs, re
+
+
+@pytest.mark.parametrize("cfg_name,N", [("tiny_1k", 1024), ("mid_1m", 203), ("large_256k", 61), ("mid_rk4", 50)])
+def test_parity_all_entries(ck, cfg_name, N):
+    cfg = ckgen.CONFIGS[cfg_name]
+    mech = ckgen.mechanism(cfg.mech)
+    T, P, Y = ckgen.states(cfg, N=N)
+    T[: N // 4] = np.linspace(350.0, 1000.0, N // 4)      # low NASA range and T = T_mid exactly
+    with ck.Mechanism(mech) as gm:
+        assert gm.info("jac_cells") in (4, 8)
+        J = gpu_jacobian(ck, gm, T, P, Y)
+    Jr = oracle.jacobian(oracle.OracleMechanism(mech), T, P, Y)
+    rs, re = violations(mech, T, P, Y, J, Jr)
+    assert rs <= 1.0 and re <= 1.0, (cfg_name, rs, re)
+
+
+@pytest.mark.parametrize("N", [1, 3, 7, 8, 9, 17])
+def test_ragged_batches_and_determinism(ck, N):
+    cfg = ckgen.CONFIGS["mid_1m"]
+    mech = ckgen.mechanism(cfg.mech)
+    T, P, Y = ckgen.states(cfg, N=N)
+    with ck.Mechanism(mech) as gm:
+        J1 = gpu_jacobian(ck, gm, T, P, Y)
+        J2 = gpu_jacobian(ck, gm, T, P, Y)
+    assert np.array_equal(J1, J2)
+    Jr = oracle.jacobian(oracle.OracleMechanism(mech), T, P, Y)
+    rs, re = violations(mech, T, P, Y, J1, Jr)
+    assert rs <= 1.0 and re <= 1.0, (N, rs, re)
+
+
+def test_single_reaction_mechanisms(ck):
+    """Each reaction type as a mechanism of its own (no reaction hides behind a larger one),
+    including irreversible ones."""
+    import dataclasses
+    mech = ckgen.mechanism(ckgen.MECH_MID)
+    cfg = dataclasses.replace(ckgen.CONFIGS["mid_1m"], T_range=(600.0, 2800.0))
+    T, P, Y = ckgen.states(cfg, N=40)
+    picks = np.concatenate([np.flatnonzero(mech.rxn_type == 3)[:4], np.flatnonzero(mech.rxn_type == 1)[:4],
+                            np.flatnonzero(mech.rxn_type == 0)[:6]])
+    for n, j in enumerate(picks):
+        sub = mech.subset([j])
+        if n % 2:
+            sub = dataclasses.replace(sub, reversible=np.zeros(1, np.uint8))
+        with ck.Mechanism(sub) as gm:
+            J = gpu_jacobian(ck, gm, T, P, Y)
+        Jr = oracle.jacobian(oracle.OracleMechanism(sub), T, P, Y)
+        rs, re = violations(sub, T, P, Y, J, Jr)
+        assert rs <= 1.0 and re <= 1.0, (int(j), rs, re)
+
+
+def test_lindemann_and_three_parameter_troe(ck):
+    import dataclasses
+    mech = ckgen.mechanism(ckgen.MECH_TINY)
+    rt = mech.rxn_type.copy()
+    troe = mech.troe.copy()
+    fo = np.flatnonzero(rt == 3)
+    rt[fo[0]] = 2                       # Lindemann
+    troe[fo[1:], 3] = np.inf            # 3-parameter Troe
+    mech = dataclasses.replace(mech, rxn_type=rt, troe=troe)
+    T, P, Y = ckgen.states(ckgen.CONFIGS["tiny_1k"], N=64)
+    with ck.Mechanism(mech) as gm:
+        J = gpu_jacobian(ck, gm, T, P, Y)
+    Jr = oracle.jacobian(oracle.OracleMechanism(mech), T, P, Y)
+    rs, re = violations(mech, T, P, Y, J, Jr)
+    assert rs <= 1.0 and re <= 1.0, (rs, re)
+
+
+@pytest.mark.parametrize("cfg_name,N", [("mid_1m", 1 << 15), ("large_256k", 1 << 13)])
+def test_bench_size_properties_and_sampled_parity(ck, cfg_name, N):
+    """At the size bench.py --jacobian times: Euler's relation sum_l Y_l J_il = 0 and mass
+    conservation sum_i W_i J_il = 0 on every cell (on the device), the oracle on a sample."""
+    cfg = ckgen.CONFIGS[cfg_name]
+    mech = ckgen.mechanism(cfg.mech)
+    S = mech.n_species
+    T, P, Y = ckgen.states(cfg, N=N)
+    dev = torch.device("cuda:0")
+    Td, Pd, Yd = (torch.from_numpy(a).to(dev) for a in (T, P, Y))
+    J = torch.empty((N, S + 1, S + 1), dtype=torch.float64, device=dev)
+    with ck.Mechanism(mech) as gm:
+        gm.jacobian(Td, Pd, Yd, J, stream=torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+    assert torch.isfinite(J).all()
+    terms = J[:, :, :S] * Yd.T[:, None, :]
+    assert (terms.sum(2).abs() <= 1e-9 * terms.abs().sum(2) + 1e-300).all()
+    del terms
+    w = torch.from_numpy(mech.mol_weight).to(dev)
+    t = J[:, :S, :] * w[None, :, None]
+    assert (t.sum(1).abs() <= 1e-9 * t.abs().sum(1) + 1e-300).all()
+    del t
+    idx = np.unique(np.concatenate([np.random.default_rng(7).integers(0, N, 40), [0, 7, 8, N - 9, N - 1]]))
+    Jr = oracle.jacobian(oracle.OracleMechanism(mech), T[idx], P[idx], np.ascontiguousarray(Y[:, idx]))
+    rs, re = violations(mech, T[idx], P[idx], np.ascontiguousarray(Y[:, idx]), J[idx].cpu().numpy(), Jr)
+    assert rs <= 1.0 and re <= 1.0, (rs, re)
+
+
+def test_errors(ck):
+    mech = ckgen.mechanism(ckgen.MECH_TINY)
+    ann = ckgen.random_kc_ann(mech.n_reactions, 1, 4, seed=1, T_range=(1000.0, 2500.0))
+    with ck.Mechanism(mech, kc_ann=ann) as gm:
+        assert gm.info("jac_cells") == 0
+        with pytest.raises(ck.CkError) as e:
+            ck.ck_jacobian(gm.handle, 8, 8, 8, 4, 8)
+        assert e.value.status == 4
+    with ck.Mechanism(mech) as gm:
+        ck.ck_jacobian(gm.handle, 0, 0, 0, 0, 0)           # N == 0: a no-op
+        with pytest.raises(ck.CkError) as e:
+            ck.ck_jacobian(gm.handle, 0, 8, 8, 4, 8)
+        assert e.value.status == 1
+        with pytest.raises(ck.CkError) as e:
+            ck.ck_jacobian(gm.handle, 8, 8, 8, -1, 8)
+        assert e.value.status == 1
