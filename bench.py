@@ -313,6 +313,67 @@ def run_ann(args):
     print(json.dumps(out))
 
 
+def run_jacobian(args):
+    """ck_jacobian, d(wdot, dT/dt)/d(Y, T) for N cells, cell-major
+    (S+1)x(S+1) matrices.  HBM-write bound: 8 (S+1)^2 bytes out per cell against 8 (S+2) in.
+    Times the three mechanism shapes; the oracle's Jacobian is timed beside it on a bounded
+    sample.  One JSON line."""
+    import torch
+    import ckgen
+    import oracle
+    import paper_2008_08483_b200 as ck
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    stream = torch.cuda.current_stream().cuda_stream
+    try:
+        hbm_peak = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
+        peak_src = "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        hbm_peak, peak_src = 6650.0, "fallback 6650 GB/s"
+    out = {"jacobian": "ck_jacobian, fp64, J[N][S+1][S+1] cell-major; device-resident inputs, CUDA events",
+           "rows": []}
+    for name, N in (("tiny_1m", 1 << 20), ("mid_1m", 1 << 16), ("large_256k", 1 << 14)):
+        if args.only and name != args.only:
+            continue
+        if args.cells:
+            N = args.cells
+        cfg = ckgen.CONFIGS[name]
+        mech = ckgen.mechanism(cfg.mech)
+        S, R = mech.n_species, mech.n_reactions
+        T, P, Y = ckgen.states(cfg, N=N)
+        Td, Pd, Yd = (torch.from_numpy(a).to(dev) for a in (T, P, Y))
+        J = torch.empty((N, S + 1, S + 1), dtype=torch.float64, device=dev)
+        with ck.Mechanism(mech) as gm:
+            for _ in range(max(args.warmup, 3)):
+                gm.jacobian(Td, Pd, Yd, J, stream=stream)
+            reps = max(args.steps, 10) if args.steps != 50 else 20
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(reps):
+                gm.jacobian(Td, Pd, Yd, J, stream=stream)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / reps
+            cells_per_tile = gm.info("jac_cells")
+        bytes_per_cell = 8 * ((S + 1) * (S + 1) + S + 2)
+        gbs = bytes_per_cell * N / (ms * 1e-3) / 1e9
+        row = {"S": S, "R": R, "N": N, "ms": ms, "cells_per_s": N / (ms * 1e-3), "cells_per_tile": cells_per_tile,
+               "roofline": {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+                            "bytes_per_cell": bytes_per_cell, "peak_source": peak_src},
+               "l2": "output %.0f MB per call vs 126 MB L2" % (8 * (S + 1) ** 2 * N / 1e6)}
+        if not args.no_cpu_baseline:
+            om = oracle.OracleMechanism(mech)
+            n = min(N, 2048 if S < 100 else 512)
+            t0 = time.perf_counter()
+            oracle.jacobian(om, T[:n], P[:n], np.ascontiguousarray(Y[:, :n]))
+            dt = time.perf_counter() - t0
+            row["cpu_baseline"] = {"value": n / dt, "unit": "cells/s", "kind": "oracle", "cores": os.cpu_count(),
+                                   "sample": "first %d cells, one pass, %.2f s" % (n, dt)}
+        out["rows"].append(row)
+    print(json.dumps(out))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -326,6 +387,8 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="configs[4]: saturation sweep over N (1 GPU)")
     ap.add_argument("--rk4", action="store_true", help="configs[4]: explicit RK4 reactor run (1 GPU)")
     ap.add_argument("--rk4-steps", type=int, default=1000)
+    ap.add_argument("--jacobian", action="store_true", help="ck_jacobian throughput and HBM roofline (1 GPU)")
+    ap.add_argument("--only", default="", help="--jacobian: only this mechanism's row (tiny_1m, mid_1m, large_256k)")
     ap.add_argument("--ann", action="store_true", help="Fig. 10 analogue: approximate-ANN vs exact log Kc (1 GPU)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -335,6 +398,8 @@ def main():
         return run_rk4(args)
     if args.ann:
         return run_ann(args)
+    if args.jacobian:
+        return run_jacobian(args)
 
     import ckgen
     cfg = ckgen.CONFIGS[args.workload]

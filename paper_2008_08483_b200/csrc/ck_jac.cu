@@ -46,7 +46,7 @@
 
 namespace ck {
 
-constexpr int kJacWarps = 8;
+constexpr int kJacWarps = 16;
 constexpr int kJacThreads = kJacWarps * 32;
 
 struct JacRowEnt {   // reaction j of row i: coefficients of a_j, b_j on the diagonal, dnu_ij
@@ -92,14 +92,37 @@ namespace ck {
 namespace {
 
 constexpr double kLn10 = 2.302585092994045684;
+constexpr int kJacStage = 64;   // row entries a warp stages in shared memory at a time
 enum { SP_C = 0, SP_INVC, SP_LNC, SP_HRT, SP_CPR, SP_DCPR, SP_GP, SP_COUNT };
-enum { CS_T = 0, CS_RHO, CS_S, CS_INVT, CS_LNT, CS_D, CS_DDT, CS_COUNT = 8 };
+enum { CS_T = 0, CS_RHO, CS_S, CS_INVT, CS_LNT, CS_D, CS_DDT, CS_INVS, CS_COUNT = 8 };
 
 // doubles of dynamic shared memory
-inline size_t jac_smem_doubles(int S, int R, int n_tb, int cells, int cpl) {
-  const size_t rx = (size_t)6 * R * cells, red = (size_t)kJacWarps * cells * (32 * cpl + 2);
+inline size_t jac_smem_doubles(int S, int R, int n_tb, int cells) {
   return (size_t)SP_COUNT * S * cells + (size_t)CS_COUNT * cells + (size_t)(n_tb > 0 ? n_tb : 1) * cells +
-         std::max(rx, red);
+         (size_t)4 * R * cells + (size_t)S * cells + (size_t)kJacWarps * kJacStage * (sizeof(JacRowEnt) / 8);
+}
+
+// Sum over the 32 lanes of v[c], c < CELLS, by a butterfly that halves the number of values a
+// lane carries at each step (CELLS - 1 + log2(32 / CELLS) shuffles instead of 5 CELLS).
+// Returns the total of cell jac_cell_of_lane<CELLS>(lane), the same on every lane of that cell.
+template <int CELLS>
+__device__ __forceinline__ int jac_cell_of_lane(int lane) {
+  return CELLS == 8 ? (lane >> 2) & 7 : (lane >> 3) & 3;
+}
+template <int CELLS>
+__device__ __forceinline__ double jac_reduce_cells(double (&v)[CELLS], int lane) {
+  int o = 16;
+#pragma unroll
+  for (int w = CELLS; w > 1; w >>= 1, o >>= 1) {
+    const bool upper = (lane & o) != 0;
+#pragma unroll
+    for (int q = 0; q < w / 2; ++q) {
+      const double send = upper ? v[q] : v[q + w / 2], keep = upper ? v[q + w / 2] : v[q];
+      v[q] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+    }
+  }
+  for (; o > 0; o >>= 1) v[0] += __shfl_xor_sync(0xffffffffu, v[0], o);
+  return v[0];
 }
 
 template <int CELLS, int CPL>
@@ -111,15 +134,12 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   double *sp = smem;                                   // [SP_COUNT][S][CELLS]
   double *cs = sp + (size_t)SP_COUNT * S * CELLS;      // [CELLS][CS_COUNT]
-  double *Mtb = cs + CS_COUNT * CELLS;                 // [n_tb][CELLS]
-  double *rx = Mtb + (size_t)(t.n_tb > 0 ? t.n_tb : 1) * CELLS;
-  double2 *AB = (double2 *)rx;                         // [R][CELLS]  (a, b)
-  double *Mm = rx + (size_t)2 * R * CELLS;             // [R][CELLS]  m
-  double *Tt = Mm + (size_t)R * CELLS;                 // t
-  double *Qq = Tt + (size_t)R * CELLS;                 // Q
-  double *Ee = Qq + (size_t)R * CELLS;                 // e
-  double *red = rx;                                    // phase E, aliases the reaction arrays
-  double *red2 = red + (size_t)kJacWarps * CELLS * 32 * CPL;
+  double *Mtb = cs + CS_COUNT * CELLS;                 // [n_tb][CELLS]  M, then m = dQ/dM
+  double2 *AB = (double2 *)(Mtb + (size_t)(t.n_tb > 0 ? t.n_tb : 1) * CELLS);   // [R][CELLS] (a, b)
+  double *Tt = (double *)AB + (size_t)2 * R * CELLS;   // [R][CELLS]  t = dQ/dT at constant C
+  double *Ee = Tt + (size_t)R * CELLS;                 // [R][CELLS]  e = sum_l C_l dQ/dC_l
+  double *Wd = Ee + (size_t)R * CELLS;                 // [S][CELLS]  wdot
+  JacRowEnt *stg = (JacRowEnt *)(Wd + (size_t)S * CELLS) + warp * kJacStage;   // this warp's staged row entries
 #define SPV(a, k, c) sp[((size_t)(a) * S + (k)) * CELLS + (c)]
   constexpr int PARTS = 32 / CELLS;
 
@@ -127,16 +147,18 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
   for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
     const long long cell0 = tile * CELLS;
     // ---- cell scalars: s = sum_k Y_k/W_k, rho; warp c <-> cell c -----------
-    for (int c = warp; c < CELLS; c += kJacWarps) {
+    if (warp < CELLS) {
+      const int c = warp;
       const long long cell = cell0 + c < N ? cell0 + c : N - 1;
       double s = 0.0;
-      for (int k = lane; k < S; k += 32) s += Yg[(size_t)k * N + cell] * t.invW[k];
+      for (int k = lane; k < S; k += 32) s += __ldcs(Yg + (size_t)k * N + cell) * t.invW[k];
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
       if (lane == 0) {
         const double T = Tg[cell], P = Pg[cell];
         cs[c * CS_COUNT + CS_T] = T;
         cs[c * CS_COUNT + CS_S] = s;
+        cs[c * CS_COUNT + CS_INVS] = 1.0 / s;
         cs[c * CS_COUNT + CS_RHO] = P / (kRu * T * s);
         cs[c * CS_COUNT + CS_INVT] = 1.0 / T;
         cs[c * CS_COUNT + CS_LNT] = log(T);
@@ -148,7 +170,7 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
       const int k = idx / CELLS, c = idx - k * CELLS;
       const long long cell = cell0 + c < N ? cell0 + c : N - 1;
       const double T = cs[c * CS_COUNT + CS_T], lnT = cs[c * CS_COUNT + CS_LNT], invT = cs[c * CS_COUNT + CS_INVT];
-      const double C = fmax(cs[c * CS_COUNT + CS_RHO] * Yg[(size_t)k * N + cell] * t.invW[k], kCFloor);
+      const double C = fmax(cs[c * CS_COUNT + CS_RHO] * __ldcs(Yg + (size_t)k * N + cell) * t.invW[k], kCFloor);
       SPV(SP_C, k, c) = C;
       SPV(SP_INVC, k, c) = 1.0 / C;
       SPV(SP_LNC, k, c) = log(C);
@@ -164,8 +186,9 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
       SPV(SP_GP, k, c) = hRT - sR - (t.ln_pref_Ru - lnT);
     }
     __syncthreads();
-    // D = rho cp = sum_k C_k Cp_k and dD/dT at constant C (+ the -D/T of dC/dT later)
-    for (int c = warp; c < CELLS; c += kJacWarps) {
+    // D = rho cp = sum_k C_k Cp_k and dD/dT (first at constant C, then the -D/T of dC/dT)
+    if (warp < CELLS) {
+      const int c = warp;
       double D = 0.0, dD = 0.0;
       for (int k = lane; k < S; k += 32) {
         D += SPV(SP_C, k, c) * SPV(SP_CPR, k, c);
@@ -181,18 +204,23 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
         cs[c * CS_COUNT + CS_DDT] = dD * kRu - D * kRu * cs[c * CS_COUNT + CS_INVT];
       }
     }
-    // ---- phase M: third-body layer M = C E, thread per (row of E, cell) -----
-    for (int idx = tid; idx < t.n_tb * CELLS; idx += kJacThreads) {
-      const int r = idx / CELLS, c = idx - r * CELLS;
-      const double *e = t.E + (size_t)r * SP;
-      double m0 = 0.0, m1 = 0.0;
-      int k = 0;
-      for (; k + 1 < S; k += 2) {
-        m0 = fma(__ldg(e + k), SPV(SP_C, k, c), m0);
-        m1 = fma(__ldg(e + k + 1), SPV(SP_C, k + 1, c), m1);
+    // ---- phase M: third-body layer M = C E: warp per row of E, lanes over the
+    //      species (coalesced row of E), the cells' partial sums reduced across the lanes
+    for (int r = warp; r < t.n_tb; r += kJacWarps) {
+      double v[CELLS];
+#pragma unroll
+      for (int c = 0; c < CELLS; ++c) v[c] = 0.0;
+#pragma unroll
+      for (int p = 0; p < CPL; ++p) {
+        const int k = lane + 32 * p;
+        if (k < S) {
+          const double e = __ldg(t.E + (size_t)r * SP + k);
+#pragma unroll
+          for (int c = 0; c < CELLS; ++c) v[c] = fma(e, SPV(SP_C, k, c), v[c]);
+        }
       }
-      if (k < S) m0 = fma(__ldg(e + k), SPV(SP_C, k, c), m0);
-      Mtb[r * CELLS + c] = m0 + m1;
+      const double tot = jac_reduce_cells<CELLS>(v, lane);
+      if ((lane & (PARTS - 1)) == 0) Mtb[r * CELLS + jac_cell_of_lane<CELLS>(lane)] = tot;
     }
     __syncthreads();
     // ---- phase B: rate layers and the derivative scalars, thread per (reaction, cell) ------
@@ -200,13 +228,25 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
       const int j = idx / CELLS, c = idx - j * CELLS;
       const JacRxn &r = t.rxn[j];
       const double lnT = cs[c * CS_COUNT + CS_LNT], invT = cs[c * CS_COUNT + CS_INVT], T = cs[c * CS_COUNT + CS_T];
+      const int s0 = r.s0, s1 = r.s1, type = r.type;
+      // the first entries of the support list in one batch of independent loads
+      JacSup u4[4];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) u4[q] = t.sup[s0 + q < s1 ? s0 + q : s0];
       // Arrhenius layer (Eq. 6) and its T-derivative
       double lnkf = r.lnA + r.b * lnT - r.EaR * invT;
       double dlnkf = (r.b + r.EaR * invT) * invT;
       // log-rate layers (Eq. 4) and the equilibrium layer (Eq. 11) over the reaction's species
       double sf = 0.0, sr = 0.0, dG = 0.0, dH = 0.0;
-      for (int e = r.s0; e < r.s1; ++e) {
-        const JacSup u = t.sup[e];
+      for (int e = s0; e < s1; ++e) {
+        JacSup u;
+        if (e - s0 < 4) {
+          u = u4[0];
+#pragma unroll
+          for (int q = 1; q < 4; ++q) if (e - s0 == q) u = u4[q];
+        } else {
+          u = t.sup[e];
+        }
         const double lc = SPV(SP_LNC, u.k, c), dnu = u.nur - u.nuf;
         sf = fma(u.nuf, lc, sf);
         sr = fma(u.nur, lc, sr);
@@ -215,15 +255,15 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
       }
       const double dlnKc = (dH - r.dn) * invT;
       double M = 1.0, phi = 1.0, gam = 1.0, dlnG = 0.0;
-      if (r.type != 0) M = Mtb[r.tb * CELLS + c];
-      if (r.type == 1) phi = M;
-      if (r.type >= 2) {
+      if (type != 0) M = Mtb[r.tb * CELLS + c];
+      if (type == 1) phi = M;
+      if (type >= 2) {
         // falloff (textbook forms): k = k_inf Pr/(1+Pr) F, Pr = k_0 M/k_inf
         const double lnk0 = r.lnA0 + r.b0 * lnT - r.Ea0R * invT;
         const double dlnk0 = (r.b0 + r.Ea0R * invT) * invT;
         const double Pr = exp(lnk0 - lnkf) * M;
         double F = 1.0, dlnF_dlnPr = 0.0, dlnF_dT = 0.0;
-        if (r.type == 3) {
+        if (type == 3) {
           const double alpha = r.troe[0], T3 = r.troe[1], T1 = r.troe[2], T2 = r.troe[3];
           const double e3 = exp(-T / T3), e1 = exp(-T / T1), e2 = exp(-T2 * invT);
           const double Fc = (1.0 - alpha) * e3 + alpha * e1 + e2;
@@ -245,141 +285,170 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
       const double qr = r.rev ? exp(lnkf + dG + sr) * gam : 0.0;   // ln k_r = ln k_f - ln Kc, ln Kc = -dG
       const double a = phi * qf, b = phi * qr;
       double m = 0.0;
-      if (r.type == 1) m = qf - qr;
-      if (r.type >= 2) m = (qf - qr) * dlnG / M;
+      if (type == 1) m = qf - qr;
+      if (type >= 2) m = (qf - qr) * dlnG / M;
       AB[idx] = make_double2(a, b);
-      Mm[idx] = m;
       Tt[idx] = a * dlnkf - b * (dlnkf - dlnKc);
-      Qq[idx] = a - b;
-      Ee[idx] = r.ordf * a - r.ordr * b + (r.type != 0 ? m * M : 0.0);
+      Ee[idx] = r.ordf * a - r.ordr * b + (type != 0 ? m * M : 0.0);
+      if (type != 0) Mtb[r.tb * CELLS + c] = m;   // M is dead: its slot carries m = dQ/dM from here on
     }
     __syncthreads();
     // ---- phase C: one warp per row i; lanes = columns, the tile's cells in registers -------
-    double eacc[CELLS][CPL];       // energy row: sum_i H_i dwdot_i/dx, this warp's rows
+    {
+      const int my_c = lane % CELLS, my_part = lane / CELLS;
+      double iw[CPL];
 #pragma unroll
-    for (int c = 0; c < CELLS; ++c)
-#pragma unroll
-      for (int p = 0; p < CPL; ++p) eacc[c][p] = 0.0;
-    double hw_acc = 0.0, cpw_acc = 0.0;   // lane c < CELLS: sum_i H_i wdot_i, sum_i Cp_i wdot_i
-    const int my_c = lane % CELLS, my_part = lane / CELLS;
-    for (int i = warp; i < S; i += kJacWarps) {
-      const int r0 = t.row_start[i], r1 = t.row_start[i + 1];
-      // (1) the row's reaction list, lanes = (cell, part): diagonal of the sparse part, T column,
-      //     wdot_i, g_i = sum_l C_l dwdot_i/dC_l (Euler's relation reaction by reaction)
-      double diag = 0.0, tsum = 0.0, wd = 0.0, g = 0.0;
-      for (int e = r0 + my_part; e < r1; e += PARTS) {
-        const JacRowEnt u = t.row_ent[e];
-        const int at = u.j * CELLS + my_c;
-        const double2 ab = AB[at];
-        diag = fma(u.cf, ab.x, fma(-u.cr, ab.y, diag));
-        tsum = fma(u.dnu, Tt[at], tsum);
-        wd = fma(u.dnu, Qq[at], wd);
-        g = fma(u.dnu, Ee[at], g);
-      }
-#pragma unroll
-      for (int o = CELLS; o < 32; o <<= 1) {
-        diag += __shfl_xor_sync(0xffffffffu, diag, o);
-        tsum += __shfl_xor_sync(0xffffffffu, tsum, o);
-        wd += __shfl_xor_sync(0xffffffffu, wd, o);
-        g += __shfl_xor_sync(0xffffffffu, g, o);
-      }
-      const double Hi_mine = SPV(SP_HRT, i, my_c) * kRu * cs[my_c * CS_COUNT + CS_T];
-      hw_acc = fma(Hi_mine, wd, hw_acc);
-      cpw_acc = fma(SPV(SP_CPR, i, my_c) * kRu, wd, cpw_acc);
-
-      double accS[CELLS][CPL], accD[CELLS][CPL];
-#pragma unroll
-      for (int c = 0; c < CELLS; ++c)
-#pragma unroll
-        for (int p = 0; p < CPL; ++p) accS[c][p] = accD[c][p] = 0.0;
-      // (2) off-diagonal sparse entries of row i, grouped by column
-#pragma unroll
-      for (int p = 0; p < CPL; ++p) {
-        const int col = lane + 32 * p;
-        const int *seg = t.off_start + (size_t)i * (SP + 1) + col;
-        const int e0 = col < SP ? seg[0] : 0, e1 = col < SP ? seg[1] : 0;
-        for (int e = e0; e < e1; ++e) {
-          const JacOffEnt u = t.off_ent[e];
-          const double2 *ab = AB + (size_t)u.j * CELLS;
-#pragma unroll
-          for (int c = 0; c < CELLS; ++c) {
-            const double2 v = ab[c];
-            accS[c][p] = fma(u.cf, v.x, fma(-u.cr, v.y, accS[c][p]));
-          }
-        }
-      }
-      // (3) third-body / falloff reactions of the row (listed first): coefficient x row of E
-      for (int e = r0; e < r1; ++e) {
-        const int tb = t.row_ent[e].tb;
-        if (tb < 0) break;
-        const double dnu = t.row_ent[e].dnu;
-        const double *mm = Mm + (size_t)t.row_ent[e].j * CELLS;
-        double ev[CPL];
-#pragma unroll
-        for (int p = 0; p < CPL; ++p) ev[p] = (lane + 32 * p < SP) ? __ldg(t.E + (size_t)tb * SP + lane + 32 * p) : 0.0;
-#pragma unroll
-        for (int c = 0; c < CELLS; ++c) {
-          const double co = dnu * mm[c];
-#pragma unroll
-          for (int p = 0; p < CPL; ++p) accD[c][p] = fma(co, ev[p], accD[c][p]);
-        }
-      }
-      // (4) C -> (Y, T) at constant P, store the row, accumulate the energy row
-#pragma unroll
-      for (int c = 0; c < CELLS; ++c) {
-        const double diag_c = __shfl_sync(0xffffffffu, diag, c);
-        const double tsum_c = __shfl_sync(0xffffffffu, tsum, c);
-        const double g_c = __shfl_sync(0xffffffffu, g, c);
-        const double rho = cs[c * CS_COUNT + CS_RHO], inv_s = 1.0 / cs[c * CS_COUNT + CS_S];
-        const double Hi = SPV(SP_HRT, i, c) * kRu * cs[c * CS_COUNT + CS_T];
-        const long long cell = cell0 + c;
+      for (int p = 0; p < CPL; ++p) iw[p] = (lane + 32 * p < S) ? t.invW[lane + 32 * p] : 0.0;
+      for (int i = warp; i < S; i += kJacWarps) {
+        const int r0 = t.row_start[i], r1 = t.row_start[i + 1];
+        // bounds and first entry of this lane's off-diagonal segments, in flight during (1)
+        int e0[CPL], e1[CPL];
+        JacOffEnt first[CPL];
 #pragma unroll
         for (int p = 0; p < CPL; ++p) {
-          const int col = lane + 32 * p;
-          double v = 0.0;
-          if (col < S) {
-            double jc = fma(accS[c][p] + (col == i ? diag_c : 0.0), SPV(SP_INVC, col, c), accD[c][p]);
-            const double iw = t.invW[col];
-            v = jc * (rho * iw) - g_c * (iw * inv_s);
-          } else if (col == S) {
-            v = tsum_c - g_c * cs[c * CS_COUNT + CS_INVT];
+          const int *seg = t.off_start + (size_t)i * (SP + 1) + lane + 32 * p;
+          e0[p] = __ldg(seg);
+          e1[p] = __ldg(seg + 1);
+        }
+#pragma unroll
+        for (int p = 0; p < CPL; ++p) first[p] = t.off_ent[e0[p]];   // (the table has a spare entry at its end)
+        // (1) the row's reaction list (staged in shared memory, 64 entries at a time), lanes =
+        //     (cell, part): diagonal of the sparse part, T column, wdot_i, and
+        //     g_i = sum_l C_l dwdot_i/dC_l by Euler's relation reaction by reaction
+        double diag = 0.0, tsum = 0.0, wd = 0.0, g = 0.0;
+        for (int base = r0; base < r1; base += kJacStage) {
+          const int cnt = min(kJacStage, r1 - base);
+          __syncwarp();
+          for (int q = lane; q < cnt * 4; q += 32) ((double *)stg)[q] = __ldg((const double *)(t.row_ent + base) + q);
+          __syncwarp();
+          for (int e = my_part; e < cnt; e += PARTS) {
+            const JacRowEnt u = stg[e];
+            const int at = u.j * CELLS + my_c;
+            const double2 ab = AB[at];
+            diag = fma(u.cf, ab.x, fma(-u.cr, ab.y, diag));
+            tsum = fma(u.dnu, Tt[at], tsum);
+            wd = fma(u.dnu, ab.x - ab.y, wd);
+            g = fma(u.dnu, Ee[at], g);
           }
-          if (col <= S && cell < N) __stcs(Jg + ((size_t)cell * n + i) * n + col, v);
-          eacc[c][p] = fma(Hi, v, eacc[c][p]);
+        }
+#pragma unroll
+        for (int o = CELLS; o < 32; o <<= 1) {
+          diag += __shfl_xor_sync(0xffffffffu, diag, o);
+          tsum += __shfl_xor_sync(0xffffffffu, tsum, o);
+          wd += __shfl_xor_sync(0xffffffffu, wd, o);
+          g += __shfl_xor_sync(0xffffffffu, g, o);
+        }
+        if (lane < CELLS) Wd[i * CELLS + lane] = wd;
+        // (2) off-diagonal sparse entries of row i, grouped by column (next entry prefetched)
+        double acc[CELLS][CPL];
+#pragma unroll
+        for (int c = 0; c < CELLS; ++c)
+#pragma unroll
+          for (int p = 0; p < CPL; ++p) acc[c][p] = 0.0;
+#pragma unroll
+        for (int p = 0; p < CPL; ++p) {
+          JacOffEnt u = first[p];
+          for (int e = e0[p]; e < e1[p]; ++e) {
+            const JacOffEnt un = t.off_ent[e + 1];
+            const double2 *ab = AB + (size_t)u.j * CELLS;
+#pragma unroll
+            for (int c = 0; c < CELLS; ++c) {
+              const double2 v = ab[c];
+              acc[c][p] = fma(u.cf, v.x, fma(-u.cr, v.y, acc[c][p]));
+            }
+            u = un;
+          }
+        }
+        // sparse part / C_l (with the diagonal), then (3) adds the dense part
+#pragma unroll
+        for (int c = 0; c < CELLS; ++c) {
+          const double diag_c = __shfl_sync(0xffffffffu, diag, c);
+#pragma unroll
+          for (int p = 0; p < CPL; ++p) {
+            const int col = lane + 32 * p;
+            acc[c][p] = col < S ? (acc[c][p] + (col == i ? diag_c : 0.0)) * SPV(SP_INVC, col, c) : 0.0;
+          }
+        }
+        // (3) third-body / falloff reactions of the row (listed first): coefficient x row of E
+        {
+          bool done = false;
+          for (int base = r0; base < r1 && !done; base += kJacStage) {
+            const int cnt = min(kJacStage, r1 - base);
+            if (r1 - r0 > kJacStage) {      // a long row: stage this chunk again
+              __syncwarp();
+              for (int q = lane; q < cnt * 4; q += 32) ((double *)stg)[q] = __ldg((const double *)(t.row_ent + base) + q);
+              __syncwarp();
+            }
+            double evn[CPL];
+#pragma unroll
+            for (int p = 0; p < CPL; ++p) evn[p] = stg[0].tb >= 0 ? __ldg(t.E + (size_t)stg[0].tb * SP + lane + 32 * p) : 0.0;
+            for (int e = 0; e < cnt; ++e) {
+              const JacRowEnt u = stg[e];
+              if (u.tb < 0) { done = true; break; }
+              double ev[CPL];
+#pragma unroll
+              for (int p = 0; p < CPL; ++p) ev[p] = evn[p];
+              const int tbn = e + 1 < cnt ? stg[e + 1].tb : -1;
+              if (tbn >= 0) {
+#pragma unroll
+                for (int p = 0; p < CPL; ++p) evn[p] = __ldg(t.E + (size_t)tbn * SP + lane + 32 * p);
+              }
+              const double *mm = Mtb + (size_t)u.tb * CELLS;
+#pragma unroll
+              for (int c = 0; c < CELLS; ++c) {
+                const double co = u.dnu * mm[c];
+#pragma unroll
+                for (int p = 0; p < CPL; ++p) acc[c][p] = fma(co, ev[p], acc[c][p]);
+              }
+            }
+          }
+        }
+        // (4) C -> (Y, T) at constant P, store the row
+#pragma unroll
+        for (int c = 0; c < CELLS; ++c) {
+          const double tsum_c = __shfl_sync(0xffffffffu, tsum, c);
+          const double g_c = __shfl_sync(0xffffffffu, g, c);
+          const double rho = cs[c * CS_COUNT + CS_RHO], inv_s = cs[c * CS_COUNT + CS_INVS];
+          const long long cell = cell0 + c;
+          if (cell < N) {
+            double *row = Jg + ((size_t)cell * n + i) * n;
+#pragma unroll
+            for (int p = 0; p < CPL; ++p) {
+              const int col = lane + 32 * p;
+              if (col < S) __stcs(row + col, acc[c][p] * (rho * iw[p]) - g_c * (iw[p] * inv_s));
+              else if (col == S) __stcs(row + col, tsum_c - g_c * cs[c * CS_COUNT + CS_INVT]);
+            }
+          }
         }
       }
     }
-    __syncthreads();   // the reaction arrays are dead: their memory becomes the reduction buffer
-    // ---- phase E: energy row dT/dt = -sum_k H_k wdot_k / D ---------------------------------
-#pragma unroll
-    for (int c = 0; c < CELLS; ++c)
-#pragma unroll
-      for (int p = 0; p < CPL; ++p) red[((size_t)warp * CELLS + c) * (32 * CPL) + lane + 32 * p] = eacc[c][p];
-    if (lane < CELLS) {
-      red2[(warp * CELLS + lane) * 2] = hw_acc;
-      red2[(warp * CELLS + lane) * 2 + 1] = cpw_acc;
-    }
     __syncthreads();
+    // ---- phase E: energy row, dT/dt = -sum_k H_k wdot_k / D; thread per (cell, column), the
+    //      species rows of the tile read back (from L2) in a fixed order
     for (int idx = tid; idx < CELLS * n; idx += kJacThreads) {
       const int c = idx / n, col = idx - c * n;
+      const long long cell = cell0 + c;
+      if (cell >= N) continue;
+      const double RuT = kRu * cs[c * CS_COUNT + CS_T];
+      const double *Jc = Jg + (size_t)cell * n * n + col;
       double hj = 0.0, hw = 0.0, cpw = 0.0;
-#pragma unroll
-      for (int w = 0; w < kJacWarps; ++w) {
-        hj += red[((size_t)w * CELLS + c) * (32 * CPL) + col];
-        hw += red2[(w * CELLS + c) * 2];
-        cpw += red2[(w * CELLS + c) * 2 + 1];
+#pragma unroll 8
+      for (int i = 0; i < S; ++i) {
+        const double H = SPV(SP_HRT, i, c) * RuT, w = Wd[i * CELLS + c];
+        hj = fma(H, __ldcg(Jc + (size_t)i * n), hj);
+        hw = fma(H, w, hw);
+        cpw = fma(SPV(SP_CPR, i, c) * kRu, w, cpw);
       }
       const double D = cs[c * CS_COUNT + CS_D], invD = 1.0 / D, Tdot = -hw * invD;
       double v;
       if (col < S) {
-        const double iw = t.invW[col];
-        const double dD = cs[c * CS_COUNT + CS_RHO] * SPV(SP_CPR, col, c) * kRu * iw - D * iw / cs[c * CS_COUNT + CS_S];
+        const double iwc = t.invW[col];
+        const double dD = cs[c * CS_COUNT + CS_RHO] * SPV(SP_CPR, col, c) * kRu * iwc - D * iwc * cs[c * CS_COUNT + CS_INVS];
         v = -hj * invD - Tdot * dD * invD;
       } else {
         v = -(cpw + hj) * invD - Tdot * cs[c * CS_COUNT + CS_DDT] * invD;
       }
-      const long long cell = cell0 + c;
-      if (cell < N) __stcs(Jg + ((size_t)cell * n + S) * n + col, v);
+      __stcs(Jg + ((size_t)cell * n + S) * n + col, v);
     }
     __syncthreads();
   }
@@ -468,13 +537,15 @@ std::string jac_create(const ck_mech_desc *d, int num_sms, size_t smem_block_max
     off_start[(size_t)i * (SP + 1) + SP] = (int)off_ent.size();
   }
   row_start[S] = (int)row_ent.size();
+  off_ent.push_back(JacOffEnt{0.0, 0.0, 0, 0});   // the kernel prefetches one entry past a segment
+  off_ent.push_back(JacOffEnt{0.0, 0.0, 0, 0});
 
   JacMech *jm = new JacMech;
   const int n_tb = (int)tb_rxn.size();
   // cells per tile: 8 if the tile's shared memory fits, else 4
   jm->cells = 8;
-  if (jac_smem_doubles(S, R, n_tb, 8, cpl) * 8 > smem_block_max) jm->cells = 4;
-  jm->smem = jac_smem_doubles(S, R, n_tb, jm->cells, cpl) * 8;
+  if (jac_smem_doubles(S, R, n_tb, 8) * 8 > smem_block_max) jm->cells = 4;
+  jm->smem = jac_smem_doubles(S, R, n_tb, jm->cells) * 8;
   if (jm->smem > smem_block_max) { delete jm; return ""; }
   jm->grid_max = num_sms;
 
