@@ -17,7 +17,7 @@
 // Y_l, column S is T.  23 KB per cell at S=53: the kernel is bound by these HBM writes
 // (DESIGN.md section 14), so the mapping is chosen for coalesced row stores:
 //
-//   block = 8 warps, tile of CELLS cells (8, or 4 for big mechanisms), persistent grid.
+//   block = 16 warps, tile of CELLS cells (8, or 4 for big mechanisms), persistent grid.
 //   phase A  thread per (species, cell): C, 1/C, ln C, NASA-7 h/RT, cp/R, d(cp/R)/dT, g'.
 //   phase M  thread per (third-body or falloff reaction, cell): M = sum_k E_kj C_k.
 //   phase B  thread per (reaction, cell): the rate layers in log form and the five scalars
@@ -94,7 +94,7 @@ namespace {
 constexpr double kLn10 = 2.302585092994045684;
 constexpr int kJacStage = 64;   // row entries a warp stages in shared memory at a time
 enum { SP_C = 0, SP_INVC, SP_LNC, SP_HRT, SP_CPR, SP_DCPR, SP_GP, SP_COUNT };
-enum { CS_T = 0, CS_RHO, CS_S, CS_INVT, CS_LNT, CS_D, CS_DDT, CS_INVS, CS_COUNT = 8 };
+enum { CS_T = 0, CS_RHO, CS_INVRS, CS_INVT, CS_LNT, CS_D, CS_DDT, CS_INVS, CS_COUNT = 8 };
 
 // doubles of dynamic shared memory
 inline size_t jac_smem_doubles(int S, int R, int n_tb, int cells) {
@@ -141,6 +141,9 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
   double *Wd = Ee + (size_t)R * CELLS;                 // [S][CELLS]  wdot
   JacRowEnt *stg = (JacRowEnt *)(Wd + (size_t)S * CELLS) + warp * kJacStage;   // this warp's staged row entries
 #define SPV(a, k, c) sp[((size_t)(a) * S + (k)) * CELLS + (c)]
+  // (a, b) of reaction j, cell c lives at AB[j * CELLS + (c ^ (j & (CELLS - 1)))]: lanes that read
+  // the same cell of different reactions (phase C (2)) then fall into different banks
+#define ABAT(j, c) ((j) * CELLS + ((c) ^ ((j) & (CELLS - 1))))
   constexpr int PARTS = 32 / CELLS;
 
   const long long n_tiles = (N + CELLS - 1) / CELLS;
@@ -157,7 +160,7 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
       if (lane == 0) {
         const double T = Tg[cell], P = Pg[cell];
         cs[c * CS_COUNT + CS_T] = T;
-        cs[c * CS_COUNT + CS_S] = s;
+        cs[c * CS_COUNT + CS_INVRS] = (kRu * T) / P;      // 1 / (rho s)
         cs[c * CS_COUNT + CS_INVS] = 1.0 / s;
         cs[c * CS_COUNT + CS_RHO] = P / (kRu * T * s);
         cs[c * CS_COUNT + CS_INVT] = 1.0 / T;
@@ -287,7 +290,7 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
       double m = 0.0;
       if (type == 1) m = qf - qr;
       if (type >= 2) m = (qf - qr) * dlnG / M;
-      AB[idx] = make_double2(a, b);
+      AB[ABAT(j, c)] = make_double2(a, b);
       Tt[idx] = a * dlnkf - b * (dlnkf - dlnKc);
       Ee[idx] = r.ordf * a - r.ordr * b + (type != 0 ? m * M : 0.0);
       if (type != 0) Mtb[r.tb * CELLS + c] = m;   // M is dead: its slot carries m = dQ/dM from here on
@@ -324,7 +327,7 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
           for (int e = my_part; e < cnt; e += PARTS) {
             const JacRowEnt u = stg[e];
             const int at = u.j * CELLS + my_c;
-            const double2 ab = AB[at];
+            const double2 ab = AB[ABAT(u.j, my_c)];
             diag = fma(u.cf, ab.x, fma(-u.cr, ab.y, diag));
             tsum = fma(u.dnu, Tt[at], tsum);
             wd = fma(u.dnu, ab.x - ab.y, wd);
@@ -351,9 +354,10 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
           for (int e = e0[p]; e < e1[p]; ++e) {
             const JacOffEnt un = t.off_ent[e + 1];
             const double2 *ab = AB + (size_t)u.j * CELLS;
+            const int sw = u.j & (CELLS - 1);
 #pragma unroll
             for (int c = 0; c < CELLS; ++c) {
-              const double2 v = ab[c];
+              const double2 v = ab[c ^ sw];
               acc[c][p] = fma(u.cf, v.x, fma(-u.cr, v.y, acc[c][p]));
             }
             u = un;
@@ -408,14 +412,15 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
         for (int c = 0; c < CELLS; ++c) {
           const double tsum_c = __shfl_sync(0xffffffffu, tsum, c);
           const double g_c = __shfl_sync(0xffffffffu, g, c);
-          const double rho = cs[c * CS_COUNT + CS_RHO], inv_s = cs[c * CS_COUNT + CS_INVS];
+          // dwdot_i/dY_l = rho/W_l (dwdot_i/dC_l - g_i/(rho s))
+          const double rho = cs[c * CS_COUNT + CS_RHO], gk = g_c * cs[c * CS_COUNT + CS_INVRS];
           const long long cell = cell0 + c;
           if (cell < N) {
             double *row = Jg + ((size_t)cell * n + i) * n;
 #pragma unroll
             for (int p = 0; p < CPL; ++p) {
               const int col = lane + 32 * p;
-              if (col < S) __stcs(row + col, acc[c][p] * (rho * iw[p]) - g_c * (iw[p] * inv_s));
+              if (col < S) __stcs(row + col, (acc[c][p] - gk) * (rho * iw[p]));
               else if (col == S) __stcs(row + col, tsum_c - g_c * cs[c * CS_COUNT + CS_INVT]);
             }
           }
@@ -453,6 +458,7 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
     __syncthreads();
   }
 #undef SPV
+#undef ABAT
 }
 
 }  // namespace
@@ -482,23 +488,30 @@ std::string jac_create(const ck_mech_desc *d, int num_sms, size_t smem_block_max
   std::vector<double> invW(S), lo(d->nasa_lo, d->nasa_lo + 7 * (size_t)S), hi(d->nasa_hi, d->nasa_hi + 7 * (size_t)S),
       tmid(d->T_mid, d->T_mid + S);
   for (int k = 0; k < S; ++k) invW[k] = 1.0 / d->mol_weight[k];
+  // Internal reaction order: by type (elementary, three-body, Lindemann, Troe), so that the warps
+  // of phase B (thread per (reaction, cell)) are homogeneous in type; oj = order[j]
+  std::vector<int> order;
+  for (int ty = 0; ty <= 3; ++ty)
+    for (int j = 0; j < R; ++j)
+      if ((d->rxn_type ? d->rxn_type[j] : 0) == ty) order.push_back(j);
   std::vector<JacRxn> rxn(R);
   std::vector<JacSup> sup;
   std::vector<int> tb_rxn;
   std::vector<double> E;
   for (int j = 0; j < R; ++j) {
+    const int oj = order[j];
     JacRxn &r = rxn[j];
     std::memset(&r, 0, sizeof r);
-    r.lnA = d->ln_A[j]; r.b = d->b[j]; r.EaR = d->Ea_over_R[j];
-    r.type = d->rxn_type ? d->rxn_type[j] : 0;
-    r.rev = d->reversible ? d->reversible[j] : 1;
+    r.lnA = d->ln_A[oj]; r.b = d->b[oj]; r.EaR = d->Ea_over_R[oj];
+    r.type = d->rxn_type ? d->rxn_type[oj] : 0;
+    r.rev = d->reversible ? d->reversible[oj] : 1;
     r.tb = -1;
     r.troe[1] = r.troe[2] = r.troe[3] = 1.0;
-    if (r.type >= 2) { r.lnA0 = d->ln_A0[j]; r.b0 = d->b0[j]; r.Ea0R = d->Ea0_over_R[j]; }
-    if (r.type == 3) for (int q = 0; q < 4; ++q) r.troe[q] = d->troe[4 * (size_t)j + q];
+    if (r.type >= 2) { r.lnA0 = d->ln_A0[oj]; r.b0 = d->b0[oj]; r.Ea0R = d->Ea0_over_R[oj]; }
+    if (r.type == 3) for (int q = 0; q < 4; ++q) r.troe[q] = d->troe[4 * (size_t)oj + q];
     r.s0 = (int)sup.size();
     for (int k = 0; k < S; ++k) {
-      const double f = d->nu_reac[(size_t)k * R + j], p = d->nu_prod[(size_t)k * R + j];
+      const double f = d->nu_reac[(size_t)k * R + oj], p = d->nu_prod[(size_t)k * R + oj];
       if (f == 0.0 && p == 0.0) continue;
       sup.push_back(JacSup{f, p, k, 0});
       r.dn += p - f; r.ordf += f; r.ordr += p;
@@ -508,7 +521,7 @@ std::string jac_create(const ck_mech_desc *d, int num_sms, size_t smem_block_max
       r.tb = (int)tb_rxn.size();
       tb_rxn.push_back(j);
       E.resize(E.size() + SP, 0.0);
-      for (int k = 0; k < S; ++k) E[(size_t)r.tb * SP + k] = d->eff ? d->eff[(size_t)k * R + j] : 1.0;
+      for (int k = 0; k < S; ++k) E[(size_t)r.tb * SP + k] = d->eff ? d->eff[(size_t)k * R + oj] : 1.0;
     }
   }
   // row lists: reactions with dnu_ij != 0, third-body / falloff ones first; off-diagonal
@@ -520,7 +533,8 @@ std::string jac_create(const ck_mech_desc *d, int num_sms, size_t smem_block_max
     row_start[i] = (int)row_ent.size();
     for (int pass = 0; pass < 2; ++pass)
       for (int j = 0; j < R; ++j) {
-        const double f = d->nu_reac[(size_t)i * R + j], p = d->nu_prod[(size_t)i * R + j], dnu = p - f;
+        const int oj = order[j];
+        const double f = d->nu_reac[(size_t)i * R + oj], p = d->nu_prod[(size_t)i * R + oj], dnu = p - f;
         if (dnu == 0.0 || (rxn[j].tb >= 0) != (pass == 0)) continue;
         row_ent.push_back(JacRowEnt{dnu, dnu * f, dnu * p, j, rxn[j].tb});
       }
@@ -528,8 +542,9 @@ std::string jac_create(const ck_mech_desc *d, int num_sms, size_t smem_block_max
       off_start[(size_t)i * (SP + 1) + l] = (int)off_ent.size();
       if (l >= S || l == i) continue;
       for (int j = 0; j < R; ++j) {
-        const double dnu = d->nu_prod[(size_t)i * R + j] - d->nu_reac[(size_t)i * R + j];
-        const double f = d->nu_reac[(size_t)l * R + j], p = d->nu_prod[(size_t)l * R + j];
+        const int oj = order[j];
+        const double dnu = d->nu_prod[(size_t)i * R + oj] - d->nu_reac[(size_t)i * R + oj];
+        const double f = d->nu_reac[(size_t)l * R + oj], p = d->nu_prod[(size_t)l * R + oj];
         if (dnu == 0.0 || (f == 0.0 && p == 0.0)) continue;
         off_ent.push_back(JacOffEnt{dnu * f, dnu * p, j, 0});
       }
