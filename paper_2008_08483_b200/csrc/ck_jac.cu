@@ -19,21 +19,25 @@
 //
 //   block = 16 warps, tile of CELLS cells (8, or 4 for big mechanisms), persistent grid.
 //   phase A  thread per (species, cell): C, 1/C, ln C, NASA-7 h/RT, cp/R, d(cp/R)/dT, g'.
-//   phase M  thread per (third-body or falloff reaction, cell): M = sum_k E_kj C_k.
-//   phase B  thread per (reaction, cell): the rate layers in log form and the five scalars
-//            every derivative of Q_j is made of:
+//   phase M  warp per third-body / falloff reaction: M = sum_k E_kj C_k, lanes over the species
+//            (coalesced row of E), the cells' partial sums reduced with a halving butterfly.
+//   phase B  thread per (reaction, cell), reactions ordered by type so that warps are
+//            homogeneous: the rate layers in log form and the scalars every derivative of Q_j
+//            is made of:
 //              a = phi q_f, b = phi q_r        dQ/dC_l|sparse = (nu'_lj a - nu''_lj b)/C_l
-//              m                               dQ/dC_l|dense  = m E_lj
-//              t = dQ/dT at constant C,  Q,    e = sum_l C_l dQ/dC_l = ord' a - ord'' b + m M
+//              m                               dQ/dC_l|dense  = m E_lj  (stored over M)
+//              t = dQ/dT at constant C,        e = sum_l C_l dQ/dC_l = ord' a - ord'' b + m M
 //   phase C  warp per row i (species), lanes = columns l, the tile's cells in registers:
 //            the row of d wdot_i/dC is gathered (never scattered: no atomics, fixed order)
-//            from three host-built lists -- the reactions of row i (diagonal, T column, wdot_i
-//            and g_i = sum_l C_l dwdot_i/dC_l, lanes = (cell, quarter of the list)), the
-//            off-diagonal sparse entries grouped by column, and the third-body reactions of
-//            the row (dense in l: coefficient x row of E) -- then mapped to (Y, T):
-//              dwdot_i/dY_l = rho/W_l dwdot_i/dC_l - g_i/(s W_l),  dwdot_i/dT = t-sum - g_i/T
-//            stored as one coalesced row per cell, and accumulated into the energy row.
-//   phase E  energy row: cross-warp sum of H_i x row i, then the quotient rule.
+//            from three host-built lists -- (1) the reactions of row i, staged in shared memory
+//            (diagonal, T column, wdot_i and g_i = sum_l C_l dwdot_i/dC_l by Euler's relation,
+//            lanes = (cell, part of the list)), (2) the off-diagonal sparse entries grouped by
+//            column, (3) the third-body reactions of the row (dense in l: coefficient x row of
+//            E) -- then (4) mapped to (Y, T):
+//              dwdot_i/dY_l = rho/W_l (dwdot_i/dC_l - g_i/(rho s)),  dwdot_i/dT = t-sum - g_i/T
+//            and stored as one coalesced row per cell.
+//   phase E  energy row, thread per (cell, column): sum_i H_i x row i read back from L2 in a
+//            fixed order, then the quotient rule on dT/dt = -sum_k H_k wdot_k / (rho cp).
 #include <cuda_runtime.h>
 
 #include <algorithm>
