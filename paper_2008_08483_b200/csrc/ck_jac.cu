@@ -42,6 +42,8 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -50,8 +52,8 @@
 
 namespace ck {
 
-constexpr int kJacWarps = 16;
-constexpr int kJacThreads = kJacWarps * 32;
+// Launch shapes: 16 warps per block, one block per SM, tiles of 4 to 32 cells (the most that fit);
+// 8 warps and two blocks per SM exist as measured alternatives (CK_JAC_SHAPE; slower).
 
 struct JacRowEnt {   // reaction j of row i: coefficients of a_j, b_j on the diagonal, dnu_ij
   double dnu, cf, cr;   // dnu_ij, dnu_ij nu'_ij, dnu_ij nu''_ij
@@ -86,6 +88,7 @@ struct JacMech {
   JacTables t{};
   void *d_blob = nullptr;
   int cells = 8;               // cells per tile
+  int warps = 16, minb = 1;    // warps per block, blocks per SM
   size_t smem = 0;
   int grid_max = 1;
 };
@@ -101,7 +104,7 @@ enum { SP_C = 0, SP_INVC, SP_LNC, SP_HRT, SP_CPR, SP_DCPR, SP_GP, SP_COUNT };
 enum { CS_T = 0, CS_RHO, CS_INVRS, CS_INVT, CS_LNT, CS_D, CS_DDT, CS_INVS, CS_COUNT = 8 };
 
 // doubles of dynamic shared memory
-inline size_t jac_smem_doubles(int S, int R, int n_tb, int cells) {
+inline size_t jac_smem_doubles(int S, int R, int n_tb, int cells, int kJacWarps) {
   return (size_t)SP_COUNT * S * cells + (size_t)CS_COUNT * cells + (size_t)(n_tb > 0 ? n_tb : 1) * cells +
          (size_t)4 * R * cells + (size_t)S * cells + (size_t)kJacWarps * kJacStage * (sizeof(JacRowEnt) / 8);
 }
@@ -111,7 +114,8 @@ inline size_t jac_smem_doubles(int S, int R, int n_tb, int cells) {
 // Returns the total of cell jac_cell_of_lane<CELLS>(lane), the same on every lane of that cell.
 template <int CELLS>
 __device__ __forceinline__ int jac_cell_of_lane(int lane) {
-  return CELLS == 8 ? (lane >> 2) & 7 : (lane >> 3) & 3;
+  // the butterfly consumes lane bits 4, 3, ... for the cell bits from the top down
+  return CELLS == 32 ? lane : CELLS == 16 ? (lane >> 1) & 15 : CELLS == 8 ? (lane >> 2) & 7 : (lane >> 3) & 3;
 }
 template <int CELLS>
 __device__ __forceinline__ double jac_reduce_cells(double (&v)[CELLS], int lane) {
@@ -129,11 +133,12 @@ __device__ __forceinline__ double jac_reduce_cells(double (&v)[CELLS], int lane)
   return v[0];
 }
 
-template <int CELLS, int CPL>
-__global__ void __launch_bounds__(kJacThreads, 1)
+template <int CELLS, int CPL, int kJacWarps, int MINB>
+__global__ void __launch_bounds__(kJacWarps * 32, MINB)
 jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *__restrict__ Pg,
                 const double *__restrict__ Yg, long long N, double *__restrict__ Jg) {
   extern __shared__ __align__(16) double smem[];
+  constexpr int kJacThreads = kJacWarps * 32;
   const int S = t.S, R = t.R, n = S + 1, SP = t.SP;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   double *sp = smem;                                   // [SP_COUNT][S][CELLS]
@@ -154,8 +159,7 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
   for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
     const long long cell0 = tile * CELLS;
     // ---- cell scalars: s = sum_k Y_k/W_k, rho; warp c <-> cell c -----------
-    if (warp < CELLS) {
-      const int c = warp;
+    for (int c = warp; c < CELLS; c += kJacWarps) {
       const long long cell = cell0 + c < N ? cell0 + c : N - 1;
       double s = 0.0;
       for (int k = lane; k < S; k += 32) s += __ldcs(Yg + (size_t)k * N + cell) * t.invW[k];
@@ -194,8 +198,7 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
     }
     __syncthreads();
     // D = rho cp = sum_k C_k Cp_k and dD/dT (first at constant C, then the -D/T of dC/dT)
-    if (warp < CELLS) {
-      const int c = warp;
+    for (int c = warp; c < CELLS; c += kJacWarps) {
       double D = 0.0, dD = 0.0;
       for (int k = lane; k < S; k += 32) {
         D += SPV(SP_C, k, c) * SPV(SP_CPR, k, c);
@@ -561,12 +564,21 @@ std::string jac_create(const ck_mech_desc *d, int num_sms, size_t smem_block_max
 
   JacMech *jm = new JacMech;
   const int n_tb = (int)tb_rxn.size();
-  // cells per tile: 8 if the tile's shared memory fits, else 4
-  jm->cells = 8;
-  if (jac_smem_doubles(S, R, n_tb, 8) * 8 > smem_block_max) jm->cells = 4;
-  jm->smem = jac_smem_doubles(S, R, n_tb, jm->cells) * 8;
+  // launch shape: 8 cells x 16 warps if the tile's shared memory fits, else 4 cells x 16 warps;
+  // CK_JAC_SHAPE=cells,warps,blocks_per_sm overrides (measurement knob)
+  // the most cells per tile (32, 16, 8, 4) whose tile fits shared memory and whose row
+  // accumulators (cells x columns per lane doubles) fit the registers of 512 threads
+  jm->cells = 4; jm->warps = 16; jm->minb = 1;
+  for (int c : {32, 16, 8})
+    if (c * cpl <= 32 && jac_smem_doubles(S, R, n_tb, c, 16) * 8 <= smem_block_max) { jm->cells = c; break; }
+  if (const char *e = std::getenv("CK_JAC_SHAPE")) {
+    int c = 0, w = 0, b = 0;
+    if (std::sscanf(e, "%d,%d,%d", &c, &w, &b) == 3 && (c == 4 || c == 8 || ((c == 16 || c == 32) && c * cpl <= 32)) && (w == 8 || w == 16) && (b == 1 || b == 2) &&
+        !(w == 16 && b == 2)) { jm->cells = c; jm->warps = w; jm->minb = b; }
+  }
+  jm->smem = jac_smem_doubles(S, R, n_tb, jm->cells, jm->warps) * 8;
   if (jm->smem > smem_block_max) { delete jm; return ""; }
-  jm->grid_max = num_sms;
+  jm->grid_max = num_sms * jm->minb;
 
   std::vector<unsigned char> blob;
   const size_t o_invW = blob_add(blob, invW), o_lo = blob_add(blob, lo), o_hi = blob_add(blob, hi),
@@ -607,16 +619,19 @@ cudaError_t jac_launch(const JacMech *jm, const double *T, const double *P, cons
   const int cpl = jm->t.SP / 32;
   const long long tiles = (N + jm->cells - 1) / jm->cells;
   const int grid = (int)std::min<long long>(tiles, jm->grid_max);
-#define CK_JAC_CASE(CE, CP)                                                                        \
-  if (jm->cells == CE && cpl == CP) {                                                              \
-    cudaError_t e = cudaFuncSetAttribute(jacobian_kernel<CE, CP>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                                         (int)jm->smem);                                           \
+#define CK_JAC_CASE(CE, CP, WA, MB)                                                                \
+  if (jm->cells == CE && cpl == CP && jm->warps == WA && jm->minb == MB) {                         \
+    cudaError_t e = cudaFuncSetAttribute(jacobian_kernel<CE, CP, WA, MB>,                          \
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)jm->smem); \
     if (e != cudaSuccess) return e;                                                                \
-    jacobian_kernel<CE, CP><<<grid, kJacThreads, jm->smem, stream>>>(jm->t, T, P, Y, (long long)N, J); \
+    jacobian_kernel<CE, CP, WA, MB><<<grid, WA * 32, jm->smem, stream>>>(jm->t, T, P, Y, (long long)N, J); \
     return cudaGetLastError();                                                                     \
   }
-  CK_JAC_CASE(8, 1) CK_JAC_CASE(8, 2) CK_JAC_CASE(8, 3) CK_JAC_CASE(8, 4)
-  CK_JAC_CASE(4, 1) CK_JAC_CASE(4, 2) CK_JAC_CASE(4, 3) CK_JAC_CASE(4, 4)
+#define CK_JAC_SHAPES(CE, CP) CK_JAC_CASE(CE, CP, 16, 1) CK_JAC_CASE(CE, CP, 8, 1) CK_JAC_CASE(CE, CP, 8, 2)
+  CK_JAC_SHAPES(8, 1) CK_JAC_SHAPES(8, 2) CK_JAC_SHAPES(8, 3) CK_JAC_SHAPES(8, 4)
+  CK_JAC_SHAPES(4, 1) CK_JAC_SHAPES(4, 2) CK_JAC_SHAPES(4, 3) CK_JAC_SHAPES(4, 4)
+  CK_JAC_CASE(32, 1, 16, 1) CK_JAC_CASE(16, 1, 16, 1) CK_JAC_CASE(16, 2, 16, 1)
+#undef CK_JAC_SHAPES
 #undef CK_JAC_CASE
   return cudaErrorInvalidConfiguration;
 }

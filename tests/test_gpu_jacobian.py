@@ -63,7 +63,7 @@ def test_parity_all_entries(ck, cfg_name, N):
     T, P, Y = ckgen.states(cfg, N=N)
     T[: N // 4] = np.linspace(350.0, 1000.0, N // 4)      # low NASA range and T = T_mid exactly
     with ck.Mechanism(mech) as gm:
-        assert gm.info("jac_cells") in (4, 8)
+        assert gm.info("jac_cells") in (4, 8, 16, 32)
         J = gpu_jacobian(ck, gm, T, P, Y)
     Jr = oracle.jacobian(oracle.OracleMechanism(mech), T, P, Y)
     rs, re = violations(mech, T, P, Y, J, Jr)
@@ -82,6 +82,28 @@ def test_ragged_batches_and_determinism(ck, N):
     Jr = oracle.jacobian(oracle.OracleMechanism(mech), T, P, Y)
     rs, re = violations(mech, T, P, Y, J1, Jr)
     assert rs <= 1.0 and re <= 1.0, (N, rs, re)
+
+
+@pytest.mark.parametrize("shape", ["4,16,1", "8,16,1", "16,16,1", "32,16,1", "4,8,2"])
+@pytest.mark.parametrize("N", [1, 31, 33, 70])
+def test_every_launch_shape_on_the_tiny_mechanism(ck, monkeypatch, shape, N):
+    """Tiles of 4 to 32 cells and both block sizes (CK_JAC_SHAPE = cells, warps, blocks per SM),
+    with batches that leave a ragged last tile: same bits from every shape (the arithmetic of a
+    cell does not depend on the tile it falls in), parity on one of them."""
+    cfg = ckgen.CONFIGS["tiny_1k"]
+    mech = ckgen.mechanism(cfg.mech)
+    T, P, Y = ckgen.states(cfg, N=N)
+    with ck.Mechanism(mech) as gm:
+        Jd = gpu_jacobian(ck, gm, T, P, Y)
+    monkeypatch.setenv("CK_JAC_SHAPE", shape)
+    with ck.Mechanism(mech) as gm:
+        assert gm.info("jac_cells") == int(shape.split(",")[0])
+        J = gpu_jacobian(ck, gm, T, P, Y)
+    Jr = oracle.jacobian(oracle.OracleMechanism(mech), T, P, Y)
+    rs, re = violations(mech, T, P, Y, J, Jr)
+    assert rs <= 1.0 and re <= 1.0, (shape, N, rs, re)
+    rs, re = violations(mech, T, P, Y, Jd, Jr)
+    assert rs <= 1.0 and re <= 1.0, ("default", N, rs, re)
 
 
 def test_single_reaction_mechanisms(ck):
