@@ -200,7 +200,9 @@ const char *ck_last_error(void);
  *       14 kernel variant in use (0 generic table-driven kernel, 1 mechanism-specialised),
  *       15 species whose accumulators the specialised kernel keeps in registers (the other
  *       S - that many accumulate in shared memory; 0 for the generic kernel),
- *       16 cells per tile of the Jacobian kernel (0 if ck_jacobian is unsupported here).
+ *       16 cells per tile of the Jacobian kernel (0 if ck_jacobian is unsupported here),
+ *       17 1 if the specialised kernel runs two threads per cell (then 9 counts both, and a
+ *       block works on half that many cells).
  * Returns -1 for a NULL handle or unknown `what`. */
 int64_t ck_mech_info(const ck_mech *m, int what);
 

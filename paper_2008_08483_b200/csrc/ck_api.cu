@@ -219,7 +219,42 @@ std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk,
           if (better) { best_nt = nt; best_b = b; best_tab = tab_smem != 0; best_smem = smem; best_sreg = s_reg; }
         }
   }
+  // Two threads per cell (CK_PAIR): for mechanisms whose accumulators do not fit one thread's
+  // registers, 2 x cells threads share the cells' columns and split the accumulators, which puts
+  // twice the warps on a scheduler for the same shared memory.  CK_JIT_PAIR=1 forces it on any
+  // mechanism (tests), =0 disables it.  Not combined with the approximate ANN.
+  const int pair_env = env_int("CK_JIT_PAIR", -1);
+  bool pair = false;
+  if (!spec.kc_ann && pair_env != 0 && (pair_env == 1 || !all_regs)) {
+    int p_nt = 0, p_sreg = 0;
+    bool p_tab = false;
+    size_t p_smem = 0;
+    for (int nt : {512, 384, 256, 128})
+      for (int tab_smem = 1; tab_smem >= 0; --tab_smem) {
+        if (nt_forced && nt != nt_forced) continue;
+        const int cells = nt / 2;
+        const int regcap = std::min(255, (65536 / nt) / 8 * 8);
+        int s_reg = std::min((S + 1) / 2, (regcap - rest) / 2);
+        if (sreg_forced >= 0) s_reg = std::min((S + 1) / 2, sreg_forced);
+        if (s_reg < 0 || 2 * s_reg + 48 > regcap) continue;
+        if (sreg_forced < 0 && 2 * s_reg < S / 4) continue;
+        const int n_cold = std::max(0, S - 2 * s_reg);
+        const size_t smem = (size_t)(S + n_cold) * (cells + 8) * 8 + (128 * spec.lut_rep + 256) * 8 +
+                            (size_t)spec.n_ranges * S * 12 * 8 +
+                            (tab_smem ? tab_bytes : (size_t)(nt / 32) * 2 * spec.tab_ranges * spec.block * spec.row * 8) +
+                            (size_t)(4 * spec.block + 8) * cells * 8 + 16;
+        if (smem > smem_blk || smem + 1024 > smem_sm) continue;
+        const bool better = nt > p_nt || (nt == p_nt && (tab_smem != 0) > p_tab);
+        if (better) { p_nt = nt; p_sreg = s_reg; p_tab = tab_smem != 0; p_smem = smem; }
+      }
+    // worth it only if it puts more threads on the SM than the one-thread-per-cell shape
+    if (p_nt > 0 && (pair_env == 1 || p_nt > best_nt * best_b)) {
+      pair = true;
+      best_nt = p_nt; best_b = 1; best_tab = p_tab; best_sreg = p_sreg; best_smem = p_smem;
+    }
+  }
   if (best_nt == 0) return "no launch shape fits registers and shared memory";
+  spec.pair = pair;
   spec.threads = best_nt; spec.min_blocks = best_b; spec.tab_in_smem = best_tab; spec.s_reg = best_sreg;
   // tuning knobs for A/B runs under ncu (defaults are the measured best)
   if (const char *e = std::getenv("CK_JIT_M")) spec.m_dmma = std::string(e) != "dfma";
@@ -313,7 +348,7 @@ void finalize_jit(const ck_mech_desc *d, HostBuild *hb, const std::vector<double
   // so that the register accumulators serve the most updates; identity if all are in registers.
   std::vector<int> perm(S), inv(S);
   for (int k = 0; k < S; ++k) perm[k] = k;
-  if (spec.s_reg < S) {
+  if (spec.pair || spec.s_reg < S) {
     std::vector<int> hits(S, 0);
     for (const ck::JitReaction &r : spec.rxn)
       for (const auto &e : r.net) hits[e.first]++;
@@ -599,6 +634,7 @@ int setup_jit(ck_mech *m, ck::JitSpec &spec, const std::string &why, size_t smem
     return give_up(std::string("loading the specialised kernel: ") + cudaGetErrorString(ce));
   }
   m->jit_threads = spec.threads; m->jit_blocks_per_sm = spec.min_blocks; m->jit_smem = smem;
+  m->jit_cells = spec.pair ? spec.threads / 2 : spec.threads;
   m->jit_spec = spec;
   m->jit_grid_max = m->num_sms * spec.min_blocks;
   const size_t elems = (size_t)m->jit_grid_max * std::max(spec.n_mb, 1) * ck::kMBlock * spec.threads;
@@ -700,7 +736,7 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   m->jit_params.thermo = (const double *)(base + o_jthermo);
   m->jit_params.logtab = (const double *)(base + o_jlog);
   if (int st = setup_jit(m, spec, hb.jit_why, hb.jit_smem)) { ck_mech_destroy(m); return st; }
-  m->jit_s_reg = spec.s_reg;
+  m->jit_s_reg = spec.pair ? std::min(2 * spec.s_reg, S) : spec.s_reg;
   // ---- tables of the Jacobian kernel (ck_jac.cu) ------------------------------------------
   {
     const std::string err = ck::jac_create(d, m->num_sms, (size_t)prop.sharedMemPerBlockOptin, &m->jac);
@@ -856,7 +892,7 @@ namespace {
 void ensure_rk4_kernel(ck_mech *m) {
   if (m->rk4_tried) return;
   m->rk4_tried = true;
-  if (!m->jit_kernel) return;
+  if (!m->jit_kernel || m->jit_spec.pair) return;   // (the two-threads-per-cell kernel has no stage variant)
   if (const char *e = std::getenv("CK_RK4_FUSED")) if (std::atoi(e) == 0) return;
   ck::JitSpec spec = m->jit_spec;
   spec.rk4 = true;
@@ -877,7 +913,7 @@ void ensure_rk4_kernel(ck_mech *m) {
 
 // tile size and grid of a launch of the specialised kernel (balanced tiles, see ck_source_terms)
 int jit_tiling(const ck_mech *m, int64_t N, int *tile_cells) {
-  const int64_t nt = m->jit_threads;
+  const int64_t nt = m->jit_cells;
   const int64_t waves = ((N + nt - 1) / nt + m->jit_grid_max - 1) / m->jit_grid_max;
   int64_t tc = (N + m->jit_grid_max * waves - 1) / (m->jit_grid_max * waves);
   tc = std::min<int64_t>(nt, (tc + 31) / 32 * 32);
@@ -987,6 +1023,7 @@ extern "C" int64_t ck_mech_info(const ck_mech *m, int what) {
     case 14: return m->jit_kernel ? 1 : 0;
     case 15: return m->jit_kernel ? m->jit_s_reg : 0;
     case 16: return m->jac ? ck::jac_cells_per_tile(m->jac) : 0;
+    case 17: return (m->jit_kernel && m->jit_spec.pair) ? 1 : 0;
     default: return -1;
   }
 }

@@ -43,7 +43,8 @@ struct JitSpec {
   bool m_dmma = true;          // M = C E on DMMA.8x8x4 (else register-tiled DFMA)
   int sync_every = 0;          // block barrier every n reaction blocks (0 = never)
   int block = 4;               // reactions per block of the core
-  int s_reg = 0;               // species with register accumulators (internal order); rest in smem
+  int s_reg = 0;               // register accumulators per thread (internal species order); rest in smem
+  bool pair = false;           // two threads per cell (CK_PAIR in ck_jit_kernel.cuh): threads = 2 x cells
   std::vector<int> perm;       // internal species -> row of Y / wdot; empty = identity
   int tab_ranges = 1, row = 10;  // rate table: ranges and doubles per row
   bool rk4 = false;            // the explicit-RK4 stage variant of the kernel (ck_rk4_integrate)
@@ -91,6 +92,7 @@ struct ck_mech {
   cudaKernel_t jit_kernel = nullptr;
   ck::JitParams jit_params{};
   int jit_threads = 0, jit_blocks_per_sm = 0, jit_grid_max = 0, jit_s_reg = 0;
+  int jit_cells = 0;          // cells per block of the specialised kernel (= threads, or half with pair)
   size_t jit_smem = 0;
   double *d_jit_scratch = nullptr;
   ck::JitSpec jit_spec;       // kept to compile the RK4 stage variant on first use

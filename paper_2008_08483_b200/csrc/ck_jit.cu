@@ -117,7 +117,7 @@ std::string jit_generate_source(const JitSpec &s) {
     << "\n#define CK_G_TB0 " << s.group_end[1] << "\n#define CK_G_FO0 " << s.group_end[3]
     << "\n#define CK_TAB_NRANGES " << s.tab_ranges << "\n#define CK_ROW " << s.row
     << "\n#define CK_RK4 " << (s.rk4 ? 1 : 0) << "\n#define CK_KC_ANN " << (s.kc_ann ? 1 : 0) << "\n#define CK_KC_NONE " << (s.kc_none ? 1 : 0)
-    << "\n#define CK_LUT_REP " << s.lut_rep << "\n#define CK_SREG " << s.s_reg << "\n#define CK_PERM " << (s.perm.empty() ? 0 : 1) << "\n";
+    << "\n#define CK_PAIR " << (s.pair ? 1 : 0) << "\n#define CK_LUT_REP " << s.lut_rep << "\n#define CK_SREG " << s.s_reg << "\n#define CK_PERM " << (s.perm.empty() ? 0 : 1) << "\n";
   if (!s.perm.empty()) {
     o << "__constant__ int ck_c_perm[" << s.perm.size() << "] = {";
     for (size_t i = 0; i < s.perm.size(); ++i) o << (i ? "," : "") << (i % 16 == 0 ? "\n  " : " ") << s.perm[i];
@@ -142,56 +142,104 @@ std::string jit_generate_source(const JitSpec &s) {
   const size_t at = text.find(marker);
   o << text.substr(0, at);
   const int B = s.block, nblk = (int)s.rxn.size() / B;
-  // One switch case per loop trip: the scatters of the previous block (Eq. 2) and the
-  // gathers of this one (Eq. 4), so that the unique code is walked in address order with one
-  // indirect branch per block; trip CK_NBLK only scatters the last block.
-  o << "__device__ __forceinline__ void ck_reactions(const CkCtx &x, double (&w)[CK_SREG > 0 ? CK_SREG : 1]) {\n"
-    << "  double gf[CK_B], gr[CK_B], q[CK_B];\n"
-    << "#if !CK_TAB_SMEM\n  ck_ring_issue(x, 0);\n#endif\n"
-    << "#pragma unroll 1\n  for (int blk = 0; blk <= CK_NBLK; ++blk) {\n"
-    << "#if !CK_TAB_SMEM\n    ck_ring_issue(x, blk + 1);\n#endif\n"
-    << "    switch (blk) {\n";
-  auto scatters = [&](int k) {
-    for (int b = 0; b < B; ++b) {
-      const JitReaction &r = s.rxn[(size_t)k * B + b];
+  const int nhot = s.pair ? std::min(2 * s.s_reg, s.S) : s.s_reg;
+  // accumulator of internal species sp, and (pair mode) the half of the cell's thread pair that owns it
+  auto acc_of = [&](int sp, int *owner) {
+    if (sp < nhot) {
+      *owner = s.pair ? (sp & 1) : 0;
+      return "w[" + std::to_string(s.pair ? sp >> 1 : sp) + "]";
+    }
+    const int c = sp - nhot;
+    *owner = s.pair ? (c & 1) : 0;
+    return "CK_WC(" + std::to_string(c) + ")";
+  };
+  // scatters of block k (Eq. 2) restricted to the species owned by `half` (-1: all), q from `qsrc`
+  auto scatters = [&](int k, int half, const std::string &qsrc) {
+    for (int bb = 0; bb < B; ++bb) {
+      const JitReaction &r = s.rxn[(size_t)k * B + bb];
+      const std::string q = qsrc + std::to_string(bb) + (qsrc == "q[" ? "]" : "");
       for (size_t e = 0; e < r.net.size(); ++e) {
-        const int sp = r.net[e].first;
+        int owner = 0;
+        const std::string acc = acc_of(r.net[e].first, &owner);
+        if (half >= 0 && owner != half) continue;
         const double c = r.net[e].second;
-        // register accumulator, or the cold species' column in shared memory
-        const std::string acc = sp < s.s_reg ? "w[" + std::to_string(sp) + "]"
-                                             : "CK_WC(" + std::to_string(sp - s.s_reg) + ")";
-        if (c == 1.0) o << "        " << acc << " += q[" << b << "];\n";
-        else if (c == -1.0) o << "        " << acc << " -= q[" << b << "];\n";
-        else o << "        " << acc << " = fma(" << lit(c) << ", q[" << b << "], " << acc << ");\n";
+        if (c == 1.0) o << "        " << acc << " += " << q << ";\n";
+        else if (c == -1.0) o << "        " << acc << " -= " << q << ";\n";
+        else o << "        " << acc << " = fma(" << lit(c) << ", " << q << ", " << acc << ");\n";
       }
     }
   };
-  for (int k = 0; k <= nblk; ++k) {
-    o << "      case " << k << ":\n";
-    if (k > 0) scatters(k - 1);
-    if (k < nblk)
-      for (int b = 0; b < B; ++b) {
-        const JitReaction &r = s.rxn[(size_t)k * B + b];
-        o << "        gf[" << b << "] = " << gather_expr(r.reac) << ";";
-        if (r.index >= 0) o << "  // reaction " << r.index;
-        o << "\n        gr[" << b << "] = " << (r.reversible ? gather_expr(r.prod) : std::string("0.0")) << ";\n";
-      }
-    o << "        break;\n";
-  }
-  o << "    }\n#if !CK_TAB_SMEM\n    ck_ring_wait();\n#endif\n";
+  auto gathers = [&](int k) {
+    for (int bb = 0; bb < B; ++bb) {
+      const JitReaction &r = s.rxn[(size_t)k * B + bb];
+      o << "        gf[" << bb << "] = " << gather_expr(r.reac) << ";";
+      if (r.index >= 0) o << "  // reaction " << r.index;
+      o << "\n        gr[" << bb << "] = " << (r.reversible ? gather_expr(r.prod) : std::string("0.0")) << ";\n";
+    }
+  };
   const char *names[6] = {"ck_core<0, 1>", "ck_core<0, 0>", "ck_core<1, 1>", "ck_core<1, 0>",
                           "ck_core<2, 1>", "ck_core<2, 0>"};
-  bool first = true;
-  for (int g = 0; g < 6; ++g) {
-    const int lo = g ? s.group_end[g - 1] : 0;
-    if (s.group_end[g] == lo) continue;
-    o << "    " << (first ? "if" : "else if") << " (blk < " << s.group_end[g] << ") " << names[g]
-      << "(x, blk, gf, gr, q);\n";
-    first = false;
+  auto dispatch = [&](const char *indent, const char *slot) {
+    bool first = true;
+    for (int g = 0; g < 6; ++g) {
+      const int lo = g ? s.group_end[g - 1] : 0;
+      if (s.group_end[g] == lo) continue;
+      o << indent << (first ? "if" : "else if") << " (blk < " << s.group_end[g] << ") " << names[g]
+        << "(x, blk, " << slot << ", gf, gr, q);\n";
+      first = false;
+    }
+  };
+  o << "__device__ __forceinline__ void ck_reactions(const CkCtx &x, double (&w)[CK_SREG > 0 ? CK_SREG : 1]) {\n"
+    << "  double gf[CK_B], gr[CK_B], q[CK_B];\n";
+  if (!s.pair) {
+    // One switch case per loop trip: the scatters of the previous block (Eq. 2) and the
+    // gathers of this one (Eq. 4), so that the unique code is walked in address order with one
+    // indirect branch per block; trip CK_NBLK only scatters the last block.
+    o << "#if !CK_TAB_SMEM\n  ck_ring_issue(x, 0, 0);\n#endif\n"
+      << "#pragma unroll 1\n  for (int blk = 0; blk <= CK_NBLK; ++blk) {\n"
+      << "#if !CK_TAB_SMEM\n    ck_ring_issue(x, blk + 1, (blk + 1) & 1);\n#endif\n"
+      << "    switch (blk) {\n";
+    for (int k = 0; k <= nblk; ++k) {
+      o << "      case " << k << ":\n";
+      if (k > 0) scatters(k - 1, -1, "q[");
+      if (k < nblk) gathers(k);
+      o << "        break;\n";
+    }
+    o << "    }\n#if !CK_TAB_SMEM\n    ck_ring_wait();\n#endif\n";
+    dispatch("    ", "blk & 1");
+    if (s.sync_every > 0)
+      o << "    if (blk % " << s.sync_every << " == " << s.sync_every - 1 << ") __syncthreads();\n";
+    o << "  }\n}\n";
+  } else {
+    // Two threads per cell: trip pr handles the pair of blocks (2 pr, 2 pr + 1).  Half h gathers and
+    // evaluates block 2 pr + h and publishes its q in the exchange buffer; after the pair's barrier
+    // (next trip) each half scatters BOTH blocks into the species it owns: its own q from
+    // registers, the other half's from shared memory.  One switch per half.
+    o << "#if !CK_TAB_SMEM\n  ck_ring_issue(x, x.half, 0);\n#endif\n"
+      << "#pragma unroll 1\n  for (int pr = 0; pr <= (CK_NBLK + 1) / 2; ++pr) {\n"
+      << "    const int blk = 2 * pr + x.half;\n"
+      << "#if !CK_TAB_SMEM\n    ck_ring_issue(x, blk + 2, (pr + 1) & 1);\n#endif\n";
+    for (int h = 0; h < 2; ++h) {
+      o << (h == 0 ? "    if (x.half == 0) {\n" : "    } else {\n") << "    switch (pr) {\n";
+      for (int k = 0; k <= (nblk + 1) / 2; ++k) {
+        o << "      case " << k << ": {\n";
+        if (k > 0) {
+          for (int bb = 0; bb < B; ++bb)
+            o << "        const double o" << bb << " = CK_XQ(" << ((k - 1) & 1) << ", " << (1 - h) << ", " << bb << ");\n";
+          if (2 * (k - 1) + h < nblk) scatters(2 * (k - 1) + h, h, "q[");
+          if (2 * (k - 1) + (1 - h) < nblk) scatters(2 * (k - 1) + (1 - h), h, "o");
+        }
+        if (2 * k + h < nblk) gathers(2 * k + h);
+        o << "      } break;\n";
+      }
+      o << "    }\n";
+    }
+    o << "    }\n#if !CK_TAB_SMEM\n    ck_ring_wait();\n#endif\n"
+      << "    if (blk < CK_NBLK) {\n";
+    dispatch("      ", "pr & 1");
+    o << "#pragma unroll\n      for (int b = 0; b < CK_B; ++b) CK_XQ(pr & 1, x.half, b) = q[b];\n"
+      << "    }\n    ck_pair_sync(x.bar);\n  }\n}\n";
   }
-  if (s.sync_every > 0)
-    o << "    if (blk % " << s.sync_every << " == " << s.sync_every - 1 << ") __syncthreads();\n";
-  o << "  }\n}\n";
   o << text.substr(at + marker.size());
   return o.str();
 }

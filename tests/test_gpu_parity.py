@@ -38,6 +38,8 @@ def test_variant_selection(ck, kernel_variant):
             if kernel_variant == "auto":
                 # S=111 does not fit 2 registers per species: hot/cold accumulator split
                 assert (gm.info("s_reg") < spec.S) == (spec is ckgen.MECH_LARGE)
+                # ... and that shape runs two threads per cell
+                assert gm.info("pair") == (1 if spec is ckgen.MECH_LARGE else 0)
 
 
 @pytest.mark.parametrize("s_reg", [0, 7, 30])
@@ -47,12 +49,33 @@ def test_cold_accumulators_on_small_mechanisms(ck, monkeypatch, kernel_variant, 
     if kernel_variant != "auto":
         pytest.skip("specialised kernel only")
     monkeypatch.setenv("CK_JIT_SREG", str(s_reg))
+    monkeypatch.setenv("CK_JIT_PAIR", "0")      # one thread per cell (the pair shape has its own test)
     for cfg_name, N in (("tiny_1k", 1024), ("mid_1m", 777)):
         cfg = ckgen.CONFIGS[cfg_name]
         mech = ckgen.mechanism(cfg.mech)
         with ck.Mechanism(mech) as gm:
             assert gm.info("jit") == 1 and gm.info("s_reg") == min(s_reg, mech.n_species)
         assert_parity(ck, mech, *ckgen.states(cfg, N=N), label="%s s_reg=%d" % (cfg_name, s_reg))
+
+
+@pytest.mark.parametrize("s_reg", [None, 0, 3, 12])
+def test_two_threads_per_cell_on_small_mechanisms(ck, monkeypatch, kernel_variant, s_reg):
+    """The two-threads-per-cell shape of the specialised kernel (CK_PAIR: halves of a cell's pair
+    take alternate reaction blocks and alternate species and exchange rates through shared
+    memory), forced on mechanisms that would not need it, with all accumulators in registers
+    and with some or all of them in the shared-memory (cold) columns; ragged batches so that
+    partly filled and idle warp pairs occur."""
+    if kernel_variant != "auto":
+        pytest.skip("specialised kernel only")
+    monkeypatch.setenv("CK_JIT_PAIR", "1")
+    if s_reg is not None:
+        monkeypatch.setenv("CK_JIT_SREG", str(s_reg))
+    for cfg_name, N in (("tiny_1k", 1024), ("tiny_1k", 77), ("mid_1m", 777), ("mid_1m", 129)):
+        cfg = ckgen.CONFIGS[cfg_name]
+        mech = ckgen.mechanism(cfg.mech)
+        with ck.Mechanism(mech) as gm:
+            assert gm.info("jit") == 1 and gm.info("pair") == 1
+        assert_parity(ck, mech, *ckgen.states(cfg, N=N), label="pair %s s_reg=%s N=%d" % (cfg_name, s_reg, N))
 
 
 def gpu_run(ck, mech, T, P, Y, gm=None):
