@@ -286,6 +286,24 @@ void finalize_jit(const ck_mech_desc *d, HostBuild *hb, const std::vector<double
   // blocks of 4 reactions; 6 when the accumulators do not all fit in registers: that shape has
   // one warp per scheduler and needs the longer independent chains (measured)
   int kJitBlock = (2 * S + 48 > 255) ? 6 : 4;   // tuning knob CK_JIT_B (1..8)
+  if (R <= 64 && kJitBlock == 4) {
+    // Small mechanisms: every group is padded to whole blocks with null reactions that cost as
+    // much as real ones (at S=9/R=21 blocks of 4 evaluate 24 slots, two of them Troe, for 21
+    // reactions): take the block size in 2..4 with the least padded work (three-body 1.2, falloff 4
+    // elementary reactions' worth).  Measured at S=9/R=21: 0.195 ms with blocks of 2, 0.224 with 4.
+    double best = 0.0;
+    for (int b = 2; b <= 4; ++b) {
+      int n[3] = {0, 0, 0}, nr[3] = {0, 0, 0};
+      for (int j = 0; j < R; ++j) {
+        const int t = orig[j].type == 0 ? 0 : (orig[j].type == 1 ? 1 : 2);
+        (orig[j].reversible ? n[t] : nr[t])++;
+      }
+      const double wgt[3] = {1.0, 1.2, 4.0};
+      double cost = 0.0;
+      for (int t = 0; t < 3; ++t) cost += wgt[t] * b * ((n[t] + b - 1) / b + (nr[t] + b - 1) / b);
+      if (b == 2 || cost < best) { best = cost; kJitBlock = b; }
+    }
+  }
   if (const char *e = std::getenv("CK_JIT_B")) kJitBlock = std::min(8, std::max(1, std::atoi(e)));
   auto group_of = [](const ck::JitReaction &r) {
     const int t = r.type == 0 ? 0 : (r.type == 1 ? 1 : 2);
