@@ -200,6 +200,24 @@ def test_temperature_at_below_and_across_T_mid(ck):
     assert_parity(ck, mech, T, P, Y, "T around T_mid")
 
 
+@pytest.mark.parametrize("cfg_name", ["tiny_1k", "mid_1m", "large_256k"])
+def test_wide_temperature_and_pressure_range(ck, cfg_name):
+    """The whole fitted temperature range of the NASA-7 data (300-3500 K, and beyond to 4500 K)
+    and four decades of pressure, far outside the configs' own state distributions: both
+    temperature ranges, rates from underflow to 1e+100 and beyond."""
+    cfg = ckgen.CONFIGS[cfg_name]
+    mech = ckgen.mechanism(cfg.mech)
+    N = 600
+    _, _, Y = ckgen.states(cfg, N=N)
+    rng = np.random.default_rng(99)
+    T = rng.uniform(300.0, 4500.0, N)
+    P = 10.0 ** rng.uniform(3.5, 7.5, N)
+    wr, dr, _ = oracle.source_terms(oracle.OracleMechanism(mech), T, P, Y)
+    ok = np.isfinite(wr).all(0) & np.isfinite(dr)          # (the oracle's product form overflows first)
+    assert ok.mean() > 0.9
+    assert_parity(ck, mech, T[ok], P[ok], np.ascontiguousarray(Y[:, ok]), "%s wide T, P" % cfg_name)
+
+
 def test_distinct_T_mid_per_species(ck):
     """Several temperature ranges: the folded equilibrium layer keeps one coefficient row
     per range delimited by the distinct T_mid values."""
