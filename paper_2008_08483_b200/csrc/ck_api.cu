@@ -170,7 +170,11 @@ int env_int(const char *name, int dflt) {
 std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk, size_t *smem_out) {
   const int S = spec.S, R = spec.R;
   const bool fits = 2 * S + 48 <= 255;
-  const int rest = std::max(48, env_int("CK_JIT_REST", fits ? 144 : 166));
+  // registers beside the accumulators: the interleaved exp chains of a block (two per reaction)
+  // dominate, so smaller blocks need fewer (measured at S=9 with blocks of 2: 512 threads x 128
+  // registers 0.183 ms, 384 x 168 0.196 ms)
+  const int rest_dflt = !fits ? 166 : (spec.block <= 2 ? 100 : (spec.block == 3 ? 124 : 144));
+  const int rest = std::max(48, env_int("CK_JIT_REST", rest_dflt));
   const int sreg_forced = std::min(S, env_int("CK_JIT_SREG", -1));   // tuning / test knob
   const size_t tab_bytes = (size_t)spec.tab_ranges * R * spec.row * sizeof(double);   // R includes padding
   const int nt_forced = env_int("CK_JIT_NT", 0), b_forced = env_int("CK_JIT_MINB", 0);
