@@ -143,6 +143,30 @@ def test_lindemann_and_three_parameter_troe(ck):
     assert rs <= 1.0 and re <= 1.0, (rs, re)
 
 
+def test_catalyst_species_real_valued_nu_and_irreversible_reactions(ck):
+    """A + B -> A + C style reactions (nu' and nu'' overlap: the species has a column but no row
+    entry for that reaction), a real-valued stoichiometric coefficient, a third of the
+    reactions irreversible."""
+    import dataclasses
+    cfg = ckgen.CONFIGS["tiny_1k"]
+    mech = ckgen.mechanism(cfg.mech)
+    nu_r, nu_p = mech.nu_reac.copy(), mech.nu_prod.copy()
+    free = int(np.flatnonzero((nu_r[:, 0] == 0) & (nu_p[:, 0] == 0))[0])
+    nu_r[free, 0] += 1.0
+    nu_p[free, 0] += 1.0
+    k = int(np.flatnonzero(nu_r[:, 1])[0])
+    nu_r[k, 1] = 1.5
+    rev = mech.reversible.copy()
+    rev[::3] = 0
+    mech = dataclasses.replace(mech, nu_reac=nu_r, nu_prod=nu_p, reversible=rev)
+    T, P, Y = ckgen.states(cfg, N=90)
+    with ck.Mechanism(mech) as gm:
+        J = gpu_jacobian(ck, gm, T, P, Y)
+    Jr = oracle.jacobian(oracle.OracleMechanism(mech), T, P, Y)
+    rs, re = violations(mech, T, P, Y, J, Jr)
+    assert rs <= 1.0 and re <= 1.0, (rs, re)
+
+
 @pytest.mark.parametrize("cfg_name,N", [("mid_1m", 1 << 15), ("large_256k", 1 << 13)])
 def test_bench_size_properties_and_sampled_parity(ck, cfg_name, N):
     """At the size bench.py --jacobian times: Euler's relation sum_l Y_l J_il = 0 and mass
