@@ -115,3 +115,33 @@ def test_jacobian_does_not_depend_on_normalisation_scaling():
     sc = column_scale(J1)
     assert (np.abs(J2[:, :, :S] * 2.5 - J1[:, :, :S]) <= 1e-11 * sc[:, :, :S]).all()
     assert (np.abs(J2[:, :, S] - J1[:, :, S]) <= 1e-11 * sc[:, :, S]).all()
+
+
+def test_finite_differences_with_catalyst_real_nu_irreversible_and_lindemann():
+    """The branches the generated mechanisms do not reach: a species on both sides of a reaction,
+    a real-valued stoichiometric coefficient (pow), irreversible reactions, Lindemann falloff and
+    the 3-parameter Troe form."""
+    import dataclasses
+    cfg = ckgen.CONFIGS["tiny_1k"]
+    mech = ckgen.mechanism(cfg.mech)
+    nu_r, nu_p = mech.nu_reac.copy(), mech.nu_prod.copy()
+    free = int(np.flatnonzero((nu_r[:, 0] == 0) & (nu_p[:, 0] == 0))[0])
+    nu_r[free, 0] += 1.0
+    nu_p[free, 0] += 1.0
+    k = int(np.flatnonzero(nu_r[:, 1])[0])
+    nu_r[k, 1] = 1.5
+    rev = mech.reversible.copy()
+    rev[::3] = 0
+    typ = mech.rxn_type.copy()
+    troe = mech.troe.copy()
+    fo = np.flatnonzero(typ == 3)
+    typ[fo[0]] = 2
+    troe[fo[1:], 3] = np.inf
+    mech = dataclasses.replace(mech, nu_reac=nu_r, nu_prod=nu_p, reversible=rev, rxn_type=typ, troe=troe)
+    T, P, Y = ckgen.states(cfg, N=16)
+    Y = np.maximum(Y, 2e-3)
+    Y /= Y.sum(0)
+    om = oracle.OracleMechanism(mech)
+    J = oracle.jacobian(om, T, P, Y)
+    err = np.abs(J - fd_jacobian(om, T, P, Y)) / column_scale(J)
+    assert err.max() < 2e-6, err.max()
