@@ -29,9 +29,10 @@ def energy_condition_number(mech, T, wdot_ref, h_RT):
     return np.abs(hw).sum(0) / np.maximum(np.abs(hw.sum(0)), 1e-300)
 
 
-def paper_matrix_form(mech, T, P, Y):
+def paper_matrix_form(mech, T, P, Y, return_log_rates=False):
     """Literal numpy evaluation of the paper's ANN-form equations, dense matrices,
-    batch dimension leading.  Returns (Omega[N,S], dTdt[N]).
+    batch dimension leading.  Returns (Omega[N,S], dTdt[N]); with
+    return_log_rates the arguments of Eq. 4's two exps instead: (ln Q_f[N,R], ln Q_r[N,R]).
 
     Eq. 6    log Kf = X_f W_f + B_f
     Eq. 10  G = X_G W_G + B_G, alpha from NASA-7 by range
@@ -99,6 +100,8 @@ def paper_matrix_form(mech, T, P, Y):
         logKf = np.where(fo[None, :], logKf + np.log(Pr / (1 + Pr)) + logF, logKf)
     logKr = logKf - logKc                                # Eq. 7 in log space
 
+    if return_log_rates:
+        return logC @ nu1 + logKf, logC @ nu2 + logKr
     # Eq. 4 and Eq. 2
     Qf = np.exp(logC @ nu1 + logKf)
     Qr = np.exp(logC @ nu2 + logKr) * mech.reversible[None, :]

@@ -61,6 +61,23 @@ def test_states_distribution_layout_and_determinism():
     assert np.allclose(Y.sum(0), 1.0, atol=1e-14) and Y.min() >= 0.99e-20
 
 
+@pytest.mark.parametrize("cfg_name", ["tiny_1k", "tiny_1m", "mid_1m", "large_256k", "mid_rk4"])
+def test_log_rates_stay_inside_fp64_exp_range(cfg_name):
+    """SURVEY.md section 8(c) tolerance notes / 8(d) NASA-7 bullet: the generator must keep
+    max |ln q| < 650 (fp64 exp overflows at 709.8) on the configs' own states, or Eq. 4's exp
+    activations would overflow in any implementation.  4096 states per config,
+    the arguments of the two exps from the matrix-form restatement in tests/helpers.py."""
+    from helpers import paper_matrix_form
+    cfg = ckgen.CONFIGS[cfg_name]
+    mech = ckgen.mechanism(cfg.mech)
+    T, P, Y = ckgen.states(cfg, N=4096)
+    lqf, lqr = paper_matrix_form(mech, T, P, Y, return_log_rates=True)
+    assert np.isfinite(lqf).all() and np.isfinite(lqr).all()
+    worst = max(np.abs(lqf).max(), np.abs(lqr).max())
+    print("%s: ln q_f in [%.1f, %.1f], ln q_r in [%.1f, %.1f]" % (cfg_name, lqf.min(), lqf.max(), lqr.min(), lqr.max()))
+    assert worst < 650.0, worst
+
+
 def test_config_table_matches_baseline_json():
     c = ckgen.CONFIGS
     assert (c["tiny_1k"].mech.S, c["tiny_1k"].mech.R, c["tiny_1k"].N) == (9, 21, 1024)

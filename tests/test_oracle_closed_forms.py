@@ -154,6 +154,70 @@ def test_troe_limits():
     assert abs(det["kf"][0] - kinf * Pr / (1 + Pr) * F) < 1e-13 * kinf
 
 
+@pytest.mark.parametrize("name,k0", [("ex4_troe_low_pressure", 7.25e-4), ("ex4_troe_high_pressure", 7.25e20)])
+def test_troe_pressure_limits_with_F_active(name, k0):
+    """Troe falloff twelve decades into either pressure limit (Pr = 1e-12, 1e+12), F != 1 in both
+    (PAPER.md:159 gives no formula; the textbook form at 50 digits, closed_forms.json).  The low
+    limit is k = k0 M F to 1e-12, the high one k = k_inf F to 1e-12."""
+    g = GOLD[name]
+    mech = two_species_mech(**{**CASES["ex4_troe"], "k0": k0})
+    det = oracle.cell_detail(oracle.OracleMechanism(mech), 1000.0, 101325.0, np.array([0.75, 0.25]))
+    rel = lambda a, b: abs(a - b) / abs(b)
+    assert rel(det["kf"][0], float(g["kf"])) < 1e-13
+    assert rel(det["Q"][0], float(g["q"])) < 1e-12
+    assert rel(det["dTdt"], float(g["dTdt"])) < 1e-12
+    F, Pr, kinf, M = float(g["F"]), float(g["Pr"]), float(g["k_inf"]), float(g["M"])
+    assert abs(F - 1.0) > 5e-4                                   # the factor is active
+    if Pr < 1:
+        assert rel(det["kf"][0], k0 * M * F) < 2e-12             # Pr/(1+Pr) -> Pr
+    else:
+        assert rel(det["kf"][0], kinf * F) < 2e-12               # Pr/(1+Pr) -> 1
+
+
+def nasa7_mech():
+    """Ex5 of tests/golden/make_closed_forms.py: A + 2 B <=> C, full NASA-7 sets (typed here
+    as floats from the same table; the golden file holds the 50-digit results, not the inputs)."""
+    lo = np.array([[3.2, 1.1e-3, -2.4e-6, 3.1e-9, -1.2e-12, -950.0, 0.7],
+                   [2.9, 2.4e-3, -4.1e-6, 2.2e-9, -0.7e-12, 29100.0, 4.9],
+                   [4.3, -0.6e-3, 8.8e-6, -9.1e-9, 3.2e-12, -17800.0, 3.4]])
+    hi = np.array([[3.0, 0.8e-3, -0.11e-6, 0.02e-9, -0.002e-12, -830.0, -1.1],
+                   [2.6, -0.03e-3, 0.05e-6, -0.01e-9, 0.001e-12, 29200.0, 4.8],
+                   [4.6, 4.1e-3, -1.3e-6, 0.21e-9, -0.012e-12, -18000.0, 0.6]])
+    S, R = 3, 1
+    return ckgen.Mechanism(
+        elements=("X",), elem_count=np.array([[2], [16], [34]]), mol_weight=np.array([2.0, 16.0, 34.0]),
+        nu_reac=np.array([[1.0], [2.0], [0.0]]), nu_prod=np.array([[0.0], [0.0], [1.0]]),
+        ln_A=np.array([math.log(3e11)]), b=np.array([-0.7]), Ea_over_R=np.array([6500.0]),
+        reversible=np.ones(R, np.uint8), nasa_lo=lo, nasa_hi=hi, T_mid=np.full(S, 1000.0),
+        rxn_type=np.zeros(R, np.uint8), eff=np.ones((S, R)), ln_A0=np.zeros(R), b0=np.zeros(R),
+        Ea0_over_R=np.zeros(R), troe=np.ones((R, 4)), p_ref=101325.0)
+
+
+@pytest.mark.parametrize("T", [800, 1000, 1600])
+def test_full_nasa7_set_in_both_ranges(T):
+    """Every NASA-7 coefficient non-zero, different sets below and above T_mid (PAPER.md:101-108,
+    Eq. 10): cp/R, h/RT, s/R, g/RT, ln Kc, the rate and dT/dt against the 50-digit evaluation.
+    A wrong divisor of a2..a5 in h or s, a swapped range or a missing a6/T, a7 fails here; T = 1000
+    is exactly T_mid and must take the LOW set (reading Q4)."""
+    g = GOLD["ex5_nasa7_T%d" % T]
+    det = oracle.cell_detail(oracle.OracleMechanism(nasa7_mech()), float(T), 3 * 101325.0,
+                             np.array([0.2, 0.5, 0.3]))
+    rel = lambda a, b: abs(a - b) / max(abs(b), 1e-300)
+    for k in range(3):
+        for key in ("cp_R", "h_RT", "s_R", "g_RT", "C"):
+            assert rel(det[key][k], float(g[key][k])) < 2e-14, (key, k)
+        assert rel(det["wdot"][k], float(g["wdot"][k])) < 1e-12
+    assert abs(math.log(det["Kc"][0]) - float(g["lnKc"])) < 2e-13
+    assert rel(det["kf"][0], float(g["kf"])) < 1e-13
+    assert rel(det["Q"][0], float(g["q"])) < 1e-12
+    assert rel(det["cp_mass"], float(g["cp_mass"])) < 1e-14
+    assert rel(det["dTdt"], float(g["dTdt"])) < 1e-12
+    # the two sets really differ at these states (the test cannot pass with the ranges swapped)
+    other = oracle.cell_detail(oracle.OracleMechanism(nasa7_mech()), float(T) + (400.0 if T <= 1000 else -800.0),
+                               3 * 101325.0, np.array([0.2, 0.5, 0.3]))
+    assert abs(other["cp_R"][2] - det["cp_R"][2]) > 0.05
+
+
 def test_irreversible_has_no_reverse_rate():
     mech = two_species_mech(**CASES["ex1_isomerisation"])
     mech.reversible[:] = 0
