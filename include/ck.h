@@ -126,8 +126,9 @@ int ck_mech_create(const ck_mech_desc *desc, ck_mech **out);
  * `stream`, allocates nothing, synchronises nothing and is deterministic run to run.
  * Inputs are not modified; outputs must not alias inputs.  Calls that share one handle
  * must be ordered on one stream (the handle owns a scratch area).  N == 0 is a
- * successful no-op.  Concentrations are floored at 1e-300 kmol/m^3, so Y_k <= 0 acts as
- * an absent species; T must be finite and > 0, P > 0; inputs are not screened for NaN.
+ * successful no-op.  A mass fraction Y_k <= 0 is an absent species: it enters W_mix, cp, M and
+ * C as 0, and concentrations are then floored at 1e-300 kmol/m^3 for the log form (DESIGN.md
+ * reading Q9); T must be finite and > 0, P > 0; inputs are not screened for NaN.
  * Errors: CK_EINVAL (NULL handle or pointer with N > 0, N < 0), CK_ECUDA. */
 int ck_source_terms(const ck_mech *m, const double *T, const double *P, const double *Y,
                     int64_t N, double *wdot, double *dTdt, void *stream);

@@ -85,7 +85,7 @@ static void ann_log_Kc(const ck_oracle_kc_ann *a, int R, double T, double *xa, d
 
 /* workspace: per-species and per-reaction scratch for one cell */
 typedef struct {
-  double *C, *cp_R, *h_RT, *s_R, *g_RT;          /* [S] */
+  double *C, *cp_R, *h_RT, *s_R, *g_RT, *Y;      /* [S] */
   double *kf, *Kc, *kr, *M, *qf, *qr, *Q, *wdot; /* [R], wdot [S] */
   double *ann_lnKc, *ann_x;                      /* [R], [2 N_H] (approximate ANN only) */
 } cell_ws;
@@ -97,12 +97,16 @@ static void one_cell(const ck_oracle_mech *m, double T, double P, const double *
   const double Ru = CK_ORACLE_RU;
 
   /* 1. concentrations: 1/W_mix = sum Y_k/W_k, rho = P W_mix/(Ru T),
-   *    C_k = rho Y_k / W_k */
+   *    C_k = rho Y_k / W_k.  Reading Q9: a mass fraction <= 0 is an absent species (Y_k = 0)
+   *    everywhere it enters -- W_mix, C, cp -- and C is then floored for the rate law. */
   double inv_Wmix = 0.0;
-  for (int k = 0; k < S; ++k) inv_Wmix += Y[k * ldY] / m->W[k];
+  for (int k = 0; k < S; ++k) {
+    w->Y[k] = Y[k * ldY] > 0.0 ? Y[k * ldY] : 0.0;
+    inv_Wmix += w->Y[k] / m->W[k];
+  }
   double rho = P / (Ru * T * inv_Wmix);
   for (int k = 0; k < S; ++k) {
-    double c = rho * Y[k * ldY] / m->W[k];
+    double c = rho * w->Y[k] / m->W[k];
     w->C[k] = c > CK_ORACLE_C_FLOOR ? c : CK_ORACLE_C_FLOOR;
   }
 
@@ -176,7 +180,7 @@ static void one_cell(const ck_oracle_mech *m, double T, double P, const double *
    *    dT/dt = - sum_k h_k wdot_k / (rho cp),  h_k = (h_k/RT) Ru T  [J/kmol] */
   double cp = 0.0, hw = 0.0;
   for (int k = 0; k < S; ++k) {
-    cp += Y[k * ldY] * w->cp_R[k] * Ru / m->W[k];
+    cp += w->Y[k] * w->cp_R[k] * Ru / m->W[k];
     hw += w->h_RT[k] * Ru * T * w->wdot[k];
   }
   *rho_out = rho;
@@ -185,11 +189,11 @@ static void one_cell(const ck_oracle_mech *m, double T, double P, const double *
 }
 
 static int ws_alloc(cell_ws *w, int S, int R, int NH) {
-  double *p = (double *)malloc(sizeof(double) * (size_t)(6 * S + 8 * R + 2 * NH));
+  double *p = (double *)malloc(sizeof(double) * (size_t)(7 * S + 8 * R + 2 * NH));
   if (!p) return -1;
   w->C = p; w->cp_R = p + S; w->h_RT = p + 2 * S; w->s_R = p + 3 * S; w->g_RT = p + 4 * S;
-  w->wdot = p + 5 * S;
-  double *q = p + 6 * S;
+  w->wdot = p + 5 * S; w->Y = p + 6 * S;
+  double *q = p + 7 * S;
   w->kf = q; w->Kc = q + R; w->kr = q + 2 * R; w->M = q + 3 * R; w->qf = q + 4 * R;
   w->qr = q + 5 * R; w->Q = q + 6 * R; w->ann_lnKc = q + 7 * R; w->ann_x = q + 8 * R;
   return 0;

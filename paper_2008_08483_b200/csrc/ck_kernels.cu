@@ -68,7 +68,8 @@ source_terms_kernel(const DeviceMech m, const double *__restrict__ Tg, const dou
     // ---- (a2, a4) Y/W columns, 1/W_mix, cp of the mixture (NASA-7 cp/R) ---
     double inv_Wmix = 0.0, cp_sum = 0.0;
     for (int k = 0; k < S; ++k) {
-      const double yw = Yg[(size_t)k * N + ii] * ldu(m.inv_W + k);
+      // (a mass fraction <= 0 is an absent species: reading Q9)
+      const double yw = fmax(Yg[(size_t)k * N + ii], 0.0) * ldu(m.inv_W + k);
       col[(size_t)k * nt] = yw;
       inv_Wmix += yw;
       const double *th = m.thermo + (size_t)k * kThermoStride;

@@ -125,34 +125,90 @@ def test_config_parity_all_cells(ck, cfg_name, N):
     assert_parity(ck, mech, T, P, Y, cfg_name)
 
 
+def full_batch_parity(ck, mech, T, P, Y, label, variants=("auto", "generic"), host_chunks=()):
+    """Every cell of a batch against the oracle (which runs once, in chunks of 65536 cells so that
+    its memory stays bounded), for each kernel variant: finiteness, mass and element conservation
+    on the device over all cells, then element by element under the north_star tolerance.
+    host_chunks: also ck_source_terms_host with these CK_HOST_CHUNKS values, against the oracle.
+    Returns the worst (wdot, dT/dt) error / tolerance over all variants."""
+    import os
+    N = T.shape[0]
+    S = mech.n_species
+    dev = torch.device("cuda:0")
+    om = oracle.OracleMechanism(mech)
+    wr = np.empty((S, N))
+    dr = np.empty(N)
+    for c0 in range(0, N, 65536):
+        c1 = min(N, c0 + 65536)
+        wr[:, c0:c1], dr[c0:c1], _ = oracle.source_terms(om, T[c0:c1], P[c0:c1], np.ascontiguousarray(Y[:, c0:c1]))
+    assert np.isfinite(wr).all() and np.isfinite(dr).all()
+    Td, Pd, Yd = (torch.from_numpy(a).to(dev) for a in (T, P, Y))
+    weights = [mech.mol_weight] + [mech.elem_count[:, e].astype(float) for e in range(mech.elem_count.shape[1])]
+    worst_w = worst_t = 0.0
+    saved = os.environ.get("CK_KERNEL")
+    try:
+        for variant in variants:
+            os.environ["CK_KERNEL"] = variant
+            with ck.Mechanism(mech) as gm:
+                assert gm.info("jit") == (1 if variant == "auto" else 0)
+                w = torch.full((S, N), float("nan"), dtype=torch.float64, device=dev)
+                d = torch.full((N,), float("nan"), dtype=torch.float64, device=dev)
+                gm.source_terms(Td, Pd, Yd, w, d, stream=torch.cuda.current_stream().cuda_stream)
+                torch.cuda.synchronize()
+                assert torch.isfinite(w).all() and torch.isfinite(d).all()
+                for wt in weights:
+                    terms = torch.from_numpy(wt).to(dev)[:, None] * w
+                    assert (terms.sum(0).abs() <= 1e-11 * terms.abs().sum(0) + 1e-300).all()
+                    del terms
+                results = [("device", w.cpu().numpy(), d.cpu().numpy())]
+                del w, d
+                for chunks in (host_chunks if variant == "auto" else ()):
+                    os.environ["CK_HOST_CHUNKS"] = str(chunks)
+                    try:
+                        wh, dh = gm.source_terms_host(T, P, Y)
+                    finally:
+                        del os.environ["CK_HOST_CHUNKS"]
+                    results.append(("host, %d chunks" % chunks, wh, dh))
+            for what, wg, dg in results:
+                rw, rt = parity_violations(wg, dg, wr, dr)
+                print("%s [%s, %s]: N=%d all cells, worst wdot err/tol %.3g, worst dT/dt err/tol %.3g"
+                      % (label, variant, what, N, rw, rt))
+                assert rw <= 1.0 and rt <= 1.0, (label, variant, what, rw, rt)
+                worst_w, worst_t = max(worst_w, rw), max(worst_t, rt)
+    finally:
+        if saved is None:
+            os.environ.pop("CK_KERNEL", None)
+        else:
+            os.environ["CK_KERNEL"] = saved
+    return worst_w, worst_t
+
+
 @pytest.mark.parametrize("cfg_name", ["tiny_1m", "mid_1m", "large_256k"])
-def test_full_size_sampled_parity_and_conservation(ck, cfg_name):
-    """BASELINE.json's full sizes in the launch configuration bench.py times: the oracle
-    checks a seeded sample of cells one by one; mass and element conservation (which hold
-    at any size) are checked on every cell on the device."""
+def test_full_size_parity_every_cell(ck, kernel_variant, cfg_name):
+    """BASELINE.json's full sizes (configs 2-4: 2^20, 2^20, 2^18 cells) in the launch
+    configuration bench.py times: EVERY cell against the oracle, both kernel variants, plus the
+    pipelined host entry point with 1, 8 and 16 chunks (north_star: "matching the oracle ... on
+    all five configs"; parity over all N cells of every config)."""
+    if kernel_variant != "auto":
+        pytest.skip("both variants are covered inside the test (the oracle runs once)")
     cfg = ckgen.CONFIGS[cfg_name]
     mech = ckgen.mechanism(cfg.mech)
     T, P, Y = ckgen.states(cfg)
-    N = cfg.N
-    dev = torch.device("cuda:0")
-    gm = ck.Mechanism(mech)
-    Td, Pd, Yd = (torch.from_numpy(a).to(dev) for a in (T, P, Y))
-    w = torch.empty((mech.n_species, N), dtype=torch.float64, device=dev)
-    d = torch.empty((N,), dtype=torch.float64, device=dev)
-    gm.source_terms(Td, Pd, Yd, w, d, stream=torch.cuda.current_stream().cuda_stream)
-    torch.cuda.synchronize()
-    assert torch.isfinite(w).all() and torch.isfinite(d).all()
-    weights = [mech.mol_weight] + [mech.elem_count[:, e].astype(float) for e in range(mech.elem_count.shape[1])]
-    for wt in weights:
-        terms = torch.from_numpy(wt).to(dev)[:, None] * w
-        assert (terms.sum(0).abs() <= 1e-11 * terms.abs().sum(0) + 1e-300).all()
-    rng = np.random.default_rng(12345)
-    idx = np.unique(np.concatenate([rng.integers(0, N, size=1500), [0, 127, 128, N - 129, N - 1]]))
-    wr, dr, _ = oracle.source_terms(oracle.OracleMechanism(mech), T[idx], P[idx],
-                                    np.ascontiguousarray(Y[:, idx]))
-    rw, rt = parity_violations(w[:, idx].cpu().numpy(), d[idx].cpu().numpy(), wr, dr)
-    assert rw <= 1.0 and rt <= 1.0, (rw, rt)
-    gm.close()
+    full_batch_parity(ck, mech, T, P, Y, cfg_name, host_chunks=(1, 8, 16))
+
+
+@pytest.mark.parametrize("N", ckgen.SWEEP_N)
+def test_sweep_sizes_parity_every_cell(ck, kernel_variant, N):
+    """BASELINE.json configs[4], sweep part: N = 2^8, 2^10, ..., 2^22 cells at S=53/R=325 (the
+    sizes bench.py --sweep times): every cell of every size against the
+    oracle.  2^22 cells are 3.66 GB of state in and out, rows past 2^31 bytes."""
+    if kernel_variant != "auto":
+        pytest.skip("specialised kernel (the one the sweep times); the generic one runs at 2^8..2^16")
+    cfg = ckgen.CONFIGS["mid_1m"]
+    mech = ckgen.mechanism(cfg.mech)
+    T, P, Y = ckgen.states(cfg, N=N)
+    full_batch_parity(ck, mech, T, P, Y, "sweep N=2^%d" % (N.bit_length() - 1),
+                      variants=("auto", "generic") if N <= 65536 else ("auto",))
 
 
 # ---------------------------------------------------------------- every reaction on its own
@@ -241,6 +297,22 @@ def test_absent_species_and_tiny_mass_fractions(ck):
     Y[5, 200:] = 1e-300
     Y /= Y.sum(0, keepdims=True)
     assert_parity(ck, mech, T, P, Y, "absent species")
+
+
+def test_negative_mass_fractions(ck):
+    """Y_k <= 0 is an absent species (reading Q9): the small negative mass fractions a caller's own
+    integrator produces enter W_mix, cp, M = C E and C as 0 on the device as in the oracle --
+    three-body and falloff rates would differ if M were built from the raw values."""
+    for cfg_name in ("tiny_1k", "mid_1m"):
+        cfg = ckgen.CONFIGS[cfg_name]
+        mech = ckgen.mechanism(cfg.mech)
+        T, P, Y = ckgen.states(cfg, N=300)
+        Y = Y.copy()
+        rng = np.random.default_rng(5)
+        neg = rng.random(Y.shape) < 0.15
+        Y[neg] = -10.0 ** rng.uniform(-14, -3, size=int(neg.sum()))
+        Y[0, :8] = -0.0
+        assert_parity(ck, mech, T, P, Y, "%s negative Y" % cfg_name)
 
 
 def test_irreversible_lindemann_and_real_valued_nu(ck):

@@ -193,3 +193,22 @@ def test_non_integer_and_absent_species():
     Om, dT = paper_matrix_form(mech2, T, P, Y)
     assert np.isfinite(w).all()
     assert (np.abs(Om.T - w) <= 1e-11 * np.abs(w).max(0)[None, :]).all()
+
+
+def test_non_positive_mass_fractions_are_absent_species():
+    """Reading Q9 (PAPER.md:56 presumes C > 0): Y_k <= 0 is an absent
+    species.  A small negative mass fraction gives exactly what Y_k = 0 gives, in W_mix, M, cp
+    and the rates -- so the result does not depend on the size of the undershoot."""
+    cfg = ckgen.CONFIGS["tiny_1k"]
+    mech = ckgen.mechanism(cfg.mech)
+    om = oracle.OracleMechanism(mech)
+    T, P, Y = ckgen.states(cfg, N=64)
+    Y0, Yn = Y.copy(), Y.copy()
+    Y0[2, :32] = 0.0
+    Yn[2, :32] = -1e-9
+    Y0[6, 16:48] = 0.0
+    Yn[6, 16:48] = -3e-4
+    w0, d0, _ = oracle.source_terms(om, T, P, Y0)
+    wn, dn, _ = oracle.source_terms(om, T, P, Yn)
+    assert np.array_equal(w0, wn) and np.array_equal(d0, dn)
+    assert np.isfinite(w0).all() and np.isfinite(d0).all()
