@@ -31,16 +31,22 @@ METRIC = "cell source-term evals/sec (fp64) at S=53,R=325; fraction of roofline"
 UNIT = "cells/s"
 
 
-def algorithmic_fp64_instr_per_cell(info):
-    """SURVEY.md section 8(d) / DESIGN.md: algorithmic FP64-pipe instructions per cell
-    (FMA, add, mul = 1; exp = 15, log = 28, div = 8 by CUDA 12.9's sm_100a fast paths)."""
+def algorithmic_fp64_instr_per_cell(info, costs=(15, 28, 8)):
+    """SURVEY.md section 8(d) / DESIGN.md section 6: algorithmic FP64-pipe instructions per cell,
+    FMA / add / mul = 1 and (exp, log, div) = `costs`.  The default (15, 28, 8) is the survey's
+    fixed convention (CUDA 12.9's libm fast paths on sm_100a): NORMALISED WORK, which a cheaper
+    hand-written exp does not change.  IMPLEMENTED_COSTS are what this library's own ck_exp /
+    ck_log / ck_rcp execute; with them the figure is the FP64 issue the kernel really needs."""
     S, R = info["S"], info["R"]
     n_fo = info["n_lindemann"] + info["n_troe"]
     n_exp = 2 * R + 5 * info["n_troe"] + info["n_lindemann"]
     n_log = S + 1 + 2 * n_fo
     n_div = 3 + 3 * n_fo
     fma = 20 * S + 2 * (R + n_fo) + info["nnz_reac"] + 2 * info["nnz_net"] + info["nnz_eff"]
-    return fma + 15 * n_exp + 28 * n_log + 8 * n_div
+    return fma + costs[0] * n_exp + costs[1] * n_log + costs[2] * n_div
+
+
+IMPLEMENTED_COSTS = (8, 11, 4)     # ck_exp, ck_log, ck_rcp of csrc/ck_jit_kernel.cuh
 
 
 class ClockSampler:
@@ -112,9 +118,17 @@ def time_oracle(mech, T, P, Y, target_s=12.0):
         oracle.source_terms(om, T[:n], P[:n], Ys)
         passes += 1
     dt = time.perf_counter() - t0
+    # one core, beside the paper's one-MPI-rank CPU baseline: about 4 s of work
+    n1 = int(min(T.shape[0], max(256, rate / max(int(cores), 1) * 4.0)))
+    Y1 = np.ascontiguousarray(Y[:, :n1])
+    t1 = time.perf_counter()
+    oracle.source_terms(om, T[:n1], P[:n1], Y1, nthreads=1)
+    dt1 = time.perf_counter() - t1
     return {"value": passes * n / dt, "unit": UNIT, "cores": int(cores), "kind": "oracle",
             "sample": "first %d cells of the workload x %d passes, %.1f s, OpenMP static over cells"
-                      % (n, passes, dt)}
+                      % (n, passes, dt),
+            "single_core": {"value": n1 / dt1, "unit": UNIT, "cores": 1,
+                            "sample": "first %d cells, one pass, %.1f s, one thread" % (n1, dt1)}}
 
 
 def run_reference(args, cfg, mech):
@@ -123,8 +137,11 @@ def run_reference(args, cfg, mech):
     import oracle
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    n = min(cfg.N, args.ref_cells)
-    T, P, Y = ckgen.states(cfg, N=n)
+    # each step = the whole workload (the same N as the GPU arm) unless --ref-cells bounds it
+    N = args.cells or cfg.N
+    n = min(N, args.ref_cells) if args.ref_cells > 0 else N
+    T, P, Y = ckgen.states(cfg, N=N)
+    T, P, Y = T[:n], P[:n], np.ascontiguousarray(Y[:, :n])
     om = oracle.OracleMechanism(mech)
     cores = 0
     for _ in range(args.warmup):
@@ -134,7 +151,8 @@ def run_reference(args, cfg, mech):
         _, _, cores = oracle.source_terms(om, T, P, Y)
     dt = time.perf_counter() - t0
     value = n * args.steps / dt
-    sample = "each step = first %d cells of the workload (oracle, OpenMP static)" % n
+    sample = "each step = %s (oracle, OpenMP static)" % (
+        "all %d cells of the workload" % n if n == N else "first %d of the workload's %d cells" % (n, N))
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
@@ -293,12 +311,14 @@ def run_ann(args):
         bufs += [torch.empty((S, N), dtype=torch.float64, device=dev), torch.empty(N, dtype=torch.float64, device=dev)]
         with ck.Mechanism(mech) as gm:
             t_exact = timed(gm, bufs)
-        os.environ["CK_JIT_KC"] = "none"
+        os.environ["CK_JIT_KC"] = "none"          # measurement-only ablation, refused by the library
+        os.environ["CK_ALLOW_ABLATION"] = "1"     # unless this is set as well
         try:
             with ck.Mechanism(mech) as gm:
+                assert gm.info("ablation") == 1
                 t_none = timed(gm, bufs)
         finally:
-            del os.environ["CK_JIT_KC"]
+            del os.environ["CK_JIT_KC"], os.environ["CK_ALLOW_ABLATION"]
         rows = []
         for n_layers in (1, 2, 3):
             for n_hidden in (2, 4, 8, 16, 32):
@@ -310,6 +330,34 @@ def run_ann(args):
                              "speedup_kc_layer": (t_exact - t_none) / max(t_ann - t_none, 1e-9)})
         out["mechanisms"].append({"S": S, "R": R, "ms_exact": t_exact, "ms_without_kc_layer": t_none,
                                   "kc_share_of_source_term": (t_exact - t_none) / t_exact, "rows": rows})
+    print(json.dumps(out))
+
+
+def run_peaks(args):
+    """the FP64 microbenchmarks the roofline and the sparse-vs-dense
+    decision rest on (ck_measure_peaks): DFMA rate, DMMA.8x8x4 rate alone and interleaved with
+    DFMA, libm exp / log rates.  One JSON line."""
+    import torch
+    import paper_2008_08483_b200 as ck
+    torch.cuda.set_device(0)
+    stream = torch.cuda.current_stream().cuda_stream
+    with ClockSampler(0) as clocks:
+        p = ck.ck_measure_peaks(stream)
+    mhz = clocks.max_mhz or 1965.0
+    sched = p["sms"] * 4
+    fma = p["dfma_per_s"]
+    out = {"peaks": "FP64 microbenchmarks, each kernel timed alone (CUDA events, best of 5)", **p,
+           "clocks": clocks.summary(),
+           "dfma_tflops": 2 * fma / 1e12,
+           "dfma_nominal_tflops": p["sms"] * 64 * 2 * mhz * 1e6 / 1e12,
+           "dfma_cycles_per_warp_instr_per_scheduler": sched * mhz * 1e6 / (fma / 32),
+           "dmma_tflops": 2 * 256 * p["dmma_per_s"] / 1e12,
+           "dmma_cycles_per_instr_per_scheduler": sched * mhz * 1e6 / p["dmma_per_s"],
+           "dmma_in_dfma_warp_instr": (fma / 32) / p["dmma_per_s"],
+           "interleaved_tflops": 2 * (256 * p["dmma_per_s_interleaved"] + p["dfma_per_s_interleaved"]) / 1e12,
+           "interleaved_cycles_per_group_per_scheduler": sched * mhz * 1e6 / p["dmma_per_s_interleaved"],
+           "libm_exp_cost_in_dfma": fma / p["libm_exp_per_s"],
+           "libm_log_cost_in_dfma": fma / p["libm_log_per_s"]}
     print(json.dumps(out))
 
 
@@ -382,7 +430,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="mid_1m")
     ap.add_argument("--cells", type=int, default=0, help="override cells per GPU")
-    ap.add_argument("--ref-cells", type=int, default=65536, help="cells per step of --impl reference")
+    ap.add_argument("--ref-cells", type=int, default=0,
+                    help="--impl reference: bound the cells per step (default 0 = the whole workload, as the GPU arm)")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="--gpus N > 1: weak = N cells per GPU (default), strong = one batch of N cells sliced over the GPUs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="configs[4]: saturation sweep over N (1 GPU)")
     ap.add_argument("--rk4", action="store_true", help="configs[4]: explicit RK4 reactor run (1 GPU)")
@@ -390,6 +441,7 @@ def main():
     ap.add_argument("--jacobian", action="store_true", help="ck_jacobian throughput and HBM roofline (1 GPU)")
     ap.add_argument("--only", default="", help="--jacobian: only this mechanism's row (tiny_1m, mid_1m, large_256k)")
     ap.add_argument("--ann", action="store_true", help="Fig. 10 analogue: approximate-ANN vs exact log Kc (1 GPU)")
+    ap.add_argument("--peaks", action="store_true", help="FP64 microbenchmarks: DFMA, DMMA.8x8x4, interleave, libm exp/log")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     if args.sweep:
@@ -400,6 +452,8 @@ def main():
         return run_ann(args)
     if args.jacobian:
         return run_jacobian(args)
+    if args.peaks:
+        return run_peaks(args)
 
     import ckgen
     cfg = ckgen.CONFIGS[args.workload]
@@ -410,7 +464,7 @@ def main():
 
     import torch
     import paper_2008_08483_b200 as ck
-    from paper_2008_08483_b200.shard import max_over_ranks
+    from paper_2008_08483_b200.shard import max_over_ranks, rank_cells
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -428,12 +482,19 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    N = args.cells or cfg.N
     S = mech.n_species
-    # each rank owns its own cells (cells are independent): no collective
-    T, P, Y = ckgen.states(cfg, N=N, seed_offset=rank)
+    # each rank owns its own cells (cells are independent): no collective.
+    # weak: N cells per rank, a different seeded batch each; strong: one batch of N cells sliced
+    n_gen, lo, hi, seed_off = rank_cells(args.cells or cfg.N, rank, world, args.scaling)
+    T, P, Y = ckgen.states(cfg, N=n_gen, seed_offset=seed_off)
+    T, P, Y = T[lo:hi], P[lo:hi], np.ascontiguousarray(Y[:, lo:hi])
+    N = hi - lo
+    n_job = n_gen if args.scaling == "strong" else world * N       # cells the whole job evaluates per step
     gm = ck.Mechanism(mech)
     info = {k: gm.info(k) for k in ck.INFO}
+    if not info["jit"] and os.environ.get("CK_KERNEL") != "generic":
+        sys.exit("bench.py: the mechanism-specialised kernel is not in use (%s); refusing to report the "
+                 "generic fallback as the product (set CK_KERNEL=generic to time it on purpose)" % gm.note())
     stream = torch.cuda.current_stream().cuda_stream
     Td, Pd, Yd = (torch.from_numpy(a).to(dev) for a in (T, P, Y))
     w = torch.empty((S, N), dtype=torch.float64, device=dev)
@@ -458,7 +519,7 @@ def main():
     step_ms = [ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps)]
     kernel_ms = float(np.mean(step_ms))          # one kernel launch per step
     total_ms = max_over_ranks(total_ms, dist, dev)
-    value = world * N * args.steps / (total_ms * 1e-3)
+    value = n_job * args.steps / (total_ms * 1e-3)
 
     # ---- end to end through the public host entry point (pinned host buffers) ---------
     Th, Ph, Yh = (torch.from_numpy(a).pin_memory() for a in (T, P, Y))
@@ -473,7 +534,7 @@ def main():
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
     e2e_s = max_over_ranks(e2e_s, dist, dev)
-    e2e_value = world * N * e2e_steps / e2e_s
+    e2e_value = n_job * e2e_steps / e2e_s
     assert np.array_equal(dh.numpy(), d.cpu().numpy()), "host and device entry points disagree"
 
     if rank != 0:
@@ -488,21 +549,35 @@ def main():
     except Exception:
         pass
     i_cell = algorithmic_fp64_instr_per_cell(info)
+    i_cell_impl = algorithmic_fp64_instr_per_cell(info, IMPLEMENTED_COSTS)
     achieved_tflops = 2.0 * i_cell * N / (kernel_ms * 1e-3) / 1e12
     peak_tflops = 2.0 * fp64_fma_per_s / 1e12
     hbm_bytes = 8.0 * (2 * S + 3) * N
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
-    traffic = None
+    ncu = {}
     try:
-        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(cfg.name)
+        ncu = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(cfg.name) or {}
+        if not isinstance(ncu, dict):
+            ncu = {"dram_bytes": ncu}
     except Exception:
         pass
     roofline = {
         "bound": "alu", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
-        "frac": achieved_tflops / peak_tflops, "traffic": traffic,
+        "frac": achieved_tflops / peak_tflops, "traffic": ncu.get("dram_bytes"),
         "kernel": "ck_source_terms_jit" if info["jit"] else "ck::source_terms_kernel",
         "kernel_ms": kernel_ms,
         "fp64_instr_per_cell": i_cell,
+        "frac_convention": "normalised work: SURVEY 8(d) counts exp/log/div at CUDA libm cost (15/28/8 FP64 "
+                           "instructions); the kernel's own exp/log/rcp take 8/11/4",
+        # the same ratio with the costs the kernel implements: the share of the FP64 pipe's issue rate
+        # the algorithmic work needs -- the number to hold against ncu's pipe-active counter
+        "frac_issue": i_cell_impl * N / (kernel_ms * 1e-3) / fp64_fma_per_s,
+        "fp64_instr_per_cell_implemented_costs": i_cell_impl,
+        # ncu counters of this kernel on this workload (profiles/traffic.json, from the committed
+        # ncu --set full capture; null if that workload was not profiled)
+        "fp64_instr_executed_per_cell": ncu.get("fp64_instr_executed_per_cell"),
+        "pipe_active_pct": ncu.get("pipe_fp64_cycles_active_pct"),
+        "ncu_source": ncu.get("source"),
         "peak_source": "DFMA microbenchmark run by this bench (ck_measure_fp64_peak), x2 flop/FMA; "
                        "nominal 148 SM x 64 lanes x 2 x sm_max_mhz = %.1f TFLOP/s"
                        % (148 * 64 * 2 * (clocks.max_mhz or 1965.0) * 1e6 / 1e12),
@@ -514,7 +589,7 @@ def main():
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "scaling": args.scaling, "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": workload_config(cfg, mech, N),
         "clocks": clocks.summary(),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(8 * (S + 2) * N),

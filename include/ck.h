@@ -111,8 +111,10 @@ typedef struct ck_mech_desc {
  * registers for S <= 103, the most updated ones in registers and the rest in shared memory
  * beyond that), falling back to the generic table-driven kernel if no launch shape fits or
  * NVRTC is unavailable; CK_KERNEL=generic forces the generic kernel,
- * CK_KERNEL=jit makes a failed specialisation an error.  Compiled cubins are cached under
- * $CK_JIT_CACHE (default ~/.cache/ck_jit; empty string disables the cache).
+ * CK_KERNEL=jit makes a failed specialisation an error (in auto mode ck_mech_note() says why
+ * the generic kernel is in use).  Compiled cubins are cached under $CK_JIT_CACHE (default
+ * $HOME/.cache/ck_jit, created 0700; empty string, or no HOME, disables the cache); a cache
+ * file carries its size and hash, and one that does not verify or load is removed and rebuilt.
  * Errors: CK_EINVAL (NULL pointers, S/R < 1, W <= 0, negative or non-finite nu, a reaction
  * without reactants or without products, T_mid <= 0, non-positive Troe temperatures,
  * p_ref <= 0), CK_EUNSUPPORTED (unknown rxn_type; S or R beyond the kernels' limits),
@@ -203,9 +205,17 @@ const char *ck_last_error(void);
  *       S - that many accumulate in shared memory; 0 for the generic kernel),
  *       16 cells per tile of the Jacobian kernel (0 if ck_jacobian is unsupported here),
  *       17 1 if the specialised kernel runs two threads per cell (then 9 counts both, and a
- *       block works on half that many cells).
+ *       block works on half that many cells),
+ *       18 1 if the handle was built as a measurement-only ABLATION whose results are not the
+ *       source term (environment CK_JIT_KC=none together with CK_ALLOW_ABLATION=1: the
+ *       equilibrium layer removed, used by bench.py --ann to cost that layer); 0 otherwise.
  * Returns -1 for a NULL handle or unknown `what`. */
 int64_t ck_mech_info(const ck_mech *m, int what);
+
+/* Why the mechanism-specialised kernel is NOT in use on this handle ("" if it is): the NVRTC or
+ * load error, "no launch shape fits ...", or "CK_KERNEL=generic".  The string lives as long as
+ * the handle.  NULL handle: "". */
+const char *ck_mech_note(const ck_mech *m);
 
 /* The CUDA source of the mechanism-specialised kernel ck_mech_create would compile for
  * `desc` on a B200 (generated reaction list inside the hand-written kernel text of
@@ -219,6 +229,19 @@ int64_t ck_mech_jit_source(const ck_mech_desc *desc, char *buf, int64_t cap);
  * `stream`.  Used as the roofline denominator for this FP64-pipe-bound path.
  * Returns CK_OK and writes *fma_per_s, or CK_ECUDA. */
 int ck_measure_fp64_peak(double *fma_per_s, void *stream);
+
+/* The FP64 microbenchmarks behind the roofline and the sparse-vs-dense design decision
+ * (DESIGN.md section 6), each kernel timed alone with CUDA events on
+ * `stream` (best of 5).  Writes 8 doubles to the HOST array `out`:
+ *   [0] DFMA           thread-level instructions / s (= ck_measure_fp64_peak)
+ *   [1] DMMA.8x8x4     warp-level instructions / s, alone (one = 256 FMA = 8 warp-wide DFMA)
+ *   [2] DMMA.8x8x4     warp-level instructions / s when 4 independent DFMA follow each DMMA
+ *   [3] DFMA           thread-level instructions / s in that same interleaved stream
+ *   [4] exp()  [5] log()   CUDA libm calls / s (thread level): the costs the survey's roofline
+ *                          accounting charges for an exponential / a logarithm
+ *   [6] number of SMs  [7] 0 (reserved)
+ * Returns CK_OK, CK_EINVAL (NULL out) or CK_ECUDA. */
+int ck_measure_peaks(double *out, void *stream);
 
 #ifdef __cplusplus
 }

@@ -22,14 +22,14 @@ from . import _build
 
 __all__ = ["Mechanism", "CkError", "ck_mech_create", "ck_source_terms", "ck_source_terms_host",
            "ck_rk4_integrate", "ck_jacobian",
-           "ck_mech_destroy", "ck_last_error", "ck_mech_info", "ck_measure_fp64_peak",
+           "ck_mech_destroy", "ck_last_error", "ck_mech_info", "ck_mech_note", "ck_measure_fp64_peak", "ck_measure_peaks",
            "ck_mech_jit_source",
            "library_path", "RU", "INFO"]
 
 RU = 8314.46261815324  # J/(kmol K), the constant compiled into the kernels
 INFO = {"S": 0, "R": 1, "nnz_reac": 2, "nnz_prod": 3, "nnz_net": 4, "n_three_body": 5,
         "n_lindemann": 6, "n_troe": 7, "n_ranges": 8, "threads": 9, "blocks_per_sm": 10,
-        "smem_bytes": 11, "launches_per_call": 12, "nnz_eff": 13, "jit": 14, "s_reg": 15, "jac_cells": 16, "pair": 17}
+        "smem_bytes": 11, "launches_per_call": 12, "nnz_eff": 13, "jit": 14, "s_reg": 15, "jac_cells": 16, "pair": 17, "ablation": 18}
 
 _dp = C.POINTER(C.c_double)
 _bp = C.POINTER(C.c_uint8)
@@ -84,10 +84,14 @@ def _load():
     lib.ck_mech_info.argtypes = [C.c_void_p, C.c_int]
     lib.ck_jacobian.restype = C.c_int
     lib.ck_jacobian.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+    lib.ck_mech_note.restype = C.c_char_p
+    lib.ck_mech_note.argtypes = [C.c_void_p]
     lib.ck_mech_jit_source.restype = C.c_int64
     lib.ck_mech_jit_source.argtypes = [C.POINTER(_Desc), C.c_char_p, C.c_int64]
     lib.ck_measure_fp64_peak.restype = C.c_int
     lib.ck_measure_fp64_peak.argtypes = [_dp, C.c_void_p]
+    lib.ck_measure_peaks.restype = C.c_int
+    lib.ck_measure_peaks.argtypes = [_dp, C.c_void_p]
     return lib
 
 
@@ -151,6 +155,10 @@ def ck_mech_info(handle, what) -> int:
     return int(_lib.ck_mech_info(handle, INFO[what] if isinstance(what, str) else int(what)))
 
 
+def ck_mech_note(handle) -> str:
+    return _lib.ck_mech_note(handle).decode()
+
+
 def ck_mech_jit_source(mech, kc_ann=None) -> str:
     """Generated CUDA source of the specialised kernel for `mech` (needs no GPU)."""
     desc, keep = make_desc(mech, kc_ann)
@@ -167,6 +175,15 @@ def ck_measure_fp64_peak(stream=0) -> float:
     out = C.c_double()
     _check(_lib.ck_measure_fp64_peak(C.byref(out), stream or None))
     return out.value
+
+
+def ck_measure_peaks(stream=0) -> dict:
+    """The FP64 microbenchmarks of include/ck.h, by name."""
+    out = (C.c_double * 8)()
+    _check(_lib.ck_measure_peaks(out, stream or None))
+    return {"dfma_per_s": out[0], "dmma_per_s": out[1], "dmma_per_s_interleaved": out[2],
+            "dfma_per_s_interleaved": out[3], "libm_exp_per_s": out[4], "libm_log_per_s": out[5],
+            "sms": int(out[6])}
 
 
 # ---- convenience wrapper -----------------------------------------------------------------
@@ -232,6 +249,10 @@ class Mechanism:
 
     def info(self, what) -> int:
         return ck_mech_info(self.handle, what)
+
+    def note(self) -> str:
+        """Why the specialised kernel is not in use ("" if it is)."""
+        return ck_mech_note(self.handle)
 
     def source_terms(self, T, P, Y, wdot, dTdt, N=None, stream=0) -> None:
         """Device buffers (torch CUDA tensors or addresses); asynchronous on `stream`."""

@@ -12,10 +12,10 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libck.so")
-SOURCES = ["ck_api.cu", "ck_kernels.cu", "ck_jit.cu", "ck_rk4.cu", "ck_jac.cu"]
+SOURCES = ["ck_api.cu", "ck_kernels.cu", "ck_jit.cu", "ck_rk4.cu", "ck_jac.cu", "ck_peaks.cu"]
 HEADERS = ["ck_internal.h", "ck_program.h", "ck_jit_kernel.cuh"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC", "-shared"]
+              "-Xcompiler", "-fPIC"]
 
 
 def _newest_source() -> float:
@@ -39,9 +39,27 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     _embed_jit_source()
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-          ["-o", LIB + ".tmp"] + [os.path.join(CSRC, f) for f in SOURCES] + ["-ldl"]
-    subprocess.run(cmd, check=True, cwd=CSRC)
+    objdir = os.path.join(HERE, "build")
+    os.makedirs(objdir, exist_ok=True)
+    newest_header = max(os.path.getmtime(f) for f in
+                        [os.path.join(CSRC, h) for h in HEADERS + ["ck_jit_source.inc"]] +
+                        [os.path.join(INCLUDE, "ck.h")])
+
+    def compile_one(src):
+        obj = os.path.join(objdir, src.replace(".cu", ".o"))
+        path = os.path.join(CSRC, src)
+        if not force and os.path.exists(obj) and os.path.getmtime(obj) >= max(os.path.getmtime(path), newest_header):
+            return obj
+        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, path]
+        subprocess.run(cmd, check=True, cwd=CSRC)
+        return obj
+
+    # the translation units compile side by side (the Jacobian kernel's templates dominate)
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(max_workers=len(SOURCES)) as pool:
+        objs = list(pool.map(compile_one, SOURCES))
+    subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB + ".tmp"] + objs + ["-ldl"],
+                   check=True, cwd=CSRC)
     os.replace(LIB + ".tmp", LIB)
     return LIB
 

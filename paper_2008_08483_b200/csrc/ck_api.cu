@@ -178,7 +178,12 @@ std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk,
   const int sreg_forced = std::min(S, env_int("CK_JIT_SREG", -1));   // tuning / test knob
   const size_t tab_bytes = (size_t)spec.tab_ranges * R * spec.row * sizeof(double);   // R includes padding
   const int nt_forced = env_int("CK_JIT_NT", 0), b_forced = env_int("CK_JIT_MINB", 0);
-  spec.lut_rep = std::max(1, env_int("CK_JIT_LUTREP", 1));
+  {
+    // copies of the exp table: a power of two in 1..16 (lane l reads copy l & (rep - 1))
+    const int rep = env_int("CK_JIT_LUTREP", 1);
+    spec.lut_rep = 1;
+    while (spec.lut_rep * 2 <= std::min(rep, 16)) spec.lut_rep *= 2;
+  }
   int best_nt = 0, best_b = 0, best_cap = 0, best_sreg = 0;
   bool best_tab = false;
   size_t best_smem = 0;
@@ -264,6 +269,8 @@ std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk,
   if (const char *e = std::getenv("CK_JIT_M")) spec.m_dmma = std::string(e) != "dfma";
   if (const char *e = std::getenv("CK_JIT_SYNC")) spec.sync_every = std::atoi(e);
   if (const char *e = std::getenv("CK_JIT_KCONST")) spec.kconst = std::atoi(e) != 0;
+  // (CK_JIT_KC=none, the ablation that removes the equilibrium layer, changes the RESULT: it is
+  //  honoured only together with CK_ALLOW_ABLATION=1, see setup_jit, and shows in ck_mech_info 18)
   if (const char *e = std::getenv("CK_JIT_KC")) spec.kc_none = std::string(e) == "none";
   *smem_out = best_smem;
   return "";
@@ -625,7 +632,14 @@ int setup_jit(ck_mech *m, ck::JitSpec &spec, const std::string &why, size_t smem
     if (mode == "generic") return fail(CK_EUNSUPPORTED, "kc_ann needs the specialised kernel (CK_KERNEL=generic)");
     mode = "jit";
   }
-  if (mode == "generic") { m->jit_note = "CK_KERNEL=generic"; return CK_OK; }
+  if (spec.kc_none && env_int("CK_ALLOW_ABLATION", 0) != 1)
+    return fail(CK_EINVAL, "CK_JIT_KC=none removes the equilibrium layer (a measurement-only ablation whose "
+                           "results are not the source term); set CK_ALLOW_ABLATION=1 to build it");
+  if (mode == "generic") {
+    if (spec.kc_none) return fail(CK_EINVAL, "CK_JIT_KC=none exists only in the specialised kernel");
+    m->jit_note = "CK_KERNEL=generic";
+    return CK_OK;
+  }
   if (mode != "auto" && mode != "jit") return fail(CK_EINVAL, "CK_KERNEL must be auto, generic or jit");
   const bool required = (mode == "jit");
   auto give_up = [&](const std::string &why) {
@@ -642,9 +656,16 @@ int setup_jit(ck_mech *m, ck::JitSpec &spec, const std::string &why, size_t smem
     }
   }
   std::vector<char> cubin;
-  const std::string err = ck::jit_compile(src, &cubin);
-  if (!err.empty()) return give_up(err);
-  cudaError_t ce = cudaLibraryLoadData(&m->jit_lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
+  cudaError_t ce = cudaSuccess;
+  for (int attempt = 0; attempt < 2; ++attempt) {
+    // second attempt: the cubin came from the on-disk cache and would not load -- compile afresh
+    const std::string err = ck::jit_compile(src, &cubin, /*use_cache=*/attempt == 0);
+    if (!err.empty()) return give_up(err);
+    ce = cudaLibraryLoadData(&m->jit_lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
+    if (ce == cudaSuccess) break;
+    cudaGetLastError();
+    m->jit_lib = nullptr;
+  }
   if (ce != cudaSuccess) return give_up(std::string("cudaLibraryLoadData: ") + cudaGetErrorString(ce));
   ce = cudaLibraryGetKernel(&m->jit_kernel, m->jit_lib, "ck_source_terms_jit");
   if (ce == cudaSuccess)
@@ -1046,9 +1067,12 @@ extern "C" int64_t ck_mech_info(const ck_mech *m, int what) {
     case 15: return m->jit_kernel ? m->jit_s_reg : 0;
     case 16: return m->jac ? ck::jac_cells_per_tile(m->jac) : 0;
     case 17: return (m->jit_kernel && m->jit_spec.pair) ? 1 : 0;
+    case 18: return (m->jit_kernel && m->jit_spec.kc_none) ? 1 : 0;
     default: return -1;
   }
 }
+
+extern "C" const char *ck_mech_note(const ck_mech *m) { return m ? m->jit_note.c_str() : ""; }
 
 extern "C" int64_t ck_mech_jit_source(const ck_mech_desc *d, char *buf, int64_t cap) {
   if (validate(d)) return -1;
@@ -1068,5 +1092,12 @@ extern "C" int ck_measure_fp64_peak(double *fma_per_s, void *stream) {
   if (!fma_per_s) return fail(CK_EINVAL, "fma_per_s is NULL");
   cudaError_t ce = ck::measure_fp64_peak(fma_per_s, (cudaStream_t)stream);
   if (ce != cudaSuccess) return fail_cuda(ce, "ck_measure_fp64_peak");
+  return CK_OK;
+}
+
+extern "C" int ck_measure_peaks(double *out, void *stream) {
+  if (!out) return fail(CK_EINVAL, "out is NULL");
+  cudaError_t ce = ck::measure_peaks(out, (cudaStream_t)stream);
+  if (ce != cudaSuccess) return fail_cuda(ce, "ck_measure_peaks");
   return CK_OK;
 }

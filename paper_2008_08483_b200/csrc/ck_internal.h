@@ -70,7 +70,8 @@ cudaError_t jac_launch(const JacMech *jm, const double *T, const double *P, cons
 
 std::string jit_generate_source(const JitSpec &spec);
 // Compiles to a cubin for sm_100a with NVRTC; returns "" on success, else the error text.
-std::string jit_compile(const std::string &src, std::vector<char> *cubin);
+// use_cache = false: do not read the on-disk cubin cache (it is still refreshed).
+std::string jit_compile(const std::string &src, std::vector<char> *cubin, bool use_cache = true);
 
 }  // namespace ck
 
@@ -133,7 +134,10 @@ cudaError_t launch_rk4_stage(int stage, const ck_mech *m, const double *P, doubl
                              double *Ys, const double *wdot, const double *dTdt, double *accT, double *accY,
                              int64_t N, double dt, cudaStream_t stream);
 
-// DFMA throughput microbenchmark (thread-level FMA instructions per second).
+// DFMA throughput microbenchmark (thread-level FMA instructions per second), ck_peaks.cu.
 cudaError_t measure_fp64_peak(double *fma_per_s, cudaStream_t stream);
+// All FP64 microbenchmarks of ck_peaks.cu; out as documented at ck_measure_peaks in ck.h.
+#define CK_N_PEAKS 8
+cudaError_t measure_peaks(double out[CK_N_PEAKS], cudaStream_t stream);
 
 }  // namespace ck

@@ -91,17 +91,70 @@ uint64_t fnv1a(const std::string &s, uint64_t h) {
   return h;
 }
 
+// Directory of the cubin cache, or "" for no cache: $CK_JIT_CACHE if set ("" disables), else
+// $HOME/.cache/ck_jit; without HOME there is no cache (a predictable path under /tmp could be
+// planted by another user).  Created 0700.
 std::string cache_dir() {
   const char *e = std::getenv("CK_JIT_CACHE");
-  if (e && !*e) return "";            // CK_JIT_CACHE="" disables the cache
+  if (e && !*e) return "";
   std::string d = e ? e : "";
   if (d.empty()) {
     const char *home = std::getenv("HOME");
-    d = std::string(home ? home : "/tmp") + "/.cache/ck_jit";
+    if (!home || !*home) return "";
+    d = std::string(home) + "/.cache/ck_jit";
+    ::mkdir((d.substr(0, d.find_last_of('/'))).c_str(), 0700);
   }
-  ::mkdir((d.substr(0, d.find_last_of('/'))).c_str(), 0755);
-  ::mkdir(d.c_str(), 0755);
+  ::mkdir(d.c_str(), 0700);
   return d;
+}
+
+// Cache file = header {magic, payload bytes, FNV-1a of the payload} + cubin.  A file that does
+// not verify (truncated, corrupt, foreign) is removed and the kernel is compiled again.
+struct CacheHeader {
+  char magic[8];
+  uint64_t size, hash;
+};
+const char kCacheMagic[8] = {'C', 'K', 'J', 'I', 'T', '0', '0', '2'};
+
+uint64_t fnv1a_bytes(const char *p, size_t n) {
+  uint64_t h = 1469598103934665603ull;
+  for (size_t i = 0; i < n; ++i) { h ^= (unsigned char)p[i]; h *= 1099511628211ull; }
+  return h;
+}
+
+bool cache_read(const std::string &path, std::vector<char> *cubin) {
+  std::ifstream in(path, std::ios::binary);
+  if (!in) return false;
+  CacheHeader h;
+  in.read((char *)&h, sizeof h);
+  bool ok = in.gcount() == (std::streamsize)sizeof h && std::memcmp(h.magic, kCacheMagic, 8) == 0 &&
+            h.size > 0 && h.size < (1ull << 30);
+  if (ok) {
+    cubin->resize((size_t)h.size);
+    in.read(cubin->data(), (std::streamsize)h.size);
+    ok = in.gcount() == (std::streamsize)h.size && in.peek() == std::ifstream::traits_type::eof() &&
+         fnv1a_bytes(cubin->data(), cubin->size()) == h.hash;
+  }
+  in.close();
+  if (!ok) {
+    cubin->clear();
+    ::unlink(path.c_str());
+  }
+  return ok;
+}
+
+void cache_write(const std::string &path, const std::vector<char> &cubin) {
+  const std::string tmp = path + ".tmp" + std::to_string((long)getpid());
+  std::ofstream out(tmp, std::ios::binary);
+  CacheHeader h;
+  std::memcpy(h.magic, kCacheMagic, 8);
+  h.size = cubin.size();
+  h.hash = fnv1a_bytes(cubin.data(), cubin.size());
+  out.write((const char *)&h, sizeof h);
+  out.write(cubin.data(), (std::streamsize)cubin.size());
+  out.close();
+  if (out) std::rename(tmp.c_str(), path.c_str());
+  else ::unlink(tmp.c_str());
 }
 
 }  // namespace
@@ -245,7 +298,9 @@ std::string jit_generate_source(const JitSpec &s) {
 }
 
 // Compiles `src` to a cubin for sm_100a.  Returns "" on success, else an error message.
-std::string jit_compile(const std::string &src, std::vector<char> *cubin) {
+// use_cache = false skips the lookup (the caller's retry after a cached cubin failed to load);
+// the freshly compiled cubin still replaces the cache entry.
+std::string jit_compile(const std::string &src, std::vector<char> *cubin, bool use_cache) {
   Nvrtc &n = nvrtc();
   if (!n.ok) return "NVRTC (libnvrtc.so.12) could not be loaded";
   int major = 0, minor = 0;
@@ -257,14 +312,10 @@ std::string jit_compile(const std::string &src, std::vector<char> *cubin) {
   if (!dir.empty()) {
     char name[96];
     const uint64_t h1 = fnv1a(src, 1469598103934665603ull), h2 = fnv1a(src, 0x9E3779B97F4A7C15ull);
-    std::snprintf(name, sizeof name, "/ck_%016llx%016llx_nvrtc%d_%d.cubin", (unsigned long long)h1,
+    std::snprintf(name, sizeof name, "/ck_%016llx%016llx_nvrtc%d_%d.ckbin", (unsigned long long)h1,
                   (unsigned long long)h2, major, minor);
     path = dir + name;
-    std::ifstream in(path, std::ios::binary);
-    if (in) {
-      cubin->assign(std::istreambuf_iterator<char>(in), std::istreambuf_iterator<char>());
-      if (!cubin->empty()) return "";
-    }
+    if (use_cache && cache_read(path, cubin)) return "";
   }
 
   nvrtcProgram prog;
@@ -288,13 +339,7 @@ std::string jit_compile(const std::string &src, std::vector<char> *cubin) {
   }
   n.DestroyProgram(&prog);
   if (rc != NVRTC_SUCCESS) return std::string("nvrtcGetCUBIN: ") + n.GetErrorString(rc);
-  if (!path.empty()) {
-    const std::string tmp = path + ".tmp" + std::to_string((long)getpid());
-    std::ofstream out(tmp, std::ios::binary);
-    out.write(cubin->data(), (std::streamsize)cubin->size());
-    out.close();
-    if (out) std::rename(tmp.c_str(), path.c_str());
-  }
+  if (!path.empty()) cache_write(path, *cubin);
   return "";
 }
 

@@ -159,22 +159,6 @@ source_terms_kernel(const DeviceMech m, const double *__restrict__ Tg, const dou
   }
 }
 
-// ---------------------------------------------------------------------------------------
-// FP64 FMA throughput: 8 independent register chains per thread, 1024 threads per block
-__global__ void __launch_bounds__(1024) dfma_peak_kernel(double *out, int iters, double a, double b) {
-  double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5,
-         x6 = x0 + 6, x7 = x0 + 7;
-  for (int i = 0; i < iters; ++i) {
-#pragma unroll
-    for (int u = 0; u < 8; ++u) {
-      x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
-      x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
-    }
-  }
-  const double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
-  if (s == 123.456) out[0] = s;   // never true for the arguments used; keeps the loop alive
-}
-
 }  // namespace
 
 cudaError_t kernel_configure(int threads, size_t smem_bytes, int *blocks_per_sm) {
@@ -198,42 +182,6 @@ cudaError_t launch_source_terms(const ck_mech *m, const double *T, const double 
   const int grid = (int)(n_tiles < m->grid_max ? n_tiles : m->grid_max);
   source_terms_kernel<<<grid, nt, m->smem_bytes, stream>>>(m->dev, T, P, Y, N, wdot, dTdt);
   return cudaGetLastError();
-}
-
-cudaError_t measure_fp64_peak(double *fma_per_s, cudaStream_t stream) {
-  int dev = 0, sms = 0;
-  cudaError_t e = cudaGetDevice(&dev);
-  if (e != cudaSuccess) return e;
-  e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  if (e != cudaSuccess) return e;
-  double *d_out = nullptr;
-  e = cudaMalloc((void **)&d_out, sizeof(double));
-  if (e != cudaSuccess) return e;
-  cudaEvent_t t0, t1;
-  cudaEventCreate(&t0);
-  cudaEventCreate(&t1);
-  const int blocks = sms * 2, threads = 1024, iters = 4096;
-  dfma_peak_kernel<<<blocks, threads, 0, stream>>>(d_out, 64, 0.999999, 1e-7);   // warm-up
-  double best_ms = 1e30;
-  for (int rep = 0; rep < 5; ++rep) {
-    cudaEventRecord(t0, stream);
-    dfma_peak_kernel<<<blocks, threads, 0, stream>>>(d_out, iters, 0.999999, 1e-7);
-    cudaEventRecord(t1, stream);
-    e = cudaEventSynchronize(t1);
-    if (e != cudaSuccess) break;
-    float ms = 0;
-    cudaEventElapsedTime(&ms, t0, t1);
-    if (ms < best_ms) best_ms = ms;
-  }
-  cudaEventDestroy(t0);
-  cudaEventDestroy(t1);
-  cudaFree(d_out);
-  if (e != cudaSuccess) return e;
-  e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
-  const double fmas = (double)blocks * threads * (double)iters * 64.0;
-  *fma_per_s = fmas / (best_ms * 1e-3);
-  return cudaSuccess;
 }
 
 }  // namespace ck

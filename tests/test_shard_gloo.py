@@ -10,7 +10,7 @@ import pytest
 
 import ckgen
 import oracle
-from paper_2008_08483_b200.shard import cell_slice, max_over_ranks
+from paper_2008_08483_b200.shard import cell_slice, max_over_ranks, rank_cells
 
 torch = pytest.importorskip("torch")
 
@@ -27,6 +27,31 @@ def test_cell_slices_partition_the_batch():
         cell_slice(10, 2, 2)
 
 
+def _rank_batch(cfg, n, rank, world, scaling):
+    """The batch bench.py --gpus N gives a rank (same three lines as there)."""
+    n_gen, lo, hi, off = rank_cells(n, rank, world, scaling)
+    T, P, Y = ckgen.states(cfg, N=n_gen, seed_offset=off)
+    return T[lo:hi], P[lo:hi], np.ascontiguousarray(Y[:, lo:hi])
+
+
+def test_weak_batches_differ_and_strong_slices_tile_one_batch():
+    cfg = ckgen.CONFIGS["tiny_1k"]
+    n, world = 1001, 3
+    weak = [_rank_batch(cfg, n, r, world, "weak") for r in range(world)]
+    assert all(b[0].shape == (n,) and b[2].shape == (cfg.mech.S, n) for b in weak)
+    for r in range(1, world):                       # rank-local seeded batches are different cells
+        assert not np.array_equal(weak[0][0], weak[r][0]) and not np.array_equal(weak[0][2], weak[r][2])
+    T, P, Y = ckgen.states(cfg, N=n)
+    assert np.array_equal(weak[0][0], T)            # rank 0 of a weak run is the 1-GPU workload
+    strong = [_rank_batch(cfg, n, r, world, "strong") for r in range(world)]
+    assert np.array_equal(np.concatenate([b[0] for b in strong]), T)
+    assert np.array_equal(np.concatenate([b[1] for b in strong]), P)
+    assert np.array_equal(np.concatenate([b[2] for b in strong], axis=1), Y)
+    assert sum(b[0].shape[0] for b in strong) == n
+    with pytest.raises(ValueError):
+        rank_cells(n, 0, world, "diagonal")
+
+
 def _free_port():
     with socket.socket() as s:
         s.bind(("127.0.0.1", 0))
@@ -40,8 +65,9 @@ def _worker(rank, world, port, n_total, out_dir):
     try:
         cfg = ckgen.CONFIGS["tiny_1k"]
         mech = ckgen.mechanism(cfg.mech)
-        T, P, Y = ckgen.states(cfg, N=n_total)
-        lo, hi = cell_slice(n_total, rank, world)
+        n_gen, lo, hi, off = rank_cells(n_total, rank, world, "strong")
+        assert (lo, hi) == cell_slice(n_total, rank, world)
+        T, P, Y = ckgen.states(cfg, N=n_gen, seed_offset=off)
         w, d, _ = oracle.source_terms(oracle.OracleMechanism(mech), T[lo:hi], P[lo:hi],
                                       np.ascontiguousarray(Y[:, lo:hi]), nthreads=1)
         np.savez(os.path.join(out_dir, "rank%d.npz" % rank), w=w, d=d, lo=lo, hi=hi)
