@@ -576,7 +576,11 @@ def main():
         # ncu counters of this kernel on this workload (profiles/traffic.json, from the committed
         # ncu --set full capture; null if that workload was not profiled)
         "fp64_instr_executed_per_cell": ncu.get("fp64_instr_executed_per_cell"),
-        "pipe_active_pct": ncu.get("pipe_fp64_cycles_active_pct"),
+        # FP64 datapath busy = FP64-pipe counter + DMMA sub-pipe counter (they do not overlap and the
+        # first does not see DMMA: profiles/r02_peaks.md)
+        "pipe_active_pct": ncu.get("fp64_datapath_busy_pct"),
+        "pipe_fp64_pct": ncu.get("pipe_fp64_cycles_active_pct"),
+        "pipe_dmma_pct": ncu.get("pipe_dmma_active_pct"),
         "ncu_source": ncu.get("source"),
         "peak_source": "DFMA microbenchmark run by this bench (ck_measure_fp64_peak), x2 flop/FMA; "
                        "nominal 148 SM x 64 lanes x 2 x sm_max_mhz = %.1f TFLOP/s"
