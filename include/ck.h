@@ -126,8 +126,9 @@ int ck_mech_create(const ck_mech_desc *desc, ck_mech **out);
  *   wdot[S][N] kmol/m^3/s (Eq. 2), dTdt[N] K/s.
  * `stream` is a cudaStream_t (NULL = default stream).  The call is asynchronous on
  * `stream`, allocates nothing, synchronises nothing and is deterministic run to run.
- * Inputs are not modified; outputs must not alias inputs.  Calls that share one handle
- * must be ordered on one stream (the handle owns a scratch area).  N == 0 is a
+ * Inputs are not modified; outputs must not alias inputs.  Re-entrant: calls that share one
+ * handle may run at the same time on different streams (and from different host threads) as
+ * long as their output buffers are distinct.  N == 0 is a
  * successful no-op.  A mass fraction Y_k <= 0 is an absent species: it enters W_mix, cp, M and
  * C as 0, and concentrations are then floored at 1e-300 kmol/m^3 for the log form (DESIGN.md
  * reading Q9); T must be finite and > 0, P > 0; inputs are not screened for NaN.
@@ -143,7 +144,8 @@ int ck_source_terms(const ck_mech *m, const double *T, const double *P, const do
  * after everything queued on `stream` at the call and `stream` ends after the last copy
  * (environment CK_HOST_CHUNKS=n overrides the chunk count, 1 = everything on `stream`).
  * Pinned host memory makes the copies asynchronous; pageable memory also works.
- * Device staging buffers are owned by the handle and grow on demand. */
+ * Device staging buffers, the two copy streams and their events are owned by the handle and grow
+ * on demand: unlike ck_source_terms, calls of this function on ONE handle must not overlap. */
 int ck_source_terms_host(ck_mech *m, const double *T, const double *P, const double *Y,
                          int64_t N, double *wdot, double *dTdt, void *stream);
 
@@ -163,7 +165,8 @@ int ck_source_terms_host(ck_mech *m, const double *T, const double *P, const dou
  * use_graph != 0: the step is captured once into a CUDA graph (re-captured when T, P, Y, N or
  * dt change) and replayed n_steps times; use_graph == 0: plain launches.  Asynchronous on
  * `stream`; the workspace ((3S+3) N doubles) is owned by the handle and grows on demand
- * (that allocation synchronises).  N == 0 or n_steps == 0 is a successful no-op.
+ * (that allocation synchronises), so calls on ONE handle must not overlap.  N == 0 or
+ * n_steps == 0 is a successful no-op.
  * Errors: CK_EINVAL (NULL handle/pointer, negative sizes, dt <= 0), CK_ENOMEM, CK_ECUDA. */
 int ck_rk4_integrate(ck_mech *m, double *T, const double *P, double *Y, int64_t N, double dt,
                      int64_t n_steps, int use_graph, void *stream);

@@ -267,6 +267,7 @@ std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk,
   spec.threads = best_nt; spec.min_blocks = best_b; spec.tab_in_smem = best_tab; spec.s_reg = best_sreg;
   // tuning knobs for A/B runs under ncu (defaults are the measured best)
   if (const char *e = std::getenv("CK_JIT_M")) spec.m_dmma = std::string(e) != "dfma";
+  if (const char *e = std::getenv("CK_JIT_MHINT")) spec.m_hint = std::atoi(e) != 0;
   if (const char *e = std::getenv("CK_JIT_SYNC")) spec.sync_every = std::atoi(e);
   if (const char *e = std::getenv("CK_JIT_KCONST")) spec.kconst = std::atoi(e) != 0;
   // (CK_JIT_KC=none, the ablation that removes the equilibrium layer, changes the RESULT: it is
@@ -624,7 +625,17 @@ void build_host(const ck_mech_desc *d, HostBuild *hb, size_t smem_sm = kSmemPerS
 // Decides whether to use the specialised kernel (env CK_KERNEL = auto | generic | jit),
 // compiles and loads it.  Returns CK_OK also when it falls back to the generic kernel in
 // auto mode (m->jit_note says why).
-int setup_jit(ck_mech *m, ck::JitSpec &spec, const std::string &why, size_t smem) {
+// M scratch of the kernel in use: n_slots slots of slot_elems doubles + the slot flags (zeroed)
+int alloc_scratch(ck_mech *m, int n_slots, size_t slot_elems) {
+  cudaError_t ce = cudaMalloc((void **)&m->d_scratch, (size_t)n_slots * slot_elems * sizeof(double));
+  if (ce == cudaSuccess) ce = cudaMalloc((void **)&m->d_slot_busy, (size_t)n_slots * sizeof(int));
+  if (ce != cudaSuccess) return fail(CK_ENOMEM, std::string("cudaMalloc M scratch: ") + cudaGetErrorString(ce));
+  ce = cudaMemset(m->d_slot_busy, 0, (size_t)n_slots * sizeof(int));
+  if (ce != cudaSuccess) return fail_cuda(ce, "cudaMemset slot flags");
+  return CK_OK;
+}
+
+int setup_jit(ck_mech *m, ck::JitSpec &spec, const std::string &why, size_t smem, size_t smem_sm) {
   const char *mode_env = std::getenv("CK_KERNEL");
   std::string mode = mode_env ? mode_env : "auto";
   if (spec.kc_ann) {
@@ -680,10 +691,13 @@ int setup_jit(ck_mech *m, ck::JitSpec &spec, const std::string &why, size_t smem
   m->jit_cells = spec.pair ? spec.threads / 2 : spec.threads;
   m->jit_spec = spec;
   m->jit_grid_max = m->num_sms * spec.min_blocks;
-  const size_t elems = (size_t)m->jit_grid_max * std::max(spec.n_mb, 1) * ck::kMBlock * spec.threads;
-  ce = cudaMalloc((void **)&m->d_jit_scratch, elems * sizeof(double));
-  if (ce != cudaSuccess) return fail(CK_ENOMEM, std::string("cudaMalloc scratch: ") + cudaGetErrorString(ce));
-  m->jit_params.m_scratch = m->d_jit_scratch;
+  // M = C E scratch in slots (ck_jit_kernel.cuh): one per block that can be resident on the device.
+  // Shared memory bounds the resident blocks per SM from above (registers can only lower it).
+  const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(std::min<size_t>(32, 2048 / spec.threads), smem_sm / (smem + 1024)));
+  if (int st = alloc_scratch(m, m->num_sms * per_sm, (size_t)std::max(spec.n_mb, 1) * ck::kMBlock * m->jit_cells)) return st;
+  m->jit_params.m_scratch = m->d_scratch;
+  m->jit_params.slot_busy = m->d_slot_busy;
+  m->jit_params.n_slots = m->num_sms * per_sm;
   return CK_OK;
 }
 
@@ -711,7 +725,7 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   size_t best_smem = 0;
   for (int threads : {128, 64, 32}) {
     size_t smem = (size_t)2 * S * threads * sizeof(double);
-    if (smem > (size_t)prop.sharedMemPerBlockOptin) continue;
+    if (smem + 64 > (size_t)prop.sharedMemPerBlockOptin) continue;   // (+ the kernel's static shared memory)
     int bps = 0;
     ce = ck::kernel_configure(threads, smem, &bps);
     if (ce != cudaSuccess) { delete m; return fail_cuda(ce, "kernel_configure"); }
@@ -756,10 +770,6 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   if (ce != cudaSuccess) { delete m; return fail(CK_ENOMEM, std::string("cudaMalloc tables: ") + cudaGetErrorString(ce)); }
   ce = cudaMemcpy(m->d_tables, pk.bytes.data(), pk.bytes.size(), cudaMemcpyHostToDevice);
   if (ce != cudaSuccess) { ck_mech_destroy(m); return fail_cuda(ce, "cudaMemcpy tables"); }
-  const size_t scratch_elems = (size_t)m->grid_max * std::max(n_mb, 1) * ck::kMBlock * best_threads;
-  ce = cudaMalloc((void **)&m->d_scratch, scratch_elems * sizeof(double));
-  if (ce != cudaSuccess) { ck_mech_destroy(m); return fail(CK_ENOMEM, std::string("cudaMalloc scratch: ") + cudaGetErrorString(ce)); }
-
   unsigned char *base = (unsigned char *)m->d_tables;
   ck::DeviceMech &dm = m->dev;
   dm.S = S; dm.R = R; dm.n_ranges = n_ranges; dm.n_m = n_m; dm.n_m_blocks = n_mb;
@@ -770,7 +780,6 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   dm.eff = (const double *)(base + o_eff);
   dm.falloff = (const double *)(base + o_fo);
   dm.program = base + o_prog;
-  dm.m_scratch = m->d_scratch;
 
   // ---- mechanism-specialised kernel (ck_jit.cu); the generic kernel stays as fallback ---
   m->jit_params.eff = (const double *)(base + o_jeff);
@@ -778,7 +787,14 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   m->jit_params.tab = (const double *)(base + o_jtab);
   m->jit_params.thermo = (const double *)(base + o_jthermo);
   m->jit_params.logtab = (const double *)(base + o_jlog);
-  if (int st = setup_jit(m, spec, hb.jit_why, hb.jit_smem)) { ck_mech_destroy(m); return st; }
+  if (int st = setup_jit(m, spec, hb.jit_why, hb.jit_smem, (size_t)prop.sharedMemPerMultiprocessor)) { ck_mech_destroy(m); return st; }
+  if (!m->jit_kernel) {
+    // generic kernel in use: its own M scratch, one slot per resident block
+    if (int st = alloc_scratch(m, m->grid_max, (size_t)std::max(n_mb, 1) * ck::kMBlock * best_threads)) { ck_mech_destroy(m); return st; }
+    dm.m_scratch = m->d_scratch;
+    dm.slot_busy = m->d_slot_busy;
+    dm.n_slots = m->grid_max;
+  }
   m->jit_s_reg = spec.pair ? std::min(2 * spec.s_reg, S) : spec.s_reg;
   // ---- tables of the Jacobian kernel (ck_jac.cu) ------------------------------------------
   {
@@ -793,12 +809,12 @@ extern "C" void ck_mech_destroy(ck_mech *m) {
   if (!m) return;
   if (m->d_tables) cudaFree(m->d_tables);
   if (m->d_scratch) cudaFree(m->d_scratch);
+  if (m->d_slot_busy) cudaFree(m->d_slot_busy);
   ck::jac_destroy(m->jac);
   if (m->d_stage) cudaFree(m->d_stage);
   if (m->host_in) cudaStreamDestroy(m->host_in);
   if (m->host_out) cudaStreamDestroy(m->host_out);
   for (cudaEvent_t e : m->host_ev) if (e) cudaEventDestroy(e);
-  if (m->d_jit_scratch) cudaFree(m->d_jit_scratch);
   if (m->rk4_graph) cudaGraphExecDestroy(m->rk4_graph);
   if (m->rk4_lib) cudaLibraryUnload(m->rk4_lib);
   if (m->d_rk4) cudaFree(m->d_rk4);

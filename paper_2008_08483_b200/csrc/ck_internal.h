@@ -20,6 +20,8 @@ namespace ck {
 struct JitParams {
   const double *eff, *eff_frag, *tab, *thermo, *logtab;
   double *m_scratch;
+  int *slot_busy;
+  int n_slots;
   const double *T, *P, *Y;
   double *wdot, *dTdt;
   long long N;
@@ -41,6 +43,7 @@ struct JitSpec {
   int n_mb = 0;                // blocks of 8 rows of M, padded to an even count
   bool tab_in_smem = true;
   bool m_dmma = true;          // M = C E on DMMA.8x8x4 (else register-tiled DFMA)
+  bool m_hint = true;          // M scratch accesses carry an L2 evict_last policy
   int sync_every = 0;          // block barrier every n reaction blocks (0 = never)
   int block = 4;               // reactions per block of the core
   int s_reg = 0;               // register accumulators per thread (internal species order); rest in smem
@@ -87,7 +90,8 @@ struct ck_mech {
   int n_three_body = 0, n_lindemann = 0, n_troe = 0;
   // one device allocation holding every table; m_scratch separately
   void *d_tables = nullptr;
-  double *d_scratch = nullptr;
+  double *d_scratch = nullptr;    // M = C E scratch of the kernel in use (slots, ck_program.h)
+  int *d_slot_busy = nullptr;
   // mechanism-specialised kernel (NULL kernel => the generic kernel is used)
   cudaLibrary_t jit_lib = nullptr;
   cudaKernel_t jit_kernel = nullptr;
@@ -95,7 +99,6 @@ struct ck_mech {
   int jit_threads = 0, jit_blocks_per_sm = 0, jit_grid_max = 0, jit_s_reg = 0;
   int jit_cells = 0;          // cells per block of the specialised kernel (= threads, or half with pair)
   size_t jit_smem = 0;
-  double *d_jit_scratch = nullptr;
   ck::JitSpec jit_spec;       // kept to compile the RK4 stage variant on first use
   cudaLibrary_t rk4_lib = nullptr;
   cudaKernel_t rk4_kernel = nullptr;

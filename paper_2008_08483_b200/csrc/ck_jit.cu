@@ -165,7 +165,7 @@ std::string jit_generate_source(const JitSpec &s) {
     << "\n#define CK_MINB " << s.min_blocks << "\n#define CK_NRANGES " << s.n_ranges
     << "\n#define CK_NM " << s.n_m << "\n#define CK_NMB " << s.n_mb
     << "\n#define CK_NFO " << s.n_fo << "\n#define CK_TAB_SMEM " << (s.tab_in_smem ? 1 : 0)
-    << "\n#define CK_M_DMMA " << (s.m_dmma ? 1 : 0) << "\n#define CK_KCONST " << (s.kconst ? 1 : 0) << "\n#define CK_SYNC_EVERY " << s.sync_every
+    << "\n#define CK_M_DMMA " << (s.m_dmma ? 1 : 0) << "\n#define CK_M_HINT " << (s.m_hint ? 1 : 0) << "\n#define CK_KCONST " << (s.kconst ? 1 : 0) << "\n#define CK_SYNC_EVERY " << s.sync_every
     << "\n#define CK_B " << s.block << "\n#define CK_NBLK " << (int)s.rxn.size() / s.block
     << "\n#define CK_G_TB0 " << s.group_end[1] << "\n#define CK_G_FO0 " << s.group_end[3]
     << "\n#define CK_TAB_NRANGES " << s.tab_ranges << "\n#define CK_ROW " << s.row

@@ -51,7 +51,15 @@ source_terms_kernel(const DeviceMech m, const double *__restrict__ Tg, const dou
   const int tid = threadIdx.x;
   double *col = smem + tid;              // col[k*nt]
   double *wd = smem + (size_t)S * nt + tid;
-  double *msc = m.m_scratch + (size_t)blockIdx.x * m.n_m_blocks * kMBlock * nt + tid;
+  // a free slot of the M scratch for this block's lifetime (ck_program.h)
+  __shared__ int s_slot;
+  if (tid == 0) {
+    int s = blockIdx.x % m.n_slots;
+    while (atomicCAS(m.slot_busy + s, 0, 1) != 0) s = (s + 1 == m.n_slots) ? 0 : s + 1;
+    s_slot = s;
+  }
+  __syncthreads();
+  double *msc = m.m_scratch + (size_t)s_slot * m.n_m_blocks * kMBlock * nt + tid;
 
   const int64_t n_tiles = (N + nt - 1) / nt;
   for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
@@ -157,6 +165,8 @@ source_terms_kernel(const DeviceMech m, const double *__restrict__ Tg, const dou
     // dT/dt = -sum_k h_k wdot_k / (rho cp), h_k = (h/RT) Ru T, cp = Ru sum_k (Y_k/W_k) cp_k/R
     if (valid) dTdt[i] = -(T * hw) / (rho * cp_sum);
   }
+  __syncthreads();
+  if (tid == 0) atomicExch(m.slot_busy + s_slot, 0);
 }
 
 }  // namespace
@@ -168,7 +178,11 @@ cudaError_t kernel_configure(int threads, size_t smem_bytes, int *blocks_per_sm)
   int optin = 0;
   e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
   if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(source_terms_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+  cudaFuncAttributes attr;
+  e = cudaFuncGetAttributes(&attr, source_terms_kernel);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(source_terms_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           optin - (int)attr.sharedSizeBytes);
   if (e != cudaSuccess) return e;
   return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, source_terms_kernel, threads,
                                                        smem_bytes);

@@ -56,7 +56,12 @@ struct DeviceMech {
   const double *eff;          // [n_m_blocks][S][kMBlock], zero padded
   const double *falloff;      // [n_fo][kFalloffStride]
   const unsigned char *program;  // R records back to back
-  double *m_scratch;          // [grid][n_m_blocks * kMBlock][threads]
+  // M = C E scratch (L2 resident): n_slots slots of [n_m_blocks * kMBlock][threads] doubles.  A block
+  // takes a free slot for its lifetime (slot_busy[s]: 0 free, 1 taken), so launches that overlap on
+  // different streams never share one; n_slots >= the blocks that can be resident on the device.
+  double *m_scratch;
+  int *slot_busy;
+  int32_t n_slots;
 };
 
 }  // namespace ck

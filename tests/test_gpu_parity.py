@@ -441,6 +441,43 @@ def test_host_entry_point_pipelined(ck, monkeypatch, kernel_variant, chunks):
     assert rw <= 1.0 and rt <= 1.0
 
 
+@pytest.mark.parametrize("cfg_name,N", [("mid_1m", 2048), ("mid_1m", 40000), ("tiny_1k", 3000), ("large_256k", 1500)])
+def test_concurrent_calls_on_two_streams_share_one_handle(ck, cfg_name, N):
+    """ck_source_terms is re-entrant for distinct output buffers.  Two
+    streams launch on ONE handle at the same time, over and over, with different inputs and
+    outputs (grids small enough to be resident side by side at the small N); every result must
+    match the oracle and be bitwise what a call alone gives -- the blocks of overlapping launches
+    each take their own slot of the M = C E scratch (third-body and falloff rates would be
+    corrupted otherwise)."""
+    cfg = ckgen.CONFIGS[cfg_name]
+    mech = ckgen.mechanism(cfg.mech)
+    S = mech.n_species
+    dev = torch.device("cuda:0")
+    om = oracle.OracleMechanism(mech)
+    batches = [ckgen.states(cfg, N=N, seed_offset=o) for o in (0, 1)]
+    refs = [oracle.source_terms(om, *b)[:2] for b in batches]
+    with ck.Mechanism(mech) as gm:
+        alone = [gpu_run(ck, mech, *b, gm) for b in batches]
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        bufs = []
+        for b, st in zip(batches, streams):
+            with torch.cuda.stream(st):
+                Td, Pd, Yd = (torch.from_numpy(a).to(dev) for a in b)
+                w = torch.empty((S, N), dtype=torch.float64, device=dev)
+                d = torch.empty((N,), dtype=torch.float64, device=dev)
+            bufs.append((Td, Pd, Yd, w, d))
+        torch.cuda.synchronize()
+        for rep in range(25):
+            for (Td, Pd, Yd, w, d), st in zip(bufs, streams):
+                gm.source_terms(Td, Pd, Yd, w, d, stream=st.cuda_stream)
+        torch.cuda.synchronize()
+        for (Td, Pd, Yd, w, d), (wa, da), (wr, dr) in zip(bufs, alone, refs):
+            wg, dg = w.cpu().numpy(), d.cpu().numpy()
+            assert np.array_equal(wg, wa) and np.array_equal(dg, da)
+            rw, rt = parity_violations(wg, dg, wr, dr)
+            assert rw <= 1.0 and rt <= 1.0, (cfg_name, rw, rt)
+
+
 def test_error_codes(ck):
     mech = ckgen.mechanism(ckgen.MECH_TINY)
     gm = ck.Mechanism(mech)
