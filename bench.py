@@ -361,6 +361,62 @@ def run_peaks(args):
     print(json.dumps(out))
 
 
+def run_precision(args):
+    """the reduced-precision variants of the rate layers
+    (ck_mech_desc.precision) against the fp64 product: time per call at the config's N and error
+    against the fp64 oracle on a sample of the same states -- wdot relative to max_k|wdot_k| per cell,
+    dT/dt relative to the scale of the energy sum -- on the three mechanisms as generated and "tamed"
+    (mild kinetics whose rates fit fp32).  One JSON line."""
+    import torch
+    import ckgen
+    import oracle
+    import paper_2008_08483_b200 as ck
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from helpers import energy_kappa, tame
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    stream = torch.cuda.current_stream().cuda_stream
+    n_err = args.cells or 32768
+    out = {"precision": "ck_source_terms with precision = f64 | mixed | f32_rates: ms per call at the config's N; "
+                        "errors against the fp64 oracle on the first %d cells" % n_err, "rows": []}
+    for name in ("tiny_1m", "mid_1m", "large_256k"):
+        cfg = ckgen.CONFIGS[name]
+        for tamed in (False, True):
+            mech = ckgen.mechanism(cfg.mech)
+            if tamed:
+                mech = tame(mech)
+            S = mech.n_species
+            T, P, Y = ckgen.states(cfg)
+            N = T.shape[0]
+            Td, Pd, Yd = (torch.from_numpy(a).to(dev) for a in (T, P, Y))
+            w = torch.empty((S, N), dtype=torch.float64, device=dev)
+            d = torch.empty(N, dtype=torch.float64, device=dev)
+            Ts, Ps, Ys = T[:n_err], P[:n_err], np.ascontiguousarray(Y[:, :n_err])
+            wr, dr, _ = oracle.source_terms(oracle.OracleMechanism(mech), Ts, Ps, Ys)
+            kap = energy_kappa(mech, Ts, wr)
+            for prec, pname in ((0, "f64"), (1, "mixed"), (2, "f32_rates")):
+                with ck.Mechanism(mech, precision=prec) as gm:
+                    for _ in range(5):
+                        gm.source_terms(Td, Pd, Yd, w, d, stream=stream)
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    torch.cuda.synchronize()
+                    e0.record()
+                    for _ in range(20):
+                        gm.source_terms(Td, Pd, Yd, w, d, stream=stream)
+                    e1.record()
+                    torch.cuda.synchronize()
+                    ms = e0.elapsed_time(e1) / 20
+                wg, dg = w[:, :n_err].cpu().numpy(), d[:n_err].cpu().numpy()
+                e_w = np.abs(wg - wr).max(0) / np.abs(wr).max(0)
+                e_t = np.abs(dg - dr) / (kap * np.abs(dr))
+                out["rows"].append({"mechanism": "S=%d R=%d%s" % (S, mech.n_reactions, " tamed" if tamed else ""),
+                                    "N": N, "precision": pname, "ms": ms, "cells_per_s": N / (ms * 1e-3),
+                                    "wdot_err_rel_max_median": float(np.median(e_w)), "wdot_err_rel_max_worst": float(e_w.max()),
+                                    "dTdt_err_rel_scale_median": float(np.median(e_t)), "dTdt_err_rel_scale_worst": float(e_t.max()),
+                                    "finite": bool(np.isfinite(wg).all() and np.isfinite(dg).all())})
+    print(json.dumps(out))
+
+
 def run_jacobian(args):
     """ck_jacobian, d(wdot, dT/dt)/d(Y, T) for N cells, cell-major
     (S+1)x(S+1) matrices.  HBM-write bound: 8 (S+1)^2 bytes out per cell against 8 (S+2) in.
@@ -441,6 +497,7 @@ def main():
     ap.add_argument("--jacobian", action="store_true", help="ck_jacobian throughput and HBM roofline (1 GPU)")
     ap.add_argument("--only", default="", help="--jacobian: only this mechanism's row (tiny_1m, mid_1m, large_256k)")
     ap.add_argument("--ann", action="store_true", help="Fig. 10 analogue: approximate-ANN vs exact log Kc (1 GPU)")
+    ap.add_argument("--precision", action="store_true", help="reduced-precision variants: time and error against the fp64 oracle")
     ap.add_argument("--peaks", action="store_true", help="FP64 microbenchmarks: DFMA, DMMA.8x8x4, interleave, libm exp/log")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -454,6 +511,8 @@ def main():
         return run_jacobian(args)
     if args.peaks:
         return run_peaks(args)
+    if args.precision:
+        return run_precision(args)
 
     import ckgen
     cfg = ckgen.CONFIGS[args.workload]

@@ -73,6 +73,21 @@ typedef struct ck_kc_ann {
   const double *out_std;  /* [R] */
 } ck_kc_ann;
 
+/* Arithmetic of the rate layers (ck_mech_desc.precision).  CK_PREC_F64 is the product: IEEE fp64
+ * throughout, the north_star tolerance holds.  The others are the reduced-precision variants the
+ * paper names as future work ("single or half-precision environments"; SURVEY.md
+ * section 8(f) item 4); state, results, M = C E and the accumulation of Eq. 2 stay fp64 in all of them:
+ *   CK_PREC_MIXED      the exp activations of Eq. 4 (and of the falloff layer) take their mantissa
+ *                      2^f from the fp32 special-function unit, the exponent is handled in fp64 /
+ *                      integer arithmetic; every rate carries a relative error <= ~6e-7, whatever its
+ *                      magnitude (no overflow: the synthetic configs' rates reach e^250);
+ *   CK_PREC_F32_RATES  additionally ln C, the gathers of Eq. 4 and the Arrhenius / equilibrium
+ *                      layers (Eq. 6, 11) run in fp32: a rate carries an ABSOLUTE error of about
+ *                      1e-7 |ln q| x (terms) in its logarithm, i.e. 1e-5 .. 1e-4 relative.
+ * Both need the mechanism-specialised kernel (CK_EUNSUPPORTED otherwise); measured errors and
+ * times: DESIGN.md section 15, bench.py --precision. */
+enum { CK_PREC_F64 = 0, CK_PREC_MIXED = 1, CK_PREC_F32_RATES = 2 };
+
 /* Mechanism description.  All pointers are HOST pointers; the arrays are copied by
  * ck_mech_create and stay owned by the caller.  S = n_species, R = n_reactions.
  * Matrices are row-major with the species index first: element (k, j) at k*R + j. */
@@ -101,6 +116,8 @@ typedef struct ck_mech_desc {
   const ck_kc_ann *kc_ann;   /* NULL: exact equilibrium layer; else log Kc from this network.
                                 Needs the mechanism-specialised kernel (CK_EUNSUPPORTED if it
                                 cannot be built) */
+  int32_t precision;         /* CK_PREC_F64 (0, the default of a zeroed struct), CK_PREC_MIXED or
+                                CK_PREC_F32_RATES */
 } ck_mech_desc;
 
 /* Validate `desc`, build the device-resident mechanism (sorted reaction program, folded
@@ -211,7 +228,8 @@ const char *ck_last_error(void);
  *       block works on half that many cells),
  *       18 1 if the handle was built as a measurement-only ABLATION whose results are not the
  *       source term (environment CK_JIT_KC=none together with CK_ALLOW_ABLATION=1: the
- *       equilibrium layer removed, used by bench.py --ann to cost that layer); 0 otherwise.
+ *       equilibrium layer removed, used by bench.py --ann to cost that layer); 0 otherwise,
+ *       19 the handle's precision (CK_PREC_*).
  * Returns -1 for a NULL handle or unknown `what`. */
 int64_t ck_mech_info(const ck_mech *m, int what);
 

@@ -24,12 +24,13 @@ __all__ = ["Mechanism", "CkError", "ck_mech_create", "ck_source_terms", "ck_sour
            "ck_rk4_integrate", "ck_jacobian",
            "ck_mech_destroy", "ck_last_error", "ck_mech_info", "ck_mech_note", "ck_measure_fp64_peak", "ck_measure_peaks",
            "ck_mech_jit_source",
-           "library_path", "RU", "INFO"]
+           "library_path", "RU", "INFO", "PREC_F64", "PREC_MIXED", "PREC_F32_RATES"]
 
 RU = 8314.46261815324  # J/(kmol K), the constant compiled into the kernels
 INFO = {"S": 0, "R": 1, "nnz_reac": 2, "nnz_prod": 3, "nnz_net": 4, "n_three_body": 5,
         "n_lindemann": 6, "n_troe": 7, "n_ranges": 8, "threads": 9, "blocks_per_sm": 10,
-        "smem_bytes": 11, "launches_per_call": 12, "nnz_eff": 13, "jit": 14, "s_reg": 15, "jac_cells": 16, "pair": 17, "ablation": 18}
+        "smem_bytes": 11, "launches_per_call": 12, "nnz_eff": 13, "jit": 14, "s_reg": 15, "jac_cells": 16, "pair": 17, "ablation": 18, "precision": 19}
+PREC_F64, PREC_MIXED, PREC_F32_RATES = 0, 1, 2
 
 _dp = C.POINTER(C.c_double)
 _bp = C.POINTER(C.c_uint8)
@@ -49,7 +50,7 @@ class _Desc(C.Structure):
         ("ln_A", _dp), ("b", _dp), ("Ea_over_R", _dp), ("reversible", _bp),
         ("nasa_lo", _dp), ("nasa_hi", _dp), ("T_mid", _dp), ("rxn_type", _bp),
         ("eff", _dp), ("ln_A0", _dp), ("b0", _dp), ("Ea0_over_R", _dp), ("troe", _dp),
-        ("p_ref", C.c_double), ("kc_ann", C.POINTER(_Ann)),
+        ("p_ref", C.c_double), ("kc_ann", C.POINTER(_Ann)), ("precision", C.c_int32),
     ]
 
 
@@ -196,7 +197,7 @@ def _u8(a):
     return np.ascontiguousarray(a, dtype=np.uint8)
 
 
-def make_desc(mech, kc_ann=None):
+def make_desc(mech, kc_ann=None, precision=PREC_F64):
     """ck_mech_desc from any object with ckgen.Mechanism's array attributes (and, optionally,
     a ck_kc_ann from one with ckgen.KcAnn's).  Returns (desc, keepalive) -- keepalive owns the
     host arrays the desc points to."""
@@ -216,6 +217,7 @@ def make_desc(mech, kc_ann=None):
             raise ValueError("%s has shape %s, expected %s" % (name, keep[name].shape, shp))
     d = _Desc()
     d.n_species, d.n_reactions, d.p_ref = S, R, float(mech.p_ref)
+    d.precision = int(precision)
     for name, arr in keep.items():
         setattr(d, name, arr.ctypes.data_as(_bp if arr.dtype == np.uint8 else _dp))
     if kc_ann is not None:
@@ -240,8 +242,8 @@ def make_desc(mech, kc_ann=None):
 class Mechanism:
     """Owns a ck_mech handle created from a mechanism's arrays."""
 
-    def __init__(self, mech, kc_ann=None):
-        desc, keep = make_desc(mech, kc_ann)
+    def __init__(self, mech, kc_ann=None, precision=PREC_F64):
+        desc, keep = make_desc(mech, kc_ann, precision)
         self.handle = ck_mech_create(desc)
         del keep                      # the library copied everything it needs
         self.S = ck_mech_info(self.handle, "S")

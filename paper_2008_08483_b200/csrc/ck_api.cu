@@ -92,6 +92,8 @@ int validate(const ck_mech_desc *d) {
         return fail(CK_EINVAL, "Troe temperatures must be > 0 (T** may be +INF)");
     }
   }
+  if (d->precision < CK_PREC_F64 || d->precision > CK_PREC_F32_RATES)
+    return fail(CK_EINVAL, "precision must be CK_PREC_F64, CK_PREC_MIXED or CK_PREC_F32_RATES");
   if (const ck_kc_ann *a = d->kc_ann) {
     if ((a->n_in != 1 && a->n_in != 6) || a->n_layers < 1 || a->n_layers > 8 || a->n_hidden < 1 ||
         a->n_hidden > 64 || (a->activation != CK_ANN_RELU && a->activation != CK_ANN_ELU))
@@ -176,7 +178,8 @@ std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk,
   const int rest_dflt = !fits ? 166 : (spec.block <= 2 ? 100 : (spec.block == 3 ? 124 : 144));
   const int rest = std::max(48, env_int("CK_JIT_REST", rest_dflt));
   const int sreg_forced = std::min(S, env_int("CK_JIT_SREG", -1));   // tuning / test knob
-  const size_t tab_bytes = (size_t)spec.tab_ranges * R * spec.row * sizeof(double);   // R includes padding
+  const size_t tab_elem = spec.prec == CK_PREC_F32_RATES ? sizeof(float) : sizeof(double);
+  const size_t tab_bytes = (size_t)spec.tab_ranges * R * spec.row * tab_elem;   // R includes padding
   const int nt_forced = env_int("CK_JIT_NT", 0), b_forced = env_int("CK_JIT_MINB", 0);
   {
     // copies of the exp table: a power of two in 1..16 (lane l reads copy l & (rep - 1))
@@ -189,7 +192,7 @@ std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk,
   size_t best_smem = 0;
   auto smem_of = [&](int nt, int s_reg, bool tab_smem) {
     return (size_t)(S + (S - s_reg) + spec.ann_nhp) * (nt + 8) * 8 + (128 * spec.lut_rep + 256) * 8 + (size_t)spec.n_ranges * S * 12 * 8 +
-           (tab_smem ? tab_bytes : (size_t)(nt / 32) * 2 * spec.tab_ranges * spec.block * spec.row * 8) + 16;
+           (tab_smem ? tab_bytes : (size_t)(nt / 32) * 2 * spec.tab_ranges * spec.block * spec.row * tab_elem) + 16;
   };
   const bool all_regs = sreg_forced < 0 ? fits : (sreg_forced == S);
   if (all_regs) {
@@ -250,7 +253,7 @@ std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk,
         const int n_cold = std::max(0, S - 2 * s_reg);
         const size_t smem = (size_t)(S + n_cold) * (cells + 8) * 8 + (128 * spec.lut_rep + 256) * 8 +
                             (size_t)spec.n_ranges * S * 12 * 8 +
-                            (tab_smem ? tab_bytes : (size_t)(nt / 32) * 2 * spec.tab_ranges * spec.block * spec.row * 8) +
+                            (tab_smem ? tab_bytes : (size_t)(nt / 32) * 2 * spec.tab_ranges * spec.block * spec.row * tab_elem) +
                             (size_t)(4 * spec.block + 8) * cells * 8 + 16;
         if (smem > smem_blk || smem + 1024 > smem_sm) continue;
         const bool better = nt > p_nt || (nt == p_nt && (tab_smem != 0) > p_tab);
@@ -463,6 +466,7 @@ void build_host(const ck_mech_desc *d, HostBuild *hb, size_t smem_sm = kSmemPerS
   std::vector<int> m_rows;       // reaction index of each row of M
   ck::JitSpec &spec = hb->spec;
   spec.S = S; spec.R = R; spec.n_ranges = n_ranges;
+  spec.prec = d->precision;
   const ck_kc_ann *ann = d->kc_ann;
   spec.kc_ann = ann != nullptr;
   if (ann) {
@@ -477,7 +481,8 @@ void build_host(const ck_mech_desc *d, HostBuild *hb, size_t smem_sm = kSmemPerS
     spec.ann_const.insert(spec.ann_const.end(), ann->B, ann->B + (size_t)NL * NH);
     spec.ann_const.insert(spec.ann_const.end(), ann->W_hid, ann->W_hid + (size_t)(NL - 1) * NH * NH);
   } else {
-    spec.tab_ranges = n_ranges; spec.row = 10;
+    // (fp32 rate layers: rows of 12 floats, three 16-byte loads)
+    spec.tab_ranges = n_ranges; spec.row = spec.prec == CK_PREC_F32_RATES ? 12 : 10;
   }
   const int ROW = spec.row;
   std::vector<double> &jit_tab = hb->jit_tab;
@@ -643,6 +648,13 @@ int setup_jit(ck_mech *m, ck::JitSpec &spec, const std::string &why, size_t smem
     if (mode == "generic") return fail(CK_EUNSUPPORTED, "kc_ann needs the specialised kernel (CK_KERNEL=generic)");
     mode = "jit";
   }
+  if (spec.prec == CK_PREC_F32_RATES && spec.kc_ann)
+    return fail(CK_EUNSUPPORTED, "CK_PREC_F32_RATES is not combined with the approximate-ANN Kc");
+  if (spec.prec != CK_PREC_F64) {
+    // so do the reduced-precision variants
+    if (mode == "generic") return fail(CK_EUNSUPPORTED, "reduced precision needs the specialised kernel (CK_KERNEL=generic)");
+    mode = "jit";
+  }
   if (spec.kc_none && env_int("CK_ALLOW_ABLATION", 0) != 1)
     return fail(CK_EINVAL, "CK_JIT_KC=none removes the equilibrium layer (a measurement-only ablation whose "
                            "results are not the source term); set CK_ALLOW_ABLATION=1 to build it");
@@ -761,7 +773,10 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   const size_t o_eff = pk.append(eff.data(), eff.size() * sizeof(double));
   const size_t o_fo = pk.append(falloff.data(), falloff.size() * sizeof(double));
   const size_t o_prog = pk.append(program.data(), program.size());
-  const size_t o_jtab = pk.append(jit_tab.data(), jit_tab.size() * sizeof(double));
+  std::vector<float> jit_tab32;
+  if (spec.prec == CK_PREC_F32_RATES) jit_tab32.assign(jit_tab.begin(), jit_tab.end());
+  const size_t o_jtab = jit_tab32.empty() ? pk.append(jit_tab.data(), jit_tab.size() * sizeof(double))
+                                          : pk.append(jit_tab32.data(), jit_tab32.size() * sizeof(float));
   const size_t o_efrag = pk.append(eff_frag.data(), eff_frag.size() * sizeof(double));
   const size_t o_jeff = pk.append(hb.jit_eff.data(), hb.jit_eff.size() * sizeof(double));
   const size_t o_jthermo = pk.append(hb.jit_thermo.data(), hb.jit_thermo.size() * sizeof(double));
@@ -1084,6 +1099,7 @@ extern "C" int64_t ck_mech_info(const ck_mech *m, int what) {
     case 16: return m->jac ? ck::jac_cells_per_tile(m->jac) : 0;
     case 17: return (m->jit_kernel && m->jit_spec.pair) ? 1 : 0;
     case 18: return (m->jit_kernel && m->jit_spec.kc_none) ? 1 : 0;
+    case 19: return m->jit_kernel ? m->jit_spec.prec : 0;
     default: return -1;
   }
 }

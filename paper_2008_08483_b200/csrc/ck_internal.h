@@ -44,6 +44,7 @@ struct JitSpec {
   bool tab_in_smem = true;
   bool m_dmma = true;          // M = C E on DMMA.8x8x4 (else register-tiled DFMA)
   bool m_hint = true;          // M scratch accesses carry an L2 evict_last policy
+  int prec = 0;                // ck_mech_desc.precision: 0 fp64, 1 mixed (CK_PREC in ck_jit_kernel.cuh)
   int sync_every = 0;          // block barrier every n reaction blocks (0 = never)
   int block = 4;               // reactions per block of the core
   int s_reg = 0;               // register accumulators per thread (internal species order); rest in smem

@@ -75,13 +75,14 @@ std::string lit(double v) {
 
 // nu^T ln C of one side of a reaction as an expression: sums and fmas of CK_LNC(k)
 std::string gather_expr(const std::vector<std::pair<int, double>> &side) {
-  if (side.empty()) return "0.0";
+  if (side.empty()) return "CK_LIT(0.0)";
   std::string e;
   for (size_t i = 0; i < side.size(); ++i) {
     const std::string c = "CK_LNC(" + std::to_string(side[i].first) + ")";
     const double nu = side[i].second;
-    if (i == 0) e = (nu == 1.0) ? c : (lit(nu) + " * " + c);
-    else e = (nu == 1.0) ? (e + " + " + c) : ("fma(" + lit(nu) + ", " + c + ", " + e + ")");
+    const std::string l = "CK_LIT(" + lit(nu) + ")";
+    if (i == 0) e = (nu == 1.0) ? c : (l + " * " + c);
+    else e = (nu == 1.0) ? (e + " + " + c) : ("fma(" + l + ", " + c + ", " + e + ")");
   }
   return e;
 }
@@ -165,7 +166,7 @@ std::string jit_generate_source(const JitSpec &s) {
     << "\n#define CK_MINB " << s.min_blocks << "\n#define CK_NRANGES " << s.n_ranges
     << "\n#define CK_NM " << s.n_m << "\n#define CK_NMB " << s.n_mb
     << "\n#define CK_NFO " << s.n_fo << "\n#define CK_TAB_SMEM " << (s.tab_in_smem ? 1 : 0)
-    << "\n#define CK_M_DMMA " << (s.m_dmma ? 1 : 0) << "\n#define CK_M_HINT " << (s.m_hint ? 1 : 0) << "\n#define CK_KCONST " << (s.kconst ? 1 : 0) << "\n#define CK_SYNC_EVERY " << s.sync_every
+    << "\n#define CK_M_DMMA " << (s.m_dmma ? 1 : 0) << "\n#define CK_M_HINT " << (s.m_hint ? 1 : 0) << "\n#define CK_PREC " << s.prec << "\n#define CK_KCONST " << (s.kconst ? 1 : 0) << "\n#define CK_SYNC_EVERY " << s.sync_every
     << "\n#define CK_B " << s.block << "\n#define CK_NBLK " << (int)s.rxn.size() / s.block
     << "\n#define CK_G_TB0 " << s.group_end[1] << "\n#define CK_G_FO0 " << s.group_end[3]
     << "\n#define CK_TAB_NRANGES " << s.tab_ranges << "\n#define CK_ROW " << s.row
@@ -227,7 +228,7 @@ std::string jit_generate_source(const JitSpec &s) {
       const JitReaction &r = s.rxn[(size_t)k * B + bb];
       o << "        gf[" << bb << "] = " << gather_expr(r.reac) << ";";
       if (r.index >= 0) o << "  // reaction " << r.index;
-      o << "\n        gr[" << bb << "] = " << (r.reversible ? gather_expr(r.prod) : std::string("0.0")) << ";\n";
+      o << "\n        gr[" << bb << "] = " << (r.reversible ? gather_expr(r.prod) : std::string("CK_LIT(0.0)")) << ";\n";
     }
   };
   const char *names[6] = {"ck_core<0, 1>", "ck_core<0, 0>", "ck_core<1, 1>", "ck_core<1, 0>",
@@ -243,7 +244,7 @@ std::string jit_generate_source(const JitSpec &s) {
     }
   };
   o << "__device__ __forceinline__ void ck_reactions(const CkCtx &x, double (&w)[CK_SREG > 0 ? CK_SREG : 1]) {\n"
-    << "  double gf[CK_B], gr[CK_B], q[CK_B];\n";
+    << "  ck_real gf[CK_B], gr[CK_B];\n  double q[CK_B];\n";
   if (!s.pair) {
     // One switch case per loop trip: the scatters of the previous block (Eq. 2) and the
     // gathers of this one (Eq. 4), so that the unique code is walked in address order with one
