@@ -229,7 +229,10 @@ const char *ck_last_error(void);
  *       18 1 if the handle was built as a measurement-only ABLATION whose results are not the
  *       source term (environment CK_JIT_KC=none together with CK_ALLOW_ABLATION=1: the
  *       equilibrium layer removed, used by bench.py --ann to cost that layer); 0 otherwise,
- *       19 the handle's precision (CK_PREC_*).
+ *       19 the handle's precision (CK_PREC_*),
+ *       20 1 if ck_source_terms runs the all-DMMA small-mechanism kernel (environment
+ *       CK_JIT_NU=dmma, at most 16 species and 64 reactions: every contraction of Eq. 2 and 4
+ *       and M = C E as dense DMMA.8x8x4 products; same results to rounding).
  * Returns -1 for a NULL handle or unknown `what`. */
 int64_t ck_mech_info(const ck_mech *m, int what);
 

@@ -12,8 +12,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libck.so")
-SOURCES = ["ck_api.cu", "ck_kernels.cu", "ck_jit.cu", "ck_rk4.cu", "ck_jac.cu", "ck_peaks.cu"]
-HEADERS = ["ck_internal.h", "ck_program.h", "ck_jit_kernel.cuh"]
+SOURCES = ["ck_api.cu", "ck_kernels.cu", "ck_jit.cu", "ck_rk4.cu", "ck_jac.cu", "ck_peaks.cu", "ck_nu.cu"]
+HEADERS = ["ck_internal.h", "ck_program.h", "ck_jit_kernel.cuh", "ck_jit_math.cuh", "ck_nu_kernel.cuh"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC"]
 
@@ -24,14 +24,22 @@ def _newest_source() -> float:
 
 
 def _embed_jit_source() -> None:
-    """ck_jit_kernel.cuh -> ck_jit_source.inc: the kernel text as C++ raw string literals
-    (the text NVRTC compiles at ck_mech_create time)."""
-    text = open(os.path.join(CSRC, "ck_jit_kernel.cuh")).read()
-    assert ')CKJIT"' not in text
-    chunks = [text[i:i + 8000] for i in range(0, len(text), 8000)]
-    with open(os.path.join(CSRC, "ck_jit_source.inc"), "w") as fh:
-        for c in chunks:
-            fh.write('R"CKJIT(' + c + ')CKJIT"\n')
+    """ck_jit_kernel.cuh, ck_nu_kernel.cuh (+ the shared ck_jit_math.cuh pasted in at their
+    //@@CK_MATH@@ line) -> ck_jit_source.inc, ck_nu_source.inc: the kernel texts as C++ raw string
+    literals (what NVRTC compiles at ck_mech_create time)."""
+    math = open(os.path.join(CSRC, "ck_jit_math.cuh")).read()
+    for src, dst in (("ck_jit_kernel.cuh", "ck_jit_source.inc"), ("ck_nu_kernel.cuh", "ck_nu_source.inc")):
+        text = open(os.path.join(CSRC, src)).read()
+        assert text.count("//@@CK_MATH@@") == 1
+        line = [l for l in text.splitlines() if l.startswith("//@@CK_MATH@@")][0]
+        text = text.replace(line, math)
+        assert ')CKJIT"' not in text
+        chunks = [text[i:i + 8000] for i in range(0, len(text), 8000)]
+        out = "".join('R"CKJIT(' + c + ')CKJIT"\n' for c in chunks)
+        path = os.path.join(CSRC, dst)
+        if not os.path.exists(path) or open(path).read() != out:      # (keeps the object cache valid)
+            with open(path, "w") as fh:
+                fh.write(out)
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

@@ -141,6 +141,7 @@ struct HostBuild {
   std::vector<double> jit_eff;
   std::vector<double> jit_thermo;   // [n_ranges][S][12], the NASA-7 set holding in each range
   std::vector<double> jit_logtab;   // [128][2]: 1/c_i, ln c_i (ck_log in ck_jit_kernel.cuh)
+  std::vector<double> tab_orig, thermo_orig;   // rate rows / thermo rows in the caller's order (ck_nu.cu)
   std::vector<unsigned char> program;
   ck::JitSpec spec;
   std::string jit_why;        // why the mechanism cannot be specialised ("" if it can)
@@ -620,6 +621,8 @@ void build_host(const ck_mech_desc *d, HostBuild *hb, size_t smem_sm = kSmemPerS
     hb->jit_logtab[2 * i + 1] = (double)(-logl((long double)inv_c));
   }
   hb->n_ranges_tmp = n_ranges;
+  hb->tab_orig = jit_tab;
+  hb->thermo_orig = hb->jit_thermo;
   finalize_jit(d, hb, falloff, smem_sm, smem_blk);
   if (falloff.empty()) falloff.resize(ck::kFalloffStride, 0.0);
   if (range_T.empty()) range_T.push_back(0.0);
@@ -811,6 +814,14 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
     dm.n_slots = m->grid_max;
   }
   m->jit_s_reg = spec.pair ? std::min(2 * spec.s_reg, S) : spec.s_reg;
+  // ---- the all-DMMA small-mechanism kernel (ck_nu.cu), on request ---------------------------
+  if (const char *e = std::getenv("CK_JIT_NU")) {
+    if (std::string(e) == "dmma") {
+      const std::string err = ck::nu_create(d, n_ranges, hb.range_T, hb.tab_orig, hb.thermo_orig, hb.jit_logtab, hb.falloff,
+                                            m->device, m->num_sms, (size_t)prop.sharedMemPerBlockOptin, &m->nu);
+      if (!err.empty()) { ck_mech_destroy(m); return fail(CK_EUNSUPPORTED, "CK_JIT_NU=dmma: " + err); }
+    }
+  }
   // ---- tables of the Jacobian kernel (ck_jac.cu) ------------------------------------------
   {
     const std::string err = ck::jac_create(d, m->num_sms, (size_t)prop.sharedMemPerBlockOptin, &m->jac);
@@ -826,6 +837,7 @@ extern "C" void ck_mech_destroy(ck_mech *m) {
   if (m->d_scratch) cudaFree(m->d_scratch);
   if (m->d_slot_busy) cudaFree(m->d_slot_busy);
   ck::jac_destroy(m->jac);
+  ck::nu_destroy(m->nu);
   if (m->d_stage) cudaFree(m->d_stage);
   if (m->host_in) cudaStreamDestroy(m->host_in);
   if (m->host_out) cudaStreamDestroy(m->host_out);
@@ -851,7 +863,9 @@ extern "C" int ck_source_terms(const ck_mech *m, const double *T, const double *
   if (((uintptr_t)T | (uintptr_t)P | (uintptr_t)Y | (uintptr_t)wdot | (uintptr_t)dTdt) & 7u)
     return fail(CK_EINVAL, "pointers must be 8-byte aligned");
   cudaError_t ce;
-  if (m->jit_kernel) {
+  if (m->nu) {
+    ce = ck::nu_launch(m->nu, T, P, Y, N, wdot, dTdt, (cudaStream_t)stream);
+  } else if (m->jit_kernel) {
     ck::JitParams prm = m->jit_params;
     prm.T = T; prm.P = P; prm.Y = Y; prm.wdot = wdot; prm.dTdt = dTdt; prm.N = N;
     // Balanced tiles: the fewest waves of full tiles the grid needs, then the tile size that
@@ -1089,9 +1103,9 @@ extern "C" int64_t ck_mech_info(const ck_mech *m, int what) {
     case 6: return m->n_lindemann;
     case 7: return m->n_troe;
     case 8: return m->dev.n_ranges;
-    case 9: return m->jit_kernel ? m->jit_threads : m->dev.threads;
+    case 9: return m->nu ? ck::nu_threads(m->nu) : (m->jit_kernel ? m->jit_threads : m->dev.threads);
     case 10: return m->jit_kernel ? m->jit_blocks_per_sm : m->blocks_per_sm;
-    case 11: return (int64_t)(m->jit_kernel ? m->jit_smem : m->smem_bytes);
+    case 11: return (int64_t)(m->nu ? ck::nu_smem(m->nu) : (m->jit_kernel ? m->jit_smem : m->smem_bytes));
     case 12: return 1;
     case 13: return m->nnz_eff;
     case 14: return m->jit_kernel ? 1 : 0;
@@ -1100,6 +1114,7 @@ extern "C" int64_t ck_mech_info(const ck_mech *m, int what) {
     case 17: return (m->jit_kernel && m->jit_spec.pair) ? 1 : 0;
     case 18: return (m->jit_kernel && m->jit_spec.kc_none) ? 1 : 0;
     case 19: return m->jit_kernel ? m->jit_spec.prec : 0;
+    case 20: return m->nu ? 1 : 0;
     default: return -1;
   }
 }

@@ -72,6 +72,18 @@ int jac_cells_per_tile(const JacMech *jm);
 cudaError_t jac_launch(const JacMech *jm, const double *T, const double *P, const double *Y, int64_t N,
                        double *J, cudaStream_t stream);
 
+// The all-DMMA small-mechanism kernel (ck_nu.cu / ck_nu_kernel.cuh).
+struct NuMech;
+std::string nu_create(const ck_mech_desc *d, int n_ranges, const std::vector<double> &range_T,
+                      const std::vector<double> &tab_orig, const std::vector<double> &thermo,
+                      const std::vector<double> &logtab, const std::vector<double> &falloff, int device,
+                      int num_sms, size_t smem_block_max, NuMech **out);
+void nu_destroy(NuMech *nm);
+cudaError_t nu_launch(const NuMech *nm, const double *T, const double *P, const double *Y, int64_t N, double *wdot,
+                      double *dTdt, cudaStream_t stream);
+int nu_threads(const NuMech *nm);
+size_t nu_smem(const NuMech *nm);
+
 std::string jit_generate_source(const JitSpec &spec);
 // Compiles to a cubin for sm_100a with NVRTC; returns "" on success, else the error text.
 // use_cache = false: do not read the on-disk cubin cache (it is still refreshed).
@@ -107,6 +119,8 @@ struct ck_mech {
   std::string jit_note;       // why the specialised kernel is not in use, if so
   // analytic Jacobian (ck_jacobian): NULL if unsupported for this mechanism
   ck::JacMech *jac = nullptr;
+  // all-DMMA small-mechanism kernel (CK_JIT_NU=dmma), used by ck_source_terms when present
+  ck::NuMech *nu = nullptr;
   // staging for ck_source_terms_host
   double *d_stage = nullptr;
   int64_t stage_cells = 0;
