@@ -87,6 +87,13 @@ struct JacTables {
 struct JacMech {
   JacTables t{};
   void *d_blob = nullptr;
+  // second kernel (lanes = cells, ck_jac_v2.cuh): tables in the same blob, scratch of its own
+  bool v2 = false;
+  int v2_mt = 0, v2_nth = 4, v2_nw = 0;
+  size_t v2_smem = 0;
+  void *v2_tables = nullptr;    // host copy of Jac2Tables (device pointers inside)
+  double *d_v2_scratch = nullptr;
+  int v2_grid = 1;
   int cells = 8;               // cells per tile
   int warps = 16, minb = 1;    // warps per block, blocks per SM
   size_t smem = 0;
@@ -468,6 +475,8 @@ jacobian_kernel(const JacTables t, const double *__restrict__ Tg, const double *
 #undef ABAT
 }
 
+#include "ck_jac_v2.cuh"
+
 }  // namespace
 }  // namespace ck
 
@@ -580,7 +589,77 @@ std::string jac_create(const ck_mech_desc *d, int num_sms, size_t smem_block_max
   if (jm->smem > smem_block_max) { delete jm; return ""; }
   jm->grid_max = num_sms * jm->minb;
 
+  // ---- tables of the second kernel (ck_jac_v2.cuh) -----------------------------------------------
+  // rows: reactions of row i with their sparse entries (l, cf, cr) over the reaction's species;
+  // dense part: the third-body / falloff reactions of row i in k-steps of 4, E gathered per row as
+  // DMMA A fragments
+  const int n1 = S + 1;
+  const int mt_need = (n1 + 7) / 8;
+  int v2_mt = 0, v2_nth = 4, v2_maxt = 512;
+  for (int cand : {2, 4, 7, 8, 12, 14, 16})
+    if (cand >= mt_need) { v2_mt = cand; break; }
+  if (v2_mt > 8) { v2_nth = 2; v2_maxt = 256; } else if (v2_mt > 4) { v2_maxt = 384; }
+  std::vector<int> rowj_start(S + 1, 0), ks_start(S + 1, 0);
+  std::vector<Jac2RowJ> rowj;
+  std::vector<Jac2Ent> ent2;
+  std::vector<Jac2Coef> coef2;
+  std::vector<double> afrag;
+  if (v2_mt) {
+    for (int i = 0; i < S; ++i) {
+      rowj_start[i] = (int)rowj.size();
+      ks_start[i] = (int)coef2.size() / 4;
+      std::vector<int> tbs;   // third-body reactions (internal index) of the row
+      for (int j = 0; j < R; ++j) {
+        const int oj = order[j];
+        const double dnu = d->nu_prod[(size_t)i * R + oj] - d->nu_reac[(size_t)i * R + oj];
+        if (dnu == 0.0) continue;
+        Jac2RowJ rj{dnu, j, (int)ent2.size(), 0, 0};
+        for (int l = 0; l < S; ++l) {
+          const double f = d->nu_reac[(size_t)l * R + oj], p = d->nu_prod[(size_t)l * R + oj];
+          if (f == 0.0 && p == 0.0) continue;
+          ent2.push_back(Jac2Ent{dnu * f, dnu * p, l, 0});
+        }
+        rj.ent1 = (int)ent2.size();
+        rowj.push_back(rj);
+        if (rxn[j].tb >= 0) tbs.push_back(j);
+      }
+      const int nks = ((int)tbs.size() + 3) / 4;
+      for (int ks = 0; ks < nks; ++ks) {
+        const size_t a0 = afrag.size();
+        afrag.resize(a0 + (size_t)v2_mt * 32, 0.0);
+        for (int qq = 0; qq < 4; ++qq) {
+          const int kk = 4 * ks + qq;
+          if (kk < (int)tbs.size()) {
+            const int j = tbs[kk], oj = order[j];
+            coef2.push_back(Jac2Coef{d->nu_prod[(size_t)i * R + oj] - d->nu_reac[(size_t)i * R + oj], rxn[j].tb, 0});
+            for (int mt = 0; mt < v2_mt; ++mt)
+              for (int gg = 0; gg < 8; ++gg) {
+                const int l = 8 * mt + gg;
+                if (l < S) afrag[a0 + (size_t)mt * 32 + gg * 4 + qq] = E[(size_t)rxn[j].tb * SP + l];
+              }
+          } else {
+            coef2.push_back(Jac2Coef{0.0, -1, 0});
+          }
+        }
+      }
+    }
+    rowj_start[S] = (int)rowj.size();
+    ks_start[S] = (int)coef2.size() / 4;
+  }
+  // work of a row (sparse entries, reactions, k-steps of the dense part), for the static balance
+  std::vector<int> row_order(S), row_work(S, 0), warp_row_start(17 + 1, 0);
+  for (int i = 0; i < S; ++i) row_order[i] = i;
+  if (v2_mt)
+    for (int i = 0; i < S; ++i) {
+      int ents = 0;
+      for (int e = rowj_start[i]; e < rowj_start[i + 1]; ++e) ents += rowj[e].ent1 - rowj[e].ent0;
+      row_work[i] = ents * 12 + (rowj_start[i + 1] - rowj_start[i]) * 20 + (ks_start[i + 1] - ks_start[i]) * 60 + 400;
+    }
+
   std::vector<unsigned char> blob;
+  const size_t o_ro = blob_add(blob, row_order), o_ws = blob_add(blob, warp_row_start);
+  const size_t o_rj0 = blob_add(blob, rowj_start), o_rj = blob_add(blob, rowj), o_e2 = blob_add(blob, ent2),
+               o_ks = blob_add(blob, ks_start), o_co = blob_add(blob, coef2), o_af = blob_add(blob, afrag);
   const size_t o_invW = blob_add(blob, invW), o_lo = blob_add(blob, lo), o_hi = blob_add(blob, hi),
                o_tmid = blob_add(blob, tmid), o_rxn = blob_add(blob, rxn), o_sup = blob_add(blob, sup),
                o_tbr = blob_add(blob, tb_rxn), o_E = blob_add(blob, E), o_rs = blob_add(blob, row_start),
@@ -602,6 +681,58 @@ std::string jac_create(const ck_mech_desc *d, int num_sms, size_t smem_block_max
   t.row_start = (const int *)(b + o_rs); t.row_ent = (const JacRowEnt *)(b + o_re);
   t.off_start = (const int *)(b + o_os); t.off_ent = (const JacOffEnt *)(b + o_oe);
   t.ln_pref_Ru = std::log(d->p_ref / kRu);
+  // ---- second kernel: warps per block from the shared memory, scratch per block ------------------
+  if (v2_mt && !(std::getenv("CK_JAC_KERNEL") && std::string(std::getenv("CK_JAC_KERNEL")) == "v1")) {
+    // warps per block: the shape with the most resident warps per SM (shared memory and the
+    // kernel's register cap decide); among equals the smaller blocks, whose tiles overlap better
+    int nw = 0, v2_bps = 1;
+    size_t smem2 = 0;
+    const int regs = v2_maxt == 512 ? 128 : (v2_maxt == 384 ? 168 : 255);
+    int best_warps = 0;
+    for (int cand : {2, 4, 6, 8, 12, 16}) {
+      if (cand * 32 > v2_maxt) continue;
+      const size_t base = std::max((size_t)cand * n1 * 33, (size_t)6 * S * 32);
+      const size_t doubles = base + (size_t)std::max(n_tb, 1) * 32 + (size_t)S * 32 + (size_t)4 * cand * 32;
+      if (doubles * 8 > smem_block_max) continue;
+      const int bps = (int)std::min<size_t>(std::min<size_t>(16, 233472 / (doubles * 8 + 1024)), 65536 / ((size_t)regs * cand * 32));
+      if (bps < 1) continue;
+      if (cand * bps > best_warps) { best_warps = cand * bps; nw = cand; v2_bps = bps; smem2 = doubles * 8; }
+    }
+    if (nw) {
+      // rows to warps: longest processing time first (fixed, so results are reproducible)
+      std::vector<int> by_work(S);
+      for (int i = 0; i < S; ++i) by_work[i] = i;
+      std::stable_sort(by_work.begin(), by_work.end(), [&](int x, int y) { return row_work[x] > row_work[y]; });
+      std::vector<std::vector<int>> rows_of(nw);
+      std::vector<long long> load(nw, 0);
+      for (int i : by_work) {
+        const int w = (int)(std::min_element(load.begin(), load.end()) - load.begin());
+        rows_of[w].push_back(i);
+        load[w] += row_work[i];
+      }
+      std::vector<int> ro, ws(nw + 1, 0);
+      for (int w = 0; w < nw; ++w) { ro.insert(ro.end(), rows_of[w].begin(), rows_of[w].end()); ws[w + 1] = (int)ro.size(); }
+      ce = cudaMemcpy((void *)(b + o_ro), ro.data(), ro.size() * sizeof(int), cudaMemcpyHostToDevice);
+      if (ce == cudaSuccess) ce = cudaMemcpy((void *)(b + o_ws), ws.data(), ws.size() * sizeof(int), cudaMemcpyHostToDevice);
+      if (ce != cudaSuccess) { jac_destroy(jm); return std::string("Jacobian tables: ") + cudaGetErrorString(ce); }
+      Jac2Tables *u = new Jac2Tables();
+      u->warp_row_start = (const int *)(b + o_ws);
+      u->rowj_start = (const int *)(b + o_rj0); u->rowj = (const Jac2RowJ *)(b + o_rj); u->ent = (const Jac2Ent *)(b + o_e2);
+      u->row_order = (const int *)(b + o_ro);
+      u->ks_start = (const int *)(b + o_ks); u->coef = (const Jac2Coef *)(b + o_co); u->afrag = (const double *)(b + o_af);
+      u->scratch_per_block = (size_t)4 * R * 32 + (size_t)2 * S * 32 + (size_t)nw * n1 * 32;
+      ce = cudaMalloc((void **)&jm->d_v2_scratch, (size_t)num_sms * v2_bps * u->scratch_per_block * sizeof(double));
+      if (ce != cudaSuccess) {
+        delete u;
+        jac_destroy(jm);
+        return std::string("Jacobian scratch: ") + cudaGetErrorString(ce);
+      }
+      u->scratch = jm->d_v2_scratch;
+      jm->v2 = true; jm->v2_mt = v2_mt; jm->v2_nth = v2_nth; jm->v2_nw = nw; jm->v2_smem = smem2;
+      jm->v2_tables = u;
+      jm->v2_grid = num_sms * v2_bps;
+    }
+  }
   *out = jm;
   return "";
 }
@@ -609,13 +740,31 @@ std::string jac_create(const ck_mech_desc *d, int num_sms, size_t smem_block_max
 void jac_destroy(JacMech *jm) {
   if (!jm) return;
   if (jm->d_blob) cudaFree(jm->d_blob);
+  if (jm->d_v2_scratch) cudaFree(jm->d_v2_scratch);
+  delete (Jac2Tables *)jm->v2_tables;
   delete jm;
 }
 
-int jac_cells_per_tile(const JacMech *jm) { return jm->cells; }
+int jac_cells_per_tile(const JacMech *jm) { return jm->v2 ? 32 : jm->cells; }
 
 cudaError_t jac_launch(const JacMech *jm, const double *T, const double *P, const double *Y, int64_t N,
                        double *J, cudaStream_t stream) {
+  if (jm->v2) {
+    const Jac2Tables &u = *(const Jac2Tables *)jm->v2_tables;
+    const int grid = (int)std::min<long long>((N + 31) / 32, jm->v2_grid);
+#define CK_JAC2_CASE(MT, NTH, MAXT)                                                                    \
+  if (jm->v2_mt == MT) {                                                                               \
+    cudaError_t e = cudaFuncSetAttribute(jacobian_kernel_v2<MT, NTH, MAXT>,                            \
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)jm->v2_smem); \
+    if (e != cudaSuccess) return e;                                                                    \
+    jacobian_kernel_v2<MT, NTH, MAXT><<<grid, jm->v2_nw * 32, jm->v2_smem, stream>>>(jm->t, u, T, P, Y, (long long)N, J); \
+    return cudaGetLastError();                                                                         \
+  }
+    CK_JAC2_CASE(2, 4, 512) CK_JAC2_CASE(4, 4, 512) CK_JAC2_CASE(7, 4, 384) CK_JAC2_CASE(8, 4, 384)
+    CK_JAC2_CASE(12, 2, 256) CK_JAC2_CASE(14, 2, 256) CK_JAC2_CASE(16, 2, 256)
+#undef CK_JAC2_CASE
+    return cudaErrorInvalidConfiguration;
+  }
   const int cpl = jm->t.SP / 32;
   const long long tiles = (N + jm->cells - 1) / jm->cells;
   const int grid = (int)std::min<long long>(tiles, jm->grid_max);

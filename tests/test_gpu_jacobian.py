@@ -28,6 +28,14 @@ def ck():
     return ck
 
 
+@pytest.fixture(autouse=True, params=["v2", "v1"])
+def jac_kernel(request, monkeypatch):
+    """Every test runs on both Jacobian kernels: v2 (lanes = cells, DMMA dense part, the default) and
+    v1 (lanes = columns, tiles of 4 to 32 cells)."""
+    monkeypatch.setenv("CK_JAC_KERNEL", request.param)
+    return request.param
+
+
 def gpu_jacobian(ck, gm, T, P, Y):
     dev = torch.device("cuda:0")
     N, S = T.shape[0], Y.shape[0]
@@ -70,7 +78,7 @@ def test_parity_all_entries(ck, cfg_name, N):
     assert rs <= 1.0 and re <= 1.0, (cfg_name, rs, re)
 
 
-@pytest.mark.parametrize("N", [1, 3, 7, 8, 9, 17])
+@pytest.mark.parametrize("N", [1, 3, 7, 8, 9, 17, 31, 32, 33, 65])
 def test_ragged_batches_and_determinism(ck, N):
     cfg = ckgen.CONFIGS["mid_1m"]
     mech = ckgen.mechanism(cfg.mech)
@@ -86,7 +94,7 @@ def test_ragged_batches_and_determinism(ck, N):
 
 @pytest.mark.parametrize("shape", ["4,16,1", "8,16,1", "16,16,1", "32,16,1", "4,8,2"])
 @pytest.mark.parametrize("N", [1, 31, 33, 70])
-def test_every_launch_shape_on_the_tiny_mechanism(ck, monkeypatch, shape, N):
+def test_every_launch_shape_on_the_tiny_mechanism(ck, monkeypatch, jac_kernel, shape, N):
     """Tiles of 4 to 32 cells and both block sizes (CK_JAC_SHAPE = cells, warps, blocks per SM),
     with batches that leave a ragged last tile: same bits from every shape (the arithmetic of a
     cell does not depend on the tile it falls in), parity on one of them."""
@@ -95,6 +103,8 @@ def test_every_launch_shape_on_the_tiny_mechanism(ck, monkeypatch, shape, N):
     T, P, Y = ckgen.states(cfg, N=N)
     with ck.Mechanism(mech) as gm:
         Jd = gpu_jacobian(ck, gm, T, P, Y)
+    if jac_kernel != "v1":
+        pytest.skip("launch shapes of the first kernel")
     monkeypatch.setenv("CK_JAC_SHAPE", shape)
     with ck.Mechanism(mech) as gm:
         assert gm.info("jac_cells") == int(shape.split(",")[0])
