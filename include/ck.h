@@ -232,7 +232,10 @@ const char *ck_last_error(void);
  *       19 the handle's precision (CK_PREC_*),
  *       20 1 if ck_source_terms runs the all-DMMA small-mechanism kernel (environment
  *       CK_JIT_NU=dmma, at most 16 species and 64 reactions: every contraction of Eq. 2 and 4
- *       and M = C E as dense DMMA.8x8x4 products; same results to rounding).
+ *       and M = C E as dense DMMA.8x8x4 products; same results to rounding),
+ *       21 the largest N for which ck_source_terms uses a small-batch shape of the specialised
+ *       kernel (8, 4 or 2 threads per cell in tiles of 32, 64 or 128 cells, whichever holds the
+ *       batch in one wave; 0 if no such shape was built).
  * Returns -1 for a NULL handle or unknown `what`. */
 int64_t ck_mech_info(const ck_mech *m, int what);
 

@@ -643,7 +643,7 @@ int alloc_scratch(ck_mech *m, int n_slots, size_t slot_elems) {
   return CK_OK;
 }
 
-int setup_jit(ck_mech *m, ck::JitSpec &spec, const std::string &why, size_t smem, size_t smem_sm) {
+int setup_jit(ck_mech *m, ck::JitSpec &spec, const std::string &why, size_t smem, size_t smem_sm, size_t smem_blk) {
   const char *mode_env = std::getenv("CK_KERNEL");
   std::string mode = mode_env ? mode_env : "auto";
   if (spec.kc_ann) {
@@ -713,6 +713,36 @@ int setup_jit(ck_mech *m, ck::JitSpec &spec, const std::string &why, size_t smem
   m->jit_params.m_scratch = m->d_scratch;
   m->jit_params.slot_busy = m->d_slot_busy;
   m->jit_params.n_slots = m->num_sms * per_sm;
+
+  // ---- the small-batch shape (CK_SPLIT = 8 threads per cell, tiles of 32 cells): one warp no longer
+  //      walks the whole mechanism alone when the batch is a few thousand cells.  Same tables, same
+  //      scratch slots.  For mechanisms whose accumulators all sit in registers, of 32 reactions or
+  //      more; CK_JIT_SPLIT=0 turns it off, a failure to build it is not an error.
+  //      CK_JIT_SPLIT=k builds only the shape with k threads per cell (0: none); default 8, 4 and 2.
+  const int only = env_int("CK_JIT_SPLIT", -1);
+  if (only != 0 && !spec.pair && spec.s_reg == spec.S && !spec.kc_ann && spec.tab_in_smem && spec.R >= 32 && per_sm == 1)
+    for (int split : {8, 4, 2}) {
+      if (only > 0 && split != only) continue;
+      ck::JitSpec s2 = spec;
+      s2.split = split; s2.threads = 256; s2.min_blocks = 1;
+      const size_t tab_elem = spec.prec == CK_PREC_F32_RATES ? sizeof(float) : sizeof(double);
+      const size_t smem2 = (size_t)spec.S * (256 / split + 8) * 8 + (128 * spec.lut_rep + 256) * 8 + (size_t)spec.n_ranges * spec.S * 12 * 8 +
+                           (size_t)spec.tab_ranges * spec.R * spec.row * tab_elem + (size_t)(spec.S + 4) * 256 * 8 + 16;
+      std::vector<char> cubin2;
+      const int at = m->n_split;
+      if (smem2 + 64 <= smem_blk && ck::jit_compile(ck::jit_generate_source(s2), &cubin2).empty() &&
+          cudaLibraryLoadData(&m->split_lib[at], cubin2.data(), nullptr, nullptr, 0, nullptr, nullptr, 0) == cudaSuccess) {
+        if (cudaLibraryGetKernel(&m->split_kernel[at], m->split_lib[at], "ck_source_terms_jit") == cudaSuccess &&
+            cudaKernelSetAttributeForDevice(m->split_kernel[at], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2, m->device) == cudaSuccess) {
+          m->split_smem[at] = smem2; m->split_cells[at] = 256 / split;
+          m->n_split++;
+        } else {
+          cudaLibraryUnload(m->split_lib[at]);
+          m->split_lib[at] = nullptr; m->split_kernel[at] = nullptr;
+        }
+      }
+      cudaGetLastError();
+    }
   return CK_OK;
 }
 
@@ -805,7 +835,8 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   m->jit_params.tab = (const double *)(base + o_jtab);
   m->jit_params.thermo = (const double *)(base + o_jthermo);
   m->jit_params.logtab = (const double *)(base + o_jlog);
-  if (int st = setup_jit(m, spec, hb.jit_why, hb.jit_smem, (size_t)prop.sharedMemPerMultiprocessor)) { ck_mech_destroy(m); return st; }
+  if (int st = setup_jit(m, spec, hb.jit_why, hb.jit_smem, (size_t)prop.sharedMemPerMultiprocessor,
+                         (size_t)prop.sharedMemPerBlockOptin)) { ck_mech_destroy(m); return st; }
   if (!m->jit_kernel) {
     // generic kernel in use: its own M scratch, one slot per resident block
     if (int st = alloc_scratch(m, m->grid_max, (size_t)std::max(n_mb, 1) * ck::kMBlock * best_threads)) { ck_mech_destroy(m); return st; }
@@ -844,6 +875,7 @@ extern "C" void ck_mech_destroy(ck_mech *m) {
   for (cudaEvent_t e : m->host_ev) if (e) cudaEventDestroy(e);
   if (m->rk4_graph) cudaGraphExecDestroy(m->rk4_graph);
   if (m->rk4_lib) cudaLibraryUnload(m->rk4_lib);
+  for (cudaLibrary_t l : m->split_lib) if (l) cudaLibraryUnload(l);
   if (m->d_rk4) cudaFree(m->d_rk4);
   if (m->jit_lib) cudaLibraryUnload(m->jit_lib);
   delete m;
@@ -865,6 +897,18 @@ extern "C" int ck_source_terms(const ck_mech *m, const double *T, const double *
   cudaError_t ce;
   if (m->nu) {
     ce = ck::nu_launch(m->nu, T, P, Y, N, wdot, dTdt, (cudaStream_t)stream);
+  } else if (m->n_split > 0 && N <= (int64_t)m->split_cells[m->n_split - 1] * m->num_sms) {
+    // small batch: one wave of tiles, the most threads per cell whose tiles hold the batch
+    int v = 0;
+    while (N > (int64_t)m->split_cells[v] * m->num_sms) ++v;
+    ck::JitParams prm = m->jit_params;
+    prm.T = T; prm.P = P; prm.Y = Y; prm.wdot = wdot; prm.dTdt = dTdt; prm.N = N;
+    int64_t tc = (N + m->num_sms - 1) / m->num_sms;
+    tc = std::min<int64_t>(m->split_cells[v], (tc + 31) / 32 * 32);
+    prm.tile_cells = (int)tc;
+    void *args[] = {&prm};
+    ce = cudaLaunchKernel((const void *)m->split_kernel[v], dim3((unsigned)((N + tc - 1) / tc)), dim3(256), args,
+                          m->split_smem[v], (cudaStream_t)stream);
   } else if (m->jit_kernel) {
     ck::JitParams prm = m->jit_params;
     prm.T = T; prm.P = P; prm.Y = Y; prm.wdot = wdot; prm.dTdt = dTdt; prm.N = N;
@@ -1115,6 +1159,7 @@ extern "C" int64_t ck_mech_info(const ck_mech *m, int what) {
     case 18: return (m->jit_kernel && m->jit_spec.kc_none) ? 1 : 0;
     case 19: return m->jit_kernel ? m->jit_spec.prec : 0;
     case 20: return m->nu ? 1 : 0;
+    case 21: return m->n_split ? (int64_t)m->split_cells[m->n_split - 1] * m->num_sms : 0;
     default: return -1;
   }
 }
@@ -1126,6 +1171,8 @@ extern "C" int64_t ck_mech_jit_source(const ck_mech_desc *d, char *buf, int64_t 
   HostBuild hb;
   build_host(d, &hb);
   if (!hb.jit_why.empty()) { fail(CK_EUNSUPPORTED, hb.jit_why); return -1; }
+  // (CK_JIT_SOURCE_SPLIT=K: the text of the small-batch shape instead, for offline inspection)
+  if (const int k = env_int("CK_JIT_SOURCE_SPLIT", 0)) { hb.spec.split = k; hb.spec.threads = 256; hb.spec.min_blocks = 1; }
   const std::string src = ck::jit_generate_source(hb.spec);
   if (buf && cap > 0) {
     const size_t n = std::min((size_t)cap - 1, src.size());

@@ -44,6 +44,7 @@ struct JitSpec {
   bool tab_in_smem = true;
   bool m_dmma = true;          // M = C E on DMMA.8x8x4 (else register-tiled DFMA)
   bool m_hint = true;          // M scratch accesses carry an L2 evict_last policy
+  int split = 1;               // small-batch shape: threads per cell (CK_SPLIT in ck_jit_kernel.cuh)
   int prec = 0;                // ck_mech_desc.precision: 0 fp64, 1 mixed (CK_PREC in ck_jit_kernel.cuh)
   int sync_every = 0;          // block barrier every n reaction blocks (0 = never)
   int block = 4;               // reactions per block of the core
@@ -113,6 +114,14 @@ struct ck_mech {
   int jit_cells = 0;          // cells per block of the specialised kernel (= threads, or half with pair)
   size_t jit_smem = 0;
   ck::JitSpec jit_spec;       // kept to compile the RK4 stage variant on first use
+  // the small-batch shape of the specialised kernel (CK_SPLIT threads per cell, tiles of 32 cells),
+  // used by ck_source_terms when the batch fits one wave of such tiles
+  // (up to three of them: 8, 4 and 2 threads per cell, tiles of 32, 64 and 128 cells)
+  cudaLibrary_t split_lib[3] = {nullptr, nullptr, nullptr};
+  cudaKernel_t split_kernel[3] = {nullptr, nullptr, nullptr};
+  size_t split_smem[3] = {0, 0, 0};
+  int split_cells[3] = {0, 0, 0};
+  int n_split = 0;
   cudaLibrary_t rk4_lib = nullptr;
   cudaKernel_t rk4_kernel = nullptr;
   bool rk4_tried = false;

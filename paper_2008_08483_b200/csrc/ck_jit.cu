@@ -166,7 +166,7 @@ std::string jit_generate_source(const JitSpec &s) {
     << "\n#define CK_MINB " << s.min_blocks << "\n#define CK_NRANGES " << s.n_ranges
     << "\n#define CK_NM " << s.n_m << "\n#define CK_NMB " << s.n_mb
     << "\n#define CK_NFO " << s.n_fo << "\n#define CK_TAB_SMEM " << (s.tab_in_smem ? 1 : 0)
-    << "\n#define CK_M_DMMA " << (s.m_dmma ? 1 : 0) << "\n#define CK_M_HINT " << (s.m_hint ? 1 : 0) << "\n#define CK_PREC " << s.prec << "\n#define CK_KCONST " << (s.kconst ? 1 : 0) << "\n#define CK_SYNC_EVERY " << s.sync_every
+    << "\n#define CK_M_DMMA " << (s.m_dmma ? 1 : 0) << "\n#define CK_M_HINT " << (s.m_hint ? 1 : 0) << "\n#define CK_PREC " << s.prec << "\n#define CK_SPLIT " << s.split << "\n#define CK_KCONST " << (s.kconst ? 1 : 0) << "\n#define CK_SYNC_EVERY " << s.sync_every
     << "\n#define CK_B " << s.block << "\n#define CK_NBLK " << (int)s.rxn.size() / s.block
     << "\n#define CK_G_TB0 " << s.group_end[1] << "\n#define CK_G_FO0 " << s.group_end[3]
     << "\n#define CK_TAB_NRANGES " << s.tab_ranges << "\n#define CK_ROW " << s.row
@@ -245,7 +245,26 @@ std::string jit_generate_source(const JitSpec &s) {
   };
   o << "__device__ __forceinline__ void ck_reactions(const CkCtx &x, double (&w)[CK_SREG > 0 ? CK_SREG : 1]) {\n"
     << "  ck_real gf[CK_B], gr[CK_B];\n  double q[CK_B];\n";
-  if (!s.pair) {
+  if (s.split > 1) {
+    // Small-batch shape: part x.half of a cell's CK_SPLIT threads walks blocks x.half, x.half + K, ..;
+    // a block's gathers, its rate core and its scatters (into this thread's own accumulators of
+    // every species) follow each other, two switches per block.
+    o << "#pragma unroll 1\n  for (int blk = x.half; blk < CK_NBLK; blk += CK_SPLIT) {\n    switch (blk) {\n";
+    for (int k = 0; k < nblk; ++k) {
+      o << "      case " << k << ":\n";
+      gathers(k);
+      o << "        break;\n";
+    }
+    o << "    }\n";
+    dispatch("    ", "0");
+    o << "    switch (blk) {\n";
+    for (int k = 0; k < nblk; ++k) {
+      o << "      case " << k << ":\n";
+      scatters(k, -1, "q[");
+      o << "        break;\n";
+    }
+    o << "    }\n  }\n}\n";
+  } else if (!s.pair) {
     // One switch case per loop trip: the scatters of the previous block (Eq. 2) and the
     // gathers of this one (Eq. 4), so that the unique code is walked in address order with one
     // indirect branch per block; trip CK_NBLK only scatters the last block.

@@ -478,6 +478,56 @@ def test_concurrent_calls_on_two_streams_share_one_handle(ck, cfg_name, N):
             assert rw <= 1.0 and rt <= 1.0, (cfg_name, rw, rt)
 
 
+@pytest.mark.parametrize("N", [1, 31, 32, 33, 256, 1000, 4096, 4736, 4737, 9472, 9473, 18944, 18945])
+def test_small_batch_shape_is_selected_and_matches_the_oracle(ck, kernel_variant, N):
+    """Below one wave of 32-cell tiles (N <= 32 x 148) ck_source_terms runs the small-batch shape of
+    the specialised kernel: 8 threads per cell taking alternate reaction blocks, partial accumulators
+    summed in a fixed order (the flat region of the paper's Fig. 9).  Parity on
+    the auto-selected shape on both sides of the switch, ragged tiles included, bitwise run to run;
+    with it turned off the same cells agree to the tolerance (another summation order)."""
+    if kernel_variant != "auto":
+        pytest.skip("specialised kernel only")
+    cfg = ckgen.CONFIGS["mid_1m"]
+    mech = ckgen.mechanism(cfg.mech)
+    T, P, Y = ckgen.states(cfg, N=N)
+    with ck.Mechanism(mech) as gm:
+        assert gm.info("small_batch_max") == 64 * 148     # (2 threads per cell do not fit shared memory at S=53)
+        w1, d1 = gpu_run(ck, mech, T, P, Y, gm)
+        w2, d2 = gpu_run(ck, mech, T, P, Y, gm)
+    assert np.array_equal(w1, w2) and np.array_equal(d1, d2)
+    wr, dr, _ = oracle.source_terms(oracle.OracleMechanism(mech), T, P, Y)
+    rw, rt = parity_violations(w1, d1, wr, dr)
+    assert rw <= 1.0 and rt <= 1.0, (N, rw, rt)
+
+
+def test_small_batch_shape_variants(ck, kernel_variant, monkeypatch):
+    """4 and 2 threads per cell (CK_JIT_SPLIT), the fp32-rates precision in the small-batch shape,
+    several temperature ranges, and mechanisms that do not get the shape (few reactions, S > 103)."""
+    if kernel_variant != "auto":
+        pytest.skip("specialised kernel only")
+    cfg = ckgen.CONFIGS["mid_1m"]
+    mech = ckgen.mechanism(cfg.mech)
+    rng = np.random.default_rng(11)
+    mech_r = dataclasses.replace(mech, T_mid=rng.choice([800.0, 1000.0, 1400.0], size=mech.n_species))
+    T, P, Y = ckgen.states(dataclasses.replace(cfg, T_range=(500.0, 2700.0)), N=777)
+    for split, cells in (("8", 32), ("4", 64), ("2", 0)):
+        monkeypatch.setenv("CK_JIT_SPLIT", split)
+        with ck.Mechanism(mech) as gm:
+            assert gm.info("small_batch_max") == cells * 148
+        assert_parity(ck, mech, T, P, Y, "split %s" % split)
+        assert_parity(ck, mech_r, T, P, Y, "split %s, four temperature ranges" % split)
+    monkeypatch.setenv("CK_JIT_SPLIT", "0")
+    with ck.Mechanism(mech) as gm:
+        assert gm.info("small_batch_max") == 0
+    monkeypatch.delenv("CK_JIT_SPLIT")
+    with ck.Mechanism(ckgen.mechanism(ckgen.MECH_TINY)) as gm:
+        assert gm.info("small_batch_max") == 0           # 21 reactions: the walk is short
+    with ck.Mechanism(ckgen.mechanism(ckgen.MECH_LARGE)) as gm:
+        assert gm.info("small_batch_max") == 0           # accumulators do not fit one thread's registers
+    with ck.Mechanism(mech, precision=2) as gm:
+        assert gm.info("small_batch_max") == 128 * 148    # (rate table in fp32: half the size)
+
+
 def test_error_codes(ck):
     mech = ckgen.mechanism(ckgen.MECH_TINY)
     gm = ck.Mechanism(mech)
