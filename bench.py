@@ -219,13 +219,25 @@ def run_sweep(args):
             torch.cuda.synchronize()
             cold.append(e0.elapsed_time(e1))
         cold_ms = float(np.median(cold))
+        # every row is checked where it is timed: finite results, mass and element conservation on
+        # every cell (the element-by-element comparison with the oracle at these sizes is
+        # tests/test_gpu_parity.py::test_sweep_sizes_parity_every_cell)
+        assert bool(torch.isfinite(w).all() and torch.isfinite(d).all()), "non-finite result at N=%d" % N
+        worst_cons = 0.0
+        for wt in [mech.mol_weight] + [mech.elem_count[:, e].astype(float) for e in range(mech.elem_count.shape[1])]:
+            terms = torch.from_numpy(wt).to(dev)[:, None] * w
+            worst_cons = max(worst_cons, float((terms.sum(0).abs() / (terms.abs().sum(0) + 1e-300)).max()))
+            del terms
+        assert worst_cons <= 1e-11, "conservation violated at N=%d: %.3g" % (N, worst_cons)
         rows.append({"N": N, "ms_back_to_back": warm_ms, "ms_l2_flushed": cold_ms,
+                     "checked": "finite; mass and element conservation residual <= %.1e of the terms on every cell" % worst_cons,
                      "cells_per_s": N / (warm_ms * 1e-3),
                      "roofline_frac": i_cell * N / (warm_ms * 1e-3) / peak,
                      "state_mb": 8 * (2 * S + 3) * N / 1e6})
     print(json.dumps({"sweep": "S=53 R=325 fp64, N = 2^8..2^22, one ck_source_terms call per timing",
                       "fp64_peak_tflops": 2 * peak / 1e12, "fp64_instr_per_cell": i_cell,
-                      "launch": {"threads": info["threads"], "blocks_per_sm": info["blocks_per_sm"]},
+                      "launch": {"threads": info["threads"], "blocks_per_sm": info["blocks_per_sm"],
+                                 "small_batch_shape_up_to_N": info["small_batch_max"]},
                       "rows": rows}))
     gm.close()
 

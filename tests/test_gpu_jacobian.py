@@ -75,6 +75,7 @@ def test_parity_all_entries(ck, cfg_name, N):
         J = gpu_jacobian(ck, gm, T, P, Y)
     Jr = oracle.jacobian(oracle.OracleMechanism(mech), T, P, Y)
     rs, re = violations(mech, T, P, Y, J, Jr)
+    print("%s: worst Jacobian error / bound: species rows %.3g, energy row %.3g" % (cfg_name, rs, re))
     assert rs <= 1.0 and re <= 1.0, (cfg_name, rs, re)
 
 
