@@ -368,6 +368,8 @@ def run_peaks(args):
            "dmma_in_dfma_warp_instr": (fma / 32) / p["dmma_per_s"],
            "interleaved_tflops": 2 * (256 * p["dmma_per_s_interleaved"] + p["dfma_per_s_interleaved"]) / 1e12,
            "interleaved_cycles_per_group_per_scheduler": sched * mhz * 1e6 / p["dmma_per_s_interleaved"],
+           "imma_cycles_per_instr_per_scheduler": sched * mhz * 1e6 / p["imma_s8_m16n8k32_per_s"],
+           "hmma_cycles_per_instr_per_scheduler": sched * mhz * 1e6 / p["hmma_f16_m16n8k16_per_s"],
            "libm_exp_cost_in_dfma": fma / p["libm_exp_per_s"],
            "libm_log_cost_in_dfma": fma / p["libm_log_per_s"]}
     print(json.dumps(out))

@@ -259,14 +259,17 @@ int ck_measure_fp64_peak(double *fma_per_s, void *stream);
 
 /* The FP64 microbenchmarks behind the roofline and the sparse-vs-dense design decision
  * (DESIGN.md section 6), each kernel timed alone with CUDA events on
- * `stream` (best of 5).  Writes 8 doubles to the HOST array `out`:
+ * `stream` (best of 5).  Writes 10 doubles to the HOST array `out`:
  *   [0] DFMA           thread-level instructions / s (= ck_measure_fp64_peak)
  *   [1] DMMA.8x8x4     warp-level instructions / s, alone (one = 256 FMA = 8 warp-wide DFMA)
  *   [2] DMMA.8x8x4     warp-level instructions / s when 4 independent DFMA follow each DMMA
  *   [3] DFMA           thread-level instructions / s in that same interleaved stream
  *   [4] exp()  [5] log()   CUDA libm calls / s (thread level): the costs the survey's roofline
  *                          accounting charges for an exponential / a logarithm
- *   [6] number of SMs  [7] 0 (reserved)
+ *   [6] number of SMs
+ *   [7] legacy mma.sync int8 m16n8k32, [8] legacy mma.sync fp16 m16n8k16 (fp32 accumulate): warp-level
+ *       instructions / s -- the paths an error-free splitting of M = C E onto low-precision tensor
+ *       cores would run on (measured to decide against it)   [9] 0 (reserved)
  * Returns CK_OK, CK_EINVAL (NULL out) or CK_ECUDA. */
 int ck_measure_peaks(double *out, void *stream);
 

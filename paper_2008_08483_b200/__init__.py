@@ -180,11 +180,11 @@ def ck_measure_fp64_peak(stream=0) -> float:
 
 def ck_measure_peaks(stream=0) -> dict:
     """The FP64 microbenchmarks of include/ck.h, by name."""
-    out = (C.c_double * 8)()
+    out = (C.c_double * 10)()
     _check(_lib.ck_measure_peaks(out, stream or None))
     return {"dfma_per_s": out[0], "dmma_per_s": out[1], "dmma_per_s_interleaved": out[2],
             "dfma_per_s_interleaved": out[3], "libm_exp_per_s": out[4], "libm_log_per_s": out[5],
-            "sms": int(out[6])}
+            "sms": int(out[6]), "imma_s8_m16n8k32_per_s": out[7], "hmma_f16_m16n8k16_per_s": out[8]}
 
 
 # ---- convenience wrapper -----------------------------------------------------------------

@@ -164,7 +164,7 @@ cudaError_t launch_rk4_stage(int stage, const ck_mech *m, const double *P, doubl
 // DFMA throughput microbenchmark (thread-level FMA instructions per second), ck_peaks.cu.
 cudaError_t measure_fp64_peak(double *fma_per_s, cudaStream_t stream);
 // All FP64 microbenchmarks of ck_peaks.cu; out as documented at ck_measure_peaks in ck.h.
-#define CK_N_PEAKS 8
+#define CK_N_PEAKS 10
 cudaError_t measure_peaks(double out[CK_N_PEAKS], cudaStream_t stream);
 
 }  // namespace ck

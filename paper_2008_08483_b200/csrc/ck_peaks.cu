@@ -78,6 +78,39 @@ __global__ void __launch_bounds__(kThreads) peak_libm(double *out, int iters, do
   if (s == 123.456) out[0] = s;
 }
 
+// legacy tensor-core paths (mma.sync): int8 m16n8k32 and fp16 m16n8k16 with fp32 accumulation, 8
+// independent accumulator sets per warp.  What an error-free splitting of M = C E onto the
+// low-precision tensor cores would run on (rejected, measured here).
+template <bool INT8>
+__global__ void __launch_bounds__(kThreads) peak_mma_legacy(double *out, int iters) {
+  unsigned a[4] = {threadIdx.x, threadIdx.x * 3u, 7u, 9u}, b[2] = {threadIdx.x * 5u, 11u};
+  int ci[8][4];
+  float cf[8][4];
+#pragma unroll
+  for (int u = 0; u < 8; ++u)
+#pragma unroll
+    for (int v = 0; v < 4; ++v) { ci[u][v] = u + v; cf[u][v] = (float)(u + v); }
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      if (INT8)
+        asm volatile("mma.sync.aligned.m16n8k32.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                     : "+r"(ci[u][0]), "+r"(ci[u][1]), "+r"(ci[u][2]), "+r"(ci[u][3])
+                     : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
+      else
+        asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                     : "+f"(cf[u][0]), "+f"(cf[u][1]), "+f"(cf[u][2]), "+f"(cf[u][3])
+                     : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
+    }
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int u = 0; u < 8; ++u)
+#pragma unroll
+    for (int v = 0; v < 4; ++v) s += INT8 ? (double)ci[u][v] : (double)cf[u][v];
+  if (s == 123.456) out[0] = s;
+}
+
 template <typename F>
 cudaError_t best_ms(F launch, cudaStream_t stream, double *ms_out) {
   cudaEvent_t t0, t1;
@@ -140,6 +173,13 @@ cudaError_t measure_peaks(double out[CK_N_PEAKS], cudaStream_t stream) {
     e = best_ms([&](int it) { peak_libm<true><<<blocks, kThreads, 0, stream>>>(d_out, it, 1e-3, 1.5); }, stream, &ms);
   if (e == cudaSuccess) out[5] = threads * kIters * 4.0 / (ms * 1e-3);
   out[6] = (double)sms;
+  // [7], [8] legacy mma.sync: int8 m16n8k32 and fp16 m16n8k16, warp-level instructions per second
+  if (e == cudaSuccess)
+    e = best_ms([&](int it) { peak_mma_legacy<true><<<blocks, kThreads, 0, stream>>>(d_out, it); }, stream, &ms);
+  if (e == cudaSuccess) out[7] = warps * kIters * 8.0 / (ms * 1e-3);
+  if (e == cudaSuccess)
+    e = best_ms([&](int it) { peak_mma_legacy<false><<<blocks, kThreads, 0, stream>>>(d_out, it); }, stream, &ms);
+  if (e == cudaSuccess) out[8] = warps * kIters * 8.0 / (ms * 1e-3);
   cudaFree(d_out);
   return e;
 }
