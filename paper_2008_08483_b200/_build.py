@@ -12,8 +12,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libck.so")
-SOURCES = ["ck_api.cu", "ck_kernels.cu", "ck_jit.cu", "ck_rk4.cu", "ck_jac.cu", "ck_peaks.cu", "ck_nu.cu"]
-HEADERS = ["ck_internal.h", "ck_program.h", "ck_jit_kernel.cuh", "ck_jit_math.cuh", "ck_nu_kernel.cuh", "ck_jac_v2.cuh"]
+SOURCES = ["ck_api.cu", "ck_kernels.cu", "ck_jit.cu", "ck_rk4.cu", "ck_jac.cu", "ck_peaks.cu", "ck_nu.cu", "ck_jacj.cu"]
+HEADERS = ["ck_internal.h", "ck_program.h", "ck_jit_kernel.cuh", "ck_jit_math.cuh", "ck_nu_kernel.cuh", "ck_jac_v2.cuh", "ck_jacj_kernel.cuh"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC"]
 
@@ -28,7 +28,8 @@ def _embed_jit_source() -> None:
     //@@CK_MATH@@ line) -> ck_jit_source.inc, ck_nu_source.inc: the kernel texts as C++ raw string
     literals (what NVRTC compiles at ck_mech_create time)."""
     math = open(os.path.join(CSRC, "ck_jit_math.cuh")).read()
-    for src, dst in (("ck_jit_kernel.cuh", "ck_jit_source.inc"), ("ck_nu_kernel.cuh", "ck_nu_source.inc")):
+    for src, dst in (("ck_jit_kernel.cuh", "ck_jit_source.inc"), ("ck_nu_kernel.cuh", "ck_nu_source.inc"),
+                     ("ck_jacj_kernel.cuh", "ck_jacj_source.inc")):
         text = open(os.path.join(CSRC, src)).read()
         assert text.count("//@@CK_MATH@@") == 1
         line = [l for l in text.splitlines() if l.startswith("//@@CK_MATH@@")][0]
@@ -50,7 +51,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
     newest_header = max(os.path.getmtime(f) for f in
-                        [os.path.join(CSRC, h) for h in HEADERS + ["ck_jit_source.inc"]] +
+                        [os.path.join(CSRC, h) for h in HEADERS + ["ck_jit_source.inc", "ck_nu_source.inc", "ck_jacj_source.inc"]] +
                         [os.path.join(INCLUDE, "ck.h")])
 
     def compile_one(src):

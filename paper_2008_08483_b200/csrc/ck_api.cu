@@ -274,6 +274,7 @@ std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk,
   if (const char *e = std::getenv("CK_JIT_MHINT")) spec.m_hint = std::atoi(e) != 0;
   if (const char *e = std::getenv("CK_JIT_SYNC")) spec.sync_every = std::atoi(e);
   if (const char *e = std::getenv("CK_JIT_KCONST")) spec.kconst = std::atoi(e) != 0;
+  spec.straight = env_int("CK_JIT_STRAIGHT", 0);
   // (CK_JIT_KC=none, the ablation that removes the equilibrium layer, changes the RESULT: it is
   //  honoured only together with CK_ALLOW_ABLATION=1, see setup_jit, and shows in ck_mech_info 18)
   if (const char *e = std::getenv("CK_JIT_KC")) spec.kc_none = std::string(e) == "none";
@@ -858,6 +859,22 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
     const std::string err = ck::jac_create(d, m->num_sms, (size_t)prop.sharedMemPerBlockOptin, &m->jac);
     if (!err.empty()) { ck_mech_destroy(m); return fail(CK_ECUDA, err); }
   }
+  // ---- the mechanism-specialised Jacobian kernel (ck_jacj.cu); CK_JAC_KERNEL=v1|v2 keeps the
+  //      table-driven ones, =v3 requires this one --------------------------------------------
+  {
+    const char *e = std::getenv("CK_JAC_KERNEL");
+    const std::string which = e ? e : "";
+    if (which != "v1" && which != "v2" && m->jac) {
+      m->jacj_note = ck::jacj_create(d, spec, hb.jit_tab, m->jit_params.thermo, m->jit_params.logtab,
+                                     m->jit_params.eff_frag, m->device, m->num_sms,
+                                     (size_t)prop.sharedMemPerBlockOptin, &m->jacj);
+      if (!m->jacj && which == "v3") {
+        const std::string why = m->jacj_note;
+        ck_mech_destroy(m);
+        return fail(CK_EUNSUPPORTED, "CK_JAC_KERNEL=v3 but " + why);
+      }
+    }
+  }
   *out = m;
   return CK_OK;
 }
@@ -868,6 +885,7 @@ extern "C" void ck_mech_destroy(ck_mech *m) {
   if (m->d_scratch) cudaFree(m->d_scratch);
   if (m->d_slot_busy) cudaFree(m->d_slot_busy);
   ck::jac_destroy(m->jac);
+  ck::jacj_destroy(m->jacj);
   ck::nu_destroy(m->nu);
   if (m->d_stage) cudaFree(m->d_stage);
   if (m->host_in) cudaStreamDestroy(m->host_in);
@@ -938,7 +956,8 @@ extern "C" int ck_jacobian(const ck_mech *m, const double *T, const double *P, c
   if (!m->jac)
     return fail(CK_EUNSUPPORTED, "ck_jacobian: not available for this mechanism (approximate-ANN Kc, S > 127, "
                                  "or the tile does not fit shared memory)");
-  const cudaError_t ce = ck::jac_launch(m->jac, T, P, Y, N, J, (cudaStream_t)stream);
+  const cudaError_t ce = m->jacj ? ck::jacj_launch(m->jacj, T, P, Y, N, J, (cudaStream_t)stream)
+                                 : ck::jac_launch(m->jac, T, P, Y, N, J, (cudaStream_t)stream);
   if (ce != cudaSuccess) return fail_cuda(ce, "ck_jacobian launch");
   return CK_OK;
 }
@@ -1154,7 +1173,7 @@ extern "C" int64_t ck_mech_info(const ck_mech *m, int what) {
     case 13: return m->nnz_eff;
     case 14: return m->jit_kernel ? 1 : 0;
     case 15: return m->jit_kernel ? m->jit_s_reg : 0;
-    case 16: return m->jac ? ck::jac_cells_per_tile(m->jac) : 0;
+    case 16: return m->jacj ? ck::jacj_cells(m->jacj) : (m->jac ? ck::jac_cells_per_tile(m->jac) : 0);
     case 17: return (m->jit_kernel && m->jit_spec.pair) ? 1 : 0;
     case 18: return (m->jit_kernel && m->jit_spec.kc_none) ? 1 : 0;
     case 19: return m->jit_kernel ? m->jit_spec.prec : 0;
@@ -1173,6 +1192,11 @@ extern "C" int64_t ck_mech_jit_source(const ck_mech_desc *d, char *buf, int64_t 
   if (!hb.jit_why.empty()) { fail(CK_EUNSUPPORTED, hb.jit_why); return -1; }
   // (CK_JIT_SOURCE_SPLIT=K: the text of the small-batch shape instead, for offline inspection)
   if (const int k = env_int("CK_JIT_SOURCE_SPLIT", 0)) { hb.spec.split = k; hb.spec.threads = 256; hb.spec.min_blocks = 1; }
+  // (CK_JACJ_DUMP=path: also write the text of the specialised Jacobian kernel there)
+  if (std::getenv("CK_JACJ_DUMP")) {
+    ck::JacJit *jj = nullptr;
+    ck::jacj_create(d, hb.spec, hb.jit_tab, nullptr, nullptr, nullptr, -1, 148, kSmemPerBlock, &jj);
+  }
   const std::string src = ck::jit_generate_source(hb.spec);
   if (buf && cap > 0) {
     const size_t n = std::min((size_t)cap - 1, src.size());

@@ -60,6 +60,7 @@ struct JitSpec {
   std::vector<double> ann_const;   // mean | 1/std | W_in | B | W_hid
   int lut_rep = 1;             // interleaved copies of the exp table (16: conflict-free lookups)
   bool kconst = false;         // polynomial coefficients as constant-bank operands (else literals)
+  int straight = 0;            // n > 0: the reaction walk in straight-line code, rate core inlined per block (measurement knob CK_JIT_STRAIGHT)
   int group_end[6] = {0, 0, 0, 0, 0, 0};   // end block of (elementary, three-body, falloff) x (rev, irrev)
   std::vector<JitReaction> rxn;
   std::vector<double> inv_W, range_T, falloff;   // constant-bank tables
@@ -72,6 +73,18 @@ void jac_destroy(JacMech *jm);
 int jac_cells_per_tile(const JacMech *jm);
 cudaError_t jac_launch(const JacMech *jm, const double *T, const double *P, const double *Y, int64_t N,
                        double *J, cudaStream_t stream);
+
+// The mechanism-specialised Jacobian kernel (ck_jacj.cu / ck_jacj_kernel.cuh), NVRTC-compiled.
+// jacj_create returns "" and sets *out, or returns why the kernel is not available (*out NULL; the
+// table-driven kernels of ck_jac.cu remain).  device < 0: only generate the source (CK_JACJ_DUMP).
+struct JacJit;
+std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::vector<double> &tab10,
+                        const double *d_thermo, const double *d_logtab, const double *d_eff_frag, int device,
+                        int num_sms, size_t smem_blk, JacJit **out);
+void jacj_destroy(JacJit *jj);
+int jacj_cells(const JacJit *jj);
+cudaError_t jacj_launch(const JacJit *jj, const double *T, const double *P, const double *Y, int64_t N, double *J,
+                        cudaStream_t stream);
 
 // The all-DMMA small-mechanism kernel (ck_nu.cu / ck_nu_kernel.cuh).
 struct NuMech;
@@ -128,6 +141,8 @@ struct ck_mech {
   std::string jit_note;       // why the specialised kernel is not in use, if so
   // analytic Jacobian (ck_jacobian): NULL if unsupported for this mechanism
   ck::JacMech *jac = nullptr;
+  ck::JacJit *jacj = nullptr;   // the mechanism-specialised Jacobian kernel, used when present
+  std::string jacj_note;        // why it is not, if so
   // all-DMMA small-mechanism kernel (CK_JIT_NU=dmma), used by ck_source_terms when present
   ck::NuMech *nu = nullptr;
   // staging for ck_source_terms_host

@@ -1,0 +1,353 @@
+// ck_jacj.cu -- host side of the mechanism-specialised Jacobian kernel (ck_jacj_kernel.cuh):
+// generates the unique code (reaction walk, column walk, one case per row of J) into the kernel
+// text, compiles it with NVRTC (ck_jit.cu), builds the tables of the dense part and launches.
+// The reaction order, the folded rate rows and the M = C E fragments are the source-term
+// kernel's (ck_api.cu: finalize_jit), so both kernels agree on what "reaction jj" is.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <sstream>
+#include <string>
+#include <vector>
+
+#include "ck_internal.h"
+
+namespace ck {
+
+namespace {
+
+const char *kJacjText =
+#include "ck_jacj_source.inc"
+    ;
+
+struct CjCoef { double dnu; int tb, pad; };
+
+// must match CjParams in ck_jacj_kernel.cuh field for field
+struct JacjParams {
+  const double *eff_frag, *tab, *thermo, *logtab, *bfrag;
+  const CjCoef *coef;
+  double *scratch;
+  const double *T, *P, *Y;
+  double *J;
+  long long N;
+  int tile_cells;
+};
+
+std::string lit(double v) {
+  char buf[40];
+  std::snprintf(buf, sizeof buf, "%.17g", v);
+  std::string s(buf);
+  if (s.find_first_of(".eEni") == std::string::npos) s += ".0";
+  return s;
+}
+
+// acc = acc + c * v as source text, c a literal
+std::string fma_line(const std::string &acc, double c, const std::string &v) {
+  if (c == 1.0) return acc + " += " + v + ";";
+  if (c == -1.0) return acc + " -= " + v + ";";
+  return acc + " = fma(" + lit(c) + ", " + v + ", " + acc + ");";
+}
+
+std::string gather_expr(const std::vector<std::pair<int, double>> &side) {
+  if (side.empty()) return "0.0";
+  std::string e;
+  for (size_t i = 0; i < side.size(); ++i) {
+    const std::string c = "CJ_LNC(" + std::to_string(side[i].first) + ")";
+    const double nu = side[i].second;
+    if (i == 0) e = (nu == 1.0) ? c : (lit(nu) + " * " + c);
+    else e = (nu == 1.0) ? (e + " + " + c) : ("fma(" + lit(nu) + ", " + c + ", " + e + ")");
+  }
+  return e;
+}
+
+}  // namespace
+
+struct JacJit {
+  cudaLibrary_t lib = nullptr;
+  cudaKernel_t kernel = nullptr;
+  JacjParams prm{};
+  void *d_blob = nullptr;
+  double *d_scratch = nullptr;
+  int threads = 0, grid_max = 1;
+  size_t smem = 0;
+};
+
+// Returns "" on success (*out set), or the reason the kernel is not available for this mechanism
+// (*out NULL; never an error: the table-driven kernels remain).
+std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::vector<double> &tab10,
+                        const double *d_thermo, const double *d_logtab, const double *d_eff_frag, int device,
+                        int num_sms, size_t smem_blk, JacJit **out) {
+  *out = nullptr;
+  const int S = spec.S, RP = spec.R, R = d->n_reactions, B = spec.block;
+  if (spec.kc_ann || spec.prec != 0) return "approximate-ANN Kc / reduced precision";
+  if (!spec.perm.empty() || spec.pair) return "species permuted (accumulators do not fit registers)";
+  if (S > 53) return "S > 53: two columns of register accumulators do not fit";
+  if ((int)spec.rxn.size() != RP || RP % B) return "inconsistent reaction list";
+  const int n_ranges = spec.n_ranges, nblk = RP / B, n1 = S + 1;
+  if (spec.tab_ranges != n_ranges || spec.row != 10) return "rate table layout";
+  const int ntl = (S + 7) / 8;
+  int ost = std::max(n1, 8 * ntl);
+  while (ost % 4 != 2) ++ost;                      // rows 16-byte aligned, 128-bit row accesses conflict-free
+  const bool bulk = (n1 % 2 == 0) && !(std::getenv("CK_JACJ_BULK") && std::atoi(std::getenv("CK_JACJ_BULK")) == 0);
+
+  // ---- launch shape: the most warps (tile = 32 cells per warp) whose tile fits shared memory ----
+  int warps = 0;
+  size_t smem = 0;
+  int w_max = 8;
+  if (const char *e = std::getenv("CK_JACJ_WARPS")) w_max = std::min(8, std::max(1, std::atoi(e)));
+  for (int w = w_max; w >= 1; --w) {
+    const size_t ovl = std::max((size_t)n_ranges * RP * 16 + 384, (size_t)w * 32 * ost);
+    const size_t doubles = (size_t)S * (32 * w + 8) + (size_t)n_ranges * S * 12 + ovl;
+    if (doubles * 8 + 64 <= smem_blk) { warps = w; smem = doubles * 8; break; }
+  }
+  if (!warps) return "tile does not fit shared memory";
+  const int NT = 32 * warps;
+
+  // ---- rate table rows of 16 doubles ----------------------------------------------------------
+  std::vector<double> range_T = spec.range_T;
+  std::vector<int> rank(S);
+  for (int k = 0; k < S; ++k)
+    rank[k] = (int)(std::lower_bound(range_T.begin(), range_T.end(), d->T_mid[k]) - range_T.begin());
+  std::vector<double> tab16((size_t)n_ranges * RP * 16, 0.0);
+  for (int rg = 0; rg < n_ranges; ++rg)
+    for (int jj = 0; jj < RP; ++jj) {
+      const double *src = &tab10[((size_t)rg * RP + jj) * 10];
+      double *row = &tab16[((size_t)rg * RP + jj) * 16];
+      for (int i = 0; i < 10; ++i) row[i] = src[i];
+      const JitReaction &r = spec.rxn[jj];
+      long double ordf = 0, ordr = 0, da1 = 0;
+      for (const auto &e : r.reac) ordf += e.second;
+      for (const auto &e : r.prod) ordr += e.second;
+      for (const auto &e : r.net) {
+        const int k = e.first;
+        const double *a = (rg > rank[k]) ? d->nasa_hi + 7 * k : d->nasa_lo + 7 * k;
+        da1 += (long double)e.second * a[0];
+      }
+      row[10] = (double)ordf; row[11] = (double)ordr;
+      row[12] = 2.0 * row[7]; row[13] = 3.0 * row[8]; row[14] = 4.0 * row[9];
+      row[15] = (double)da1;
+    }
+
+  // ---- dense part: k-steps of 4 third-body / falloff reactions per row, E gathered as B fragments ----
+  std::vector<int> ks_start(S + 2, 0);
+  std::vector<CjCoef> coef;
+  std::vector<double> bfrag;
+  for (int i = 0; i <= S; ++i) {
+    ks_start[i] = (int)coef.size() / 4;
+    std::vector<std::pair<int, double>> tbs;   // (padded reaction index, coefficient)
+    for (int jj = 0; jj < RP; ++jj) {
+      const JitReaction &r = spec.rxn[jj];
+      if (r.index < 0 || r.m_slot < 0) continue;
+      if (i == S) { tbs.emplace_back(jj, 1.0); continue; }
+      for (const auto &e : r.net)
+        if (e.first == i && e.second != 0.0) tbs.emplace_back(jj, e.second);
+    }
+    const int nks = ((int)tbs.size() + 3) / 4;
+    for (int ks = 0; ks < nks; ++ks) {
+      const size_t b0 = bfrag.size();
+      bfrag.resize(b0 + (size_t)ntl * 32, 0.0);
+      for (int qq = 0; qq < 4; ++qq) {
+        const int kk = 4 * ks + qq;
+        if (kk >= (int)tbs.size()) { coef.push_back(CjCoef{0.0, -1, 0}); continue; }
+        const JitReaction &r = spec.rxn[tbs[kk].first];
+        coef.push_back(CjCoef{tbs[kk].second, r.m_slot, 0});
+        for (int nt = 0; nt < ntl; ++nt)
+          for (int gg = 0; gg < 8; ++gg) {
+            const int l = 8 * nt + gg;
+            if (l < S)
+              bfrag[b0 + (size_t)nt * 32 + gg * 4 + qq] =
+                  (d->eff ? d->eff[(size_t)l * R + r.index] : 1.0) / d->mol_weight[l];
+          }
+      }
+    }
+  }
+  ks_start[S + 1] = (int)coef.size() / 4;
+  if (coef.empty()) coef.push_back(CjCoef{0.0, -1, 0});
+  if (bfrag.empty()) bfrag.push_back(0.0);
+
+  // ---- source text -------------------------------------------------------------------------------
+  std::ostringstream o;
+  o << "#define CJ_S " << S << "\n#define CJ_R " << RP << "\n#define CJ_NT " << NT << "\n#define CJ_NRANGES " << n_ranges
+    << "\n#define CJ_B " << B << "\n#define CJ_NBLK " << nblk << "\n#define CJ_G_TB0 " << spec.group_end[1]
+    << "\n#define CJ_G_FO0 " << spec.group_end[3] << "\n#define CJ_NM " << spec.n_m << "\n#define CJ_NMB " << spec.n_mb
+    << "\n#define CJ_NFO " << spec.n_fo << "\n#define CJ_NTL " << ntl << "\n#define CJ_OST " << ost
+    << "\n#define CJ_BULK " << (bulk ? 1 : 0) << "\n";
+  auto emit = [&](const char *name, const std::vector<double> &v) {
+    o << "__constant__ double " << name << "[" << (v.empty() ? 1 : v.size()) << "] = {";
+    for (size_t i = 0; i < v.size(); ++i) o << (i ? "," : "") << (i % 6 == 0 ? "\n  " : " ") << lit(v[i]);
+    if (v.empty()) o << "0.0";
+    o << "};\n";
+  };
+  emit("ck_c_rangeT", spec.range_T);
+  emit("ck_c_falloff", spec.falloff);
+  {
+    std::vector<double> iw(S);
+    for (int k = 0; k < S; ++k) iw[k] = 1.0 / d->mol_weight[k];
+    emit("cj_c_invW", iw);
+  }
+  o << "__constant__ int cj_c_ks[" << S + 2 << "] = {";
+  for (int i = 0; i < S + 2; ++i) o << (i ? ", " : "") << ks_start[i];
+  o << "};\n";
+  const std::string text(kJacjText);
+  const std::string marker = "//@@CJ_GENERATED@@";
+  const size_t at = text.find(marker);
+  o << text.substr(0, at);
+
+  const char *names[6] = {"cj_core<0, 1>", "cj_core<0, 0>", "cj_core<1, 1>", "cj_core<1, 0>", "cj_core<2, 1>", "cj_core<2, 0>"};
+  // P1: one switch case per loop trip: energy-row scatters of the previous block, gathers of this one
+  o << "__device__ __forceinline__ void cj_reactions(const CjCtx &x, double (&er)[CJ_S], double (&sc)[4]) {\n"
+    << "  double gf[CJ_B], gr[CJ_B], ha[CJ_B], hb[CJ_B];\n"
+    << "#pragma unroll 1\n  for (int blk = 0; blk <= CJ_NBLK; ++blk) {\n    switch (blk) {\n";
+  for (int k = 0; k <= nblk; ++k) {
+    o << "      case " << k << ":\n";
+    if (k > 0)
+      for (int bb = 0; bb < B; ++bb) {
+        const JitReaction &r = spec.rxn[(size_t)(k - 1) * B + bb];
+        for (const auto &e : r.reac)
+          o << "        " << fma_line("er[" + std::to_string(e.first) + "]", e.second, "ha[" + std::to_string(bb) + "]") << "\n";
+        if (r.reversible)
+          for (const auto &e : r.prod)
+            o << "        " << fma_line("er[" + std::to_string(e.first) + "]", -e.second, "hb[" + std::to_string(bb) + "]") << "\n";
+      }
+    if (k < nblk)
+      for (int bb = 0; bb < B; ++bb) {
+        const JitReaction &r = spec.rxn[(size_t)k * B + bb];
+        o << "        gf[" << bb << "] = " << gather_expr(r.reac) << ";";
+        if (r.index >= 0) o << "  // reaction " << r.index;
+        o << "\n        gr[" << bb << "] = " << (r.reversible ? gather_expr(r.prod) : std::string("0.0")) << ";\n";
+      }
+    o << "        break;\n";
+  }
+  o << "    }\n";
+  {
+    bool first = true;
+    for (int g = 0; g < 6; ++g) {
+      const int lo = g ? spec.group_end[g - 1] : 0;
+      if (spec.group_end[g] == lo) continue;
+      o << "    " << (first ? "if" : "else if") << " (blk < " << spec.group_end[g] << ") " << names[g]
+        << "(x, blk, gf, gr, ha, hb, sc);\n";
+      first = false;
+    }
+  }
+  o << "  }\n}\n";
+  // P1b: tc_i = sum_j dnu_ij t_j, gc_i = sum_j dnu_ij e_j
+  o << "__device__ __forceinline__ void cj_columns(const CjCtx &x, double (&tc)[CJ_S], double (&gc)[CJ_S]) {\n"
+    << "#pragma unroll 1\n  for (int blk = 0; blk < CJ_NBLK; ++blk) {\n    double t[CJ_B], e[CJ_B];\n"
+    << "#pragma unroll\n    for (int b = 0; b < CJ_B; ++b) { t[b] = CJ_SCR(CJ_OFF_T, blk * CJ_B + b); e[b] = CJ_SCR(CJ_OFF_E, blk * CJ_B + b); }\n"
+    << "    switch (blk) {\n";
+  for (int k = 0; k < nblk; ++k) {
+    o << "      case " << k << ":\n";
+    for (int bb = 0; bb < B; ++bb) {
+      const JitReaction &r = spec.rxn[(size_t)k * B + bb];
+      for (const auto &e : r.net) {
+        o << "        " << fma_line("tc[" + std::to_string(e.first) + "]", e.second, "t[" + std::to_string(bb) + "]") << " "
+          << fma_line("gc[" + std::to_string(e.first) + "]", e.second, "e[" + std::to_string(bb) + "]") << "\n";
+      }
+    }
+    o << "        break;\n";
+  }
+  o << "    }\n  }\n}\n";
+  // P2: sparse part of row i: for every reaction with dnu_ij != 0 the entries dnu_ij nu'_lj a_j - dnu_ij nu''_lj b_j
+  o << "__device__ __forceinline__ void cj_row_sparse(const CjCtx &x, const int i, double (&acc)[CJ_S]) {\n  switch (i) {\n";
+  for (int i = 0; i < S; ++i) {
+    o << "    case " << i << ": {\n";
+    for (int jj = 0; jj < RP; ++jj) {
+      const JitReaction &r = spec.rxn[jj];
+      if (r.index < 0) continue;
+      double dnu = 0.0;
+      for (const auto &e : r.net) if (e.first == i) dnu = e.second;
+      if (dnu == 0.0) continue;
+      o << "      { const double a = CJ_A(" << jj << ")";
+      if (r.reversible) o << ", b = CJ_Bq(" << jj << ")";
+      o << ";\n";
+      for (const auto &e : r.reac) o << "        " << fma_line("acc[" + std::to_string(e.first) + "]", dnu * e.second, "a") << "\n";
+      if (r.reversible)
+        for (const auto &e : r.prod) o << "        " << fma_line("acc[" + std::to_string(e.first) + "]", -dnu * e.second, "b") << "\n";
+      o << "      }\n";
+    }
+    o << "    } break;\n";
+  }
+  o << "  }\n}\n";
+  o << text.substr(at + marker.size());
+  const std::string src = o.str();
+  if (const char *e = std::getenv("CK_JACJ_DUMP")) {
+    if (FILE *f = std::fopen(e, "w")) {
+      std::fwrite(src.data(), 1, src.size(), f);
+      std::fclose(f);
+    }
+  }
+  if (device < 0) return "source only";
+
+  // ---- compile, load ---------------------------------------------------------------------------------
+  JacJit *jj = new JacJit;
+  std::vector<char> cubin;
+  cudaError_t ce = cudaSuccess;
+  for (int attempt = 0; attempt < 2; ++attempt) {
+    const std::string err = jit_compile(src, &cubin, attempt == 0);
+    if (!err.empty()) { delete jj; return err; }
+    ce = cudaLibraryLoadData(&jj->lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
+    if (ce == cudaSuccess) break;
+    cudaGetLastError();
+    jj->lib = nullptr;
+  }
+  if (ce == cudaSuccess) ce = cudaLibraryGetKernel(&jj->kernel, jj->lib, "ck_jacobian_jit");
+  if (ce == cudaSuccess)
+    ce = cudaKernelSetAttributeForDevice(jj->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem, device);
+  // ---- tables and scratch ------------------------------------------------------------------------------
+  size_t o_tab = 0, o_bf = 0, o_co = 0, bytes = 0;
+  auto place = [&](size_t n) { const size_t off = (bytes + 255) / 256 * 256; bytes = off + n; return off; };
+  o_tab = place(tab16.size() * 8); o_bf = place(bfrag.size() * 8); o_co = place(coef.size() * sizeof(CjCoef));
+  if (ce == cudaSuccess) ce = cudaMalloc(&jj->d_blob, bytes);
+  if (ce == cudaSuccess) ce = cudaMemcpy((char *)jj->d_blob + o_tab, tab16.data(), tab16.size() * 8, cudaMemcpyHostToDevice);
+  if (ce == cudaSuccess) ce = cudaMemcpy((char *)jj->d_blob + o_bf, bfrag.data(), bfrag.size() * 8, cudaMemcpyHostToDevice);
+  if (ce == cudaSuccess) ce = cudaMemcpy((char *)jj->d_blob + o_co, coef.data(), coef.size() * sizeof(CjCoef), cudaMemcpyHostToDevice);
+  const size_t scr_rows = (size_t)4 * RP + (size_t)2 * spec.n_mb * 8 + (size_t)3 * S;
+  if (ce == cudaSuccess) ce = cudaMalloc((void **)&jj->d_scratch, (size_t)num_sms * scr_rows * NT * sizeof(double));
+  if (ce != cudaSuccess) {
+    const std::string msg = std::string("specialised Jacobian kernel: ") + cudaGetErrorString(ce);
+    cudaGetLastError();
+    jacj_destroy(jj);
+    return msg;
+  }
+  jj->threads = NT; jj->grid_max = num_sms; jj->smem = smem;
+  jj->prm.eff_frag = d_eff_frag; jj->prm.thermo = d_thermo; jj->prm.logtab = d_logtab;
+  jj->prm.tab = (const double *)((char *)jj->d_blob + o_tab);
+  jj->prm.bfrag = (const double *)((char *)jj->d_blob + o_bf);
+  jj->prm.coef = (const CjCoef *)((char *)jj->d_blob + o_co);
+  jj->prm.scratch = jj->d_scratch;
+  *out = jj;
+  return "";
+}
+
+void jacj_destroy(JacJit *jj) {
+  if (!jj) return;
+  if (jj->d_blob) cudaFree(jj->d_blob);
+  if (jj->d_scratch) cudaFree(jj->d_scratch);
+  if (jj->lib) cudaLibraryUnload(jj->lib);
+  delete jj;
+}
+
+int jacj_cells(const JacJit *jj) { return jj->threads; }
+
+cudaError_t jacj_launch(const JacJit *jj, const double *T, const double *P, const double *Y, int64_t N, double *J,
+                        cudaStream_t stream) {
+  JacjParams prm = jj->prm;
+  prm.T = T; prm.P = P; prm.Y = Y; prm.J = J; prm.N = N;
+  // balanced tiles, as for the source-term kernel: the fewest waves of full tiles, then the tile size
+  // (a multiple of 32) that spreads the cells evenly over grid x waves
+  const int64_t per_wave = (int64_t)jj->grid_max * jj->threads;
+  const int64_t waves = (N + per_wave - 1) / per_wave;
+  int64_t tc = (N + waves * jj->grid_max - 1) / (waves * jj->grid_max);
+  tc = std::min<int64_t>(jj->threads, (tc + 31) / 32 * 32);
+  prm.tile_cells = (int)tc;
+  const int64_t tiles = (N + tc - 1) / tc;
+  const int grid = (int)std::min<int64_t>(tiles, jj->grid_max);
+  void *args[] = {&prm};
+  return cudaLaunchKernel((const void *)jj->kernel, dim3(grid), dim3(jj->threads), args, jj->smem, stream);
+}
+
+}  // namespace ck

@@ -264,6 +264,20 @@ std::string jit_generate_source(const JitSpec &s) {
       o << "        break;\n";
     }
     o << "    }\n  }\n}\n";
+  } else if (!s.pair && s.straight > 0 && s.tab_in_smem) {
+    // Straight-line walk: gathers, the rate core (inlined with the block number as a literal)
+    // and scatters of every block one after the other, no loop, no switch: the instruction
+    // stream is sequential, so the fetch unit's prefetcher can run ahead of it.
+    for (int k = 0; k < nblk; ++k) {
+      int g = 0;
+      while (k >= s.group_end[g]) ++g;
+      o << "  {\n";
+      gathers(k);
+      o << "    " << names[g] << "(x, " << k << ", 0, gf, gr, q);\n";
+      scatters(k, -1, "q[");
+      o << "  }\n";
+    }
+    o << "}\n";
   } else if (!s.pair) {
     // One switch case per loop trip: the scatters of the previous block (Eq. 2) and the
     // gathers of this one (Eq. 4), so that the unique code is walked in address order with one
