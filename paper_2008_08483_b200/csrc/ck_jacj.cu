@@ -29,7 +29,6 @@ struct CjCoef { double dnu; int tb, pad; };
 // must match CjParams in ck_jacj_kernel.cuh field for field
 struct JacjParams {
   const double *eff_frag, *tab, *thermo, *logtab, *bfrag;
-  const CjCoef *coef;
   double *scratch;
   const double *T, *P, *Y;
   double *J;
@@ -86,12 +85,14 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
   if (spec.kc_ann || spec.prec != 0) return "approximate-ANN Kc / reduced precision";
   if (!spec.perm.empty() || spec.pair) return "species permuted (accumulators do not fit registers)";
   if (S > 53) return "S > 53: two columns of register accumulators do not fit";
+  if (spec.n_m > 640) return "too many third-body reactions for the constant-bank k-slot tables";
   if ((int)spec.rxn.size() != RP || RP % B) return "inconsistent reaction list";
   const int n_ranges = spec.n_ranges, nblk = RP / B, n1 = S + 1;
   if (spec.tab_ranges != n_ranges || spec.row != 10) return "rate table layout";
   const int ntl = (S + 7) / 8;
   int ost = std::max(n1, 8 * ntl);
   while (ost % 4 != 2) ++ost;                      // rows 16-byte aligned, 128-bit row accesses conflict-free
+  const int hint = std::getenv("CK_JACJ_HINT") ? std::atoi(std::getenv("CK_JACJ_HINT")) : 1;
   const bool bulk = (n1 % 2 == 0) && !(std::getenv("CK_JACJ_BULK") && std::atoi(std::getenv("CK_JACJ_BULK")) == 0);
 
   // ---- launch shape: the most warps (tile = 32 cells per warp) whose tile fits shared memory ----
@@ -106,6 +107,8 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
   }
   if (!warps) return "tile does not fit shared memory";
   const int NT = 32 * warps;
+  const int env_chunk = std::getenv("CK_JACJ_CHUNK") ? std::atoi(std::getenv("CK_JACJ_CHUNK")) : 8;
+  const int pf_rows = std::getenv("CK_JACJ_PFROWS") ? std::atoi(std::getenv("CK_JACJ_PFROWS")) : 0;
 
   // ---- rate table rows of 16 doubles ----------------------------------------------------------
   std::vector<double> range_T = spec.range_T;
@@ -175,7 +178,7 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
     << "\n#define CJ_B " << B << "\n#define CJ_NBLK " << nblk << "\n#define CJ_G_TB0 " << spec.group_end[1]
     << "\n#define CJ_G_FO0 " << spec.group_end[3] << "\n#define CJ_NM " << spec.n_m << "\n#define CJ_NMB " << spec.n_mb
     << "\n#define CJ_NFO " << spec.n_fo << "\n#define CJ_NTL " << ntl << "\n#define CJ_OST " << ost
-    << "\n#define CJ_BULK " << (bulk ? 1 : 0) << "\n";
+    << "\n#define CJ_BULK " << (bulk ? 1 : 0) << "\n#define CJ_HINT " << hint << "\n#define CJ_KP " << (std::getenv("CK_JACJ_KP") ? std::max(1, std::atoi(std::getenv("CK_JACJ_KP"))) : 4) << "\n#define CJ_PREF " << (std::getenv("CK_JACJ_PREF") ? std::atoi(std::getenv("CK_JACJ_PREF")) : 6) << "\n#define CJ_EXP " << (std::getenv("CK_JACJ_EXP") ? std::atoi(std::getenv("CK_JACJ_EXP")) : 0) << "\n";
   auto emit = [&](const char *name, const std::vector<double> &v) {
     o << "__constant__ double " << name << "[" << (v.empty() ? 1 : v.size()) << "] = {";
     for (size_t i = 0; i < v.size(); ++i) o << (i ? "," : "") << (i % 6 == 0 ? "\n  " : " ") << lit(v[i]);
@@ -192,6 +195,14 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
   o << "__constant__ int cj_c_ks[" << S + 2 << "] = {";
   for (int i = 0; i < S + 2; ++i) o << (i ? ", " : "") << ks_start[i];
   o << "};\n";
+  {
+    std::vector<double> dn(coef.size());
+    for (size_t i = 0; i < coef.size(); ++i) dn[i] = coef[i].dnu;
+    emit("cj_c_dnu", dn);
+    o << "__constant__ int cj_c_tb[" << coef.size() << "] = {";
+    for (size_t i = 0; i < coef.size(); ++i) o << (i ? "," : "") << (i % 24 == 0 ? "\n  " : " ") << std::max(coef[i].tb, 0);
+    o << "};\n";
+  }
   const std::string text(kJacjText);
   const std::string marker = "//@@CJ_GENERATED@@";
   const size_t at = text.find(marker);
@@ -237,7 +248,8 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
   // P1b: tc_i = sum_j dnu_ij t_j, gc_i = sum_j dnu_ij e_j
   o << "__device__ __forceinline__ void cj_columns(const CjCtx &x, double (&tc)[CJ_S], double (&gc)[CJ_S]) {\n"
     << "#pragma unroll 1\n  for (int blk = 0; blk < CJ_NBLK; ++blk) {\n    double t[CJ_B], e[CJ_B];\n"
-    << "#pragma unroll\n    for (int b = 0; b < CJ_B; ++b) { t[b] = CJ_SCR(CJ_OFF_T, blk * CJ_B + b); e[b] = CJ_SCR(CJ_OFF_E, blk * CJ_B + b); }\n"
+    << "#if CJ_PREF\n    if (blk + 1 < CJ_NBLK) {\n#pragma unroll\n      for (int b = 0; b < CJ_B; ++b) { CJ_PF1(&CJ_SCR(CJ_OFF_T, (blk + 1) * CJ_B + b)); CJ_PF1(&CJ_SCR(CJ_OFF_E, (blk + 1) * CJ_B + b)); }\n    }\n#endif\n"
+    << "#pragma unroll\n    for (int b = 0; b < CJ_B; ++b) { t[b] = cj_ld(&CJ_SCR(CJ_OFF_T, blk * CJ_B + b), x.ps); e[b] = cj_ld(&CJ_SCR(CJ_OFF_E, blk * CJ_B + b), x.ps); }\n"
     << "    switch (blk) {\n";
   for (int k = 0; k < nblk; ++k) {
     o << "      case " << k << ":\n";
@@ -253,20 +265,47 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
   o << "    }\n  }\n}\n";
   // P2: sparse part of row i: for every reaction with dnu_ij != 0 the entries dnu_ij nu'_lj a_j - dnu_ij nu''_lj b_j
   o << "__device__ __forceinline__ void cj_row_sparse(const CjCtx &x, const int i, double (&acc)[CJ_S]) {\n  switch (i) {\n";
-  for (int i = 0; i < S; ++i) {
-    o << "    case " << i << ": {\n";
+  const int chunk = std::max(1, env_chunk);
+  auto row_list = [&](int i) {
+    std::vector<std::pair<int, double>> rows;   // (reaction, dnu) of row i
     for (int jj = 0; jj < RP; ++jj) {
       const JitReaction &r = spec.rxn[jj];
       if (r.index < 0) continue;
       double dnu = 0.0;
       for (const auto &e : r.net) if (e.first == i) dnu = e.second;
-      if (dnu == 0.0) continue;
-      o << "      { const double a = CJ_A(" << jj << ")";
-      if (r.reversible) o << ", b = CJ_Bq(" << jj << ")";
-      o << ";\n";
-      for (const auto &e : r.reac) o << "        " << fma_line("acc[" + std::to_string(e.first) + "]", dnu * e.second, "a") << "\n";
-      if (r.reversible)
-        for (const auto &e : r.prod) o << "        " << fma_line("acc[" + std::to_string(e.first) + "]", -dnu * e.second, "b") << "\n";
+      if (dnu != 0.0) rows.emplace_back(jj, dnu);
+    }
+    return rows;
+  };
+  for (int i = 0; i < S; ++i) {
+    o << "    case " << i << ": {\n";
+    const std::vector<std::pair<int, double>> rows = row_list(i);
+    // the next row's (a, b) towards L2 (the scratch of the cells in flight does not stay resident)
+    if (pf_rows > 0 && i + pf_rows < S) {
+      for (const auto &rj : row_list(i + pf_rows)) {
+        o << "      CJ_PFA(" << rj.first << ");";
+        if (spec.rxn[rj.first].reversible) o << " CJ_PFB(" << rj.first << ");";
+        o << "\n";
+      }
+    }
+    // the loads of a chunk of reactions first (they keep their order), then the chunk's FMAs
+    for (size_t c0 = 0; c0 < rows.size(); c0 += chunk) {
+      const size_t c1 = std::min(rows.size(), c0 + chunk);
+      o << "      {\n";
+      for (size_t c = c0; c < c1; ++c) {
+        const int jj = rows[c].first;
+        o << "        const double a" << jj << " = CJ_A(" << jj << ")";
+        if (spec.rxn[jj].reversible) o << ", b" << jj << " = CJ_Bq(" << jj << ")";
+        o << ";\n";
+      }
+      for (size_t c = c0; c < c1; ++c) {
+        const int jj = rows[c].first;
+        const double dnu = rows[c].second;
+        const JitReaction &r = spec.rxn[jj];
+        for (const auto &e : r.reac) o << "        " << fma_line("acc[" + std::to_string(e.first) + "]", dnu * e.second, "a" + std::to_string(jj)) << "\n";
+        if (r.reversible)
+          for (const auto &e : r.prod) o << "        " << fma_line("acc[" + std::to_string(e.first) + "]", -dnu * e.second, "b" + std::to_string(jj)) << "\n";
+      }
       o << "      }\n";
     }
     o << "    } break;\n";
@@ -298,13 +337,12 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
   if (ce == cudaSuccess)
     ce = cudaKernelSetAttributeForDevice(jj->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem, device);
   // ---- tables and scratch ------------------------------------------------------------------------------
-  size_t o_tab = 0, o_bf = 0, o_co = 0, bytes = 0;
+  size_t o_tab = 0, o_bf = 0, bytes = 0;
   auto place = [&](size_t n) { const size_t off = (bytes + 255) / 256 * 256; bytes = off + n; return off; };
-  o_tab = place(tab16.size() * 8); o_bf = place(bfrag.size() * 8); o_co = place(coef.size() * sizeof(CjCoef));
+  o_tab = place(tab16.size() * 8); o_bf = place(bfrag.size() * 8);
   if (ce == cudaSuccess) ce = cudaMalloc(&jj->d_blob, bytes);
   if (ce == cudaSuccess) ce = cudaMemcpy((char *)jj->d_blob + o_tab, tab16.data(), tab16.size() * 8, cudaMemcpyHostToDevice);
   if (ce == cudaSuccess) ce = cudaMemcpy((char *)jj->d_blob + o_bf, bfrag.data(), bfrag.size() * 8, cudaMemcpyHostToDevice);
-  if (ce == cudaSuccess) ce = cudaMemcpy((char *)jj->d_blob + o_co, coef.data(), coef.size() * sizeof(CjCoef), cudaMemcpyHostToDevice);
   const size_t scr_rows = (size_t)4 * RP + (size_t)2 * spec.n_mb * 8 + (size_t)3 * S;
   if (ce == cudaSuccess) ce = cudaMalloc((void **)&jj->d_scratch, (size_t)num_sms * scr_rows * NT * sizeof(double));
   if (ce != cudaSuccess) {
@@ -317,7 +355,6 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
   jj->prm.eff_frag = d_eff_frag; jj->prm.thermo = d_thermo; jj->prm.logtab = d_logtab;
   jj->prm.tab = (const double *)((char *)jj->d_blob + o_tab);
   jj->prm.bfrag = (const double *)((char *)jj->d_blob + o_bf);
-  jj->prm.coef = (const CjCoef *)((char *)jj->d_blob + o_co);
   jj->prm.scratch = jj->d_scratch;
   *out = jj;
   return "";
