@@ -98,8 +98,10 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
   // ---- launch shape: the most warps (tile = 32 cells per warp) whose tile fits shared memory ----
   int warps = 0;
   size_t smem = 0;
-  int w_max = 8;
-  if (const char *e = std::getenv("CK_JACJ_WARPS")) w_max = std::min(8, std::max(1, std::atoi(e)));
+  // (registers: two columns of accumulators, 4 S, and about 60 beside them at the least; 512 threads x 128
+  //  registers when that fits, else 256 x 255)
+  int w_max = (4 * S + 60 <= 128) ? 16 : 8;
+  if (const char *e = std::getenv("CK_JACJ_WARPS")) w_max = std::min(w_max, std::max(1, std::atoi(e)));
   for (int w = w_max; w >= 1; --w) {
     const size_t ovl = std::max((size_t)n_ranges * RP * 16 + 384, (size_t)w * 32 * ost);
     const size_t doubles = (size_t)S * (32 * w + 8) + (size_t)n_ranges * S * 12 + ovl;
@@ -169,6 +171,11 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
     }
   }
   ks_start[S + 1] = (int)coef.size() / 4;
+  // k-steps of a species row whose A values are loaded ahead of the sparse part: the longest row's, at most 4
+  int kp = 1;
+  for (int i = 0; i < S; ++i) kp = std::max(kp, ks_start[i + 1] - ks_start[i]);
+  kp = std::min(kp, 4);
+  if (const char *e = std::getenv("CK_JACJ_KP")) kp = std::max(1, std::atoi(e));
   if (coef.empty()) coef.push_back(CjCoef{0.0, -1, 0});
   if (bfrag.empty()) bfrag.push_back(0.0);
 
@@ -178,7 +185,7 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
     << "\n#define CJ_B " << B << "\n#define CJ_NBLK " << nblk << "\n#define CJ_G_TB0 " << spec.group_end[1]
     << "\n#define CJ_G_FO0 " << spec.group_end[3] << "\n#define CJ_NM " << spec.n_m << "\n#define CJ_NMB " << spec.n_mb
     << "\n#define CJ_NFO " << spec.n_fo << "\n#define CJ_NTL " << ntl << "\n#define CJ_OST " << ost
-    << "\n#define CJ_BULK " << (bulk ? 1 : 0) << "\n#define CJ_HINT " << hint << "\n#define CJ_KP " << (std::getenv("CK_JACJ_KP") ? std::max(1, std::atoi(std::getenv("CK_JACJ_KP"))) : 4) << "\n#define CJ_PREF " << (std::getenv("CK_JACJ_PREF") ? std::atoi(std::getenv("CK_JACJ_PREF")) : 6) << "\n#define CJ_EXP " << (std::getenv("CK_JACJ_EXP") ? std::atoi(std::getenv("CK_JACJ_EXP")) : 0) << "\n";
+    << "\n#define CJ_BULK " << (bulk ? 1 : 0) << "\n#define CJ_HINT " << hint << "\n#define CJ_KP " << kp << "\n#define CJ_PREF " << (std::getenv("CK_JACJ_PREF") ? std::atoi(std::getenv("CK_JACJ_PREF")) : 6) << "\n#define CJ_EXP " << (std::getenv("CK_JACJ_EXP") ? std::atoi(std::getenv("CK_JACJ_EXP")) : 0) << "\n";
   auto emit = [&](const char *name, const std::vector<double> &v) {
     o << "__constant__ double " << name << "[" << (v.empty() ? 1 : v.size()) << "] = {";
     for (size_t i = 0; i < v.size(); ++i) o << (i ? "," : "") << (i % 6 == 0 ? "\n  " : " ") << lit(v[i]);

@@ -76,7 +76,7 @@ def test_parity_all_entries(ck, cfg_name, N):
     T, P, Y = ckgen.states(cfg, N=N)
     T[: N // 4] = np.linspace(350.0, 1000.0, N // 4)      # low NASA range and T = T_mid exactly
     with ck.Mechanism(mech) as gm:
-        assert gm.info("jac_cells") in (4, 8, 16, 32, 64, 96, 128, 160, 192, 224, 256)
+        assert gm.info("jac_cells") in (4, 8, 16) or (gm.info("jac_cells") % 32 == 0 and gm.info("jac_cells") <= 512)
         J = gpu_jacobian(ck, gm, T, P, Y)
     Jr = oracle.jacobian(oracle.OracleMechanism(mech), T, P, Y)
     rs, re = violations(mech, T, P, Y, J, Jr)
