@@ -474,9 +474,11 @@ def run_jacobian(args):
             torch.cuda.synchronize()
             ms = e0.elapsed_time(e1) / reps
             cells_per_tile = gm.info("jac_cells")
+            kernel = {0: "none", 1: "jacobian_kernel (table-driven, lanes = columns)", 2: "jacobian_kernel_v2 (table-driven, lanes = cells)",
+                      3: "ck_jacobian_jit (specialised to the mechanism)"}[gm.info("jac_kernel")]
         bytes_per_cell = 8 * ((S + 1) * (S + 1) + S + 2)
         gbs = bytes_per_cell * N / (ms * 1e-3) / 1e9
-        row = {"S": S, "R": R, "N": N, "ms": ms, "cells_per_s": N / (ms * 1e-3), "cells_per_tile": cells_per_tile,
+        row = {"S": S, "R": R, "N": N, "ms": ms, "cells_per_s": N / (ms * 1e-3), "kernel": kernel, "cells_per_tile": cells_per_tile,
                "roofline": {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
                             "bytes_per_cell": bytes_per_cell, "peak_source": peak_src},
                "l2": "output %.0f MB per call vs 126 MB L2" % (8 * (S + 1) ** 2 * N / 1e6)}

@@ -202,7 +202,9 @@ int ck_rk4_integrate(ck_mech *m, double *T, const double *P, double *Y, int64_t 
  * T, P, Y: DEVICE pointers laid out as for ck_source_terms.  J: DEVICE, [N][S+1][S+1]
  * doubles, cell-major and row-major per cell (a strided batch of matrices, lda = S+1); row
  * i < S is wdot_i, row S is dT/dt; column l < S is Y_l, column S is T; every entry is written.
- * Asynchronous on `stream`, allocates nothing, deterministic run to run (no atomics).
+ * Asynchronous on `stream`, allocates nothing, deterministic run to run (no atomics).  Calls on ONE
+ * handle must be ordered on one stream: the per-(reaction, cell) scalars of the cells in flight
+ * live in a scratch area the handle owns (ck_source_terms has no such restriction).
  * N == 0 is a successful no-op.  Errors: CK_EINVAL (NULL handle or pointer with N > 0, N < 0,
  * misaligned pointer), CK_EUNSUPPORTED (mechanism with the approximate-ANN Kc, S > 127, or
  * a tile that does not fit shared memory), CK_ECUDA. */
@@ -223,7 +225,7 @@ const char *ck_last_error(void);
  *       14 kernel variant in use (0 generic table-driven kernel, 1 mechanism-specialised),
  *       15 species whose accumulators the specialised kernel keeps in registers (the other
  *       S - that many accumulate in shared memory; 0 for the generic kernel),
- *       16 cells per tile of the Jacobian kernel (0 if ck_jacobian is unsupported here),
+ *       16 cells per tile of the Jacobian kernel in use (0 if ck_jacobian is unsupported here),
  *       17 1 if the specialised kernel runs two threads per cell (then 9 counts both, and a
  *       block works on half that many cells),
  *       18 1 if the handle was built as a measurement-only ABLATION whose results are not the
@@ -235,7 +237,11 @@ const char *ck_last_error(void);
  *       and M = C E as dense DMMA.8x8x4 products; same results to rounding),
  *       21 the largest N for which ck_source_terms uses a small-batch shape of the specialised
  *       kernel (8, 4 or 2 threads per cell in tiles of 32, 64 or 128 cells, whichever holds the
- *       batch in one wave; 0 if no such shape was built).
+ *       batch in one wave; 0 if no such shape was built),
+ *       22 the kernel ck_jacobian runs: 0 none (unsupported here), 1 the first table-driven kernel
+ *       (lanes = columns), 2 the second (lanes = cells), 3 the mechanism-specialised kernel
+ *       (NVRTC-compiled at create time; mechanisms of at most 53 species at fp64 without the
+ *       approximate-ANN Kc; environment CK_JAC_KERNEL=v1|v2 keeps the table-driven ones).
  * Returns -1 for a NULL handle or unknown `what`. */
 int64_t ck_mech_info(const ck_mech *m, int what);
 

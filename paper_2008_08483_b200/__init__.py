@@ -29,7 +29,7 @@ __all__ = ["Mechanism", "CkError", "ck_mech_create", "ck_source_terms", "ck_sour
 RU = 8314.46261815324  # J/(kmol K), the constant compiled into the kernels
 INFO = {"S": 0, "R": 1, "nnz_reac": 2, "nnz_prod": 3, "nnz_net": 4, "n_three_body": 5,
         "n_lindemann": 6, "n_troe": 7, "n_ranges": 8, "threads": 9, "blocks_per_sm": 10,
-        "smem_bytes": 11, "launches_per_call": 12, "nnz_eff": 13, "jit": 14, "s_reg": 15, "jac_cells": 16, "pair": 17, "ablation": 18, "precision": 19, "all_dmma": 20, "small_batch_max": 21}
+        "smem_bytes": 11, "launches_per_call": 12, "nnz_eff": 13, "jit": 14, "s_reg": 15, "jac_cells": 16, "pair": 17, "ablation": 18, "precision": 19, "all_dmma": 20, "small_batch_max": 21, "jac_kernel": 22}
 PREC_F64, PREC_MIXED, PREC_F32_RATES = 0, 1, 2
 
 _dp = C.POINTER(C.c_double)

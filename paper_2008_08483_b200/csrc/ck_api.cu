@@ -956,7 +956,7 @@ extern "C" int ck_jacobian(const ck_mech *m, const double *T, const double *P, c
   if (!m->jac)
     return fail(CK_EUNSUPPORTED, "ck_jacobian: not available for this mechanism (approximate-ANN Kc, S > 127, "
                                  "or the tile does not fit shared memory)");
-  const cudaError_t ce = m->jacj ? ck::jacj_launch(m->jacj, T, P, Y, N, J, (cudaStream_t)stream)
+  const cudaError_t ce = (m->jacj && ck::jacj_takes(m->jacj, J)) ? ck::jacj_launch(m->jacj, T, P, Y, N, J, (cudaStream_t)stream)
                                  : ck::jac_launch(m->jac, T, P, Y, N, J, (cudaStream_t)stream);
   if (ce != cudaSuccess) return fail_cuda(ce, "ck_jacobian launch");
   return CK_OK;
@@ -1179,6 +1179,7 @@ extern "C" int64_t ck_mech_info(const ck_mech *m, int what) {
     case 19: return m->jit_kernel ? m->jit_spec.prec : 0;
     case 20: return m->nu ? 1 : 0;
     case 21: return m->n_split ? (int64_t)m->split_cells[m->n_split - 1] * m->num_sms : 0;
+    case 22: return m->jacj ? 3 : (m->jac ? (ck::jac_cells_per_tile(m->jac) == 32 && ck::jac_is_v2(m->jac) ? 2 : 1) : 0);
     default: return -1;
   }
 }

@@ -71,6 +71,7 @@ struct JacMech;   // device tables of the Jacobian kernel (ck_jac.cu)
 std::string jac_create(const ck_mech_desc *d, int num_sms, size_t smem_block_max, JacMech **out);
 void jac_destroy(JacMech *jm);
 int jac_cells_per_tile(const JacMech *jm);
+bool jac_is_v2(const JacMech *jm);
 cudaError_t jac_launch(const JacMech *jm, const double *T, const double *P, const double *Y, int64_t N,
                        double *J, cudaStream_t stream);
 
@@ -83,6 +84,8 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
                         int num_sms, size_t smem_blk, JacJit **out);
 void jacj_destroy(JacJit *jj);
 int jacj_cells(const JacJit *jj);
+// false if J is not aligned for the kernel's bulk row stores (16 bytes): the table-driven kernels take the call
+bool jacj_takes(const JacJit *jj, const double *J);
 cudaError_t jacj_launch(const JacJit *jj, const double *T, const double *P, const double *Y, int64_t N, double *J,
                         cudaStream_t stream);
 

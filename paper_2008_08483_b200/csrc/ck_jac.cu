@@ -746,6 +746,7 @@ void jac_destroy(JacMech *jm) {
 }
 
 int jac_cells_per_tile(const JacMech *jm) { return jm->v2 ? 32 : jm->cells; }
+bool jac_is_v2(const JacMech *jm) { return jm->v2; }
 
 cudaError_t jac_launch(const JacMech *jm, const double *T, const double *P, const double *Y, int64_t N,
                        double *J, cudaStream_t stream) {

@@ -3,6 +3,7 @@
 // text, compiles it with NVRTC (ck_jit.cu), builds the tables of the dense part and launches.
 // The reaction order, the folded rate rows and the M = C E fragments are the source-term
 // kernel's (ck_api.cu: finalize_jit), so both kernels agree on what "reaction jj" is.
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -63,6 +64,23 @@ std::string gather_expr(const std::vector<std::pair<int, double>> &side) {
   return e;
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (libck.so does not link libcuda)
+typedef CUresult (*TmapEncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                 const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                 CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+TmapEncodeFn tmap_encoder() {
+  static TmapEncodeFn fn = [] {
+    void *f = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      f = nullptr;
+    cudaGetLastError();
+    return (TmapEncodeFn)f;
+  }();
+  return fn;
+}
+
 }  // namespace
 
 struct JacJit {
@@ -71,7 +89,7 @@ struct JacJit {
   JacjParams prm{};
   void *d_blob = nullptr;
   double *d_scratch = nullptr;
-  int threads = 0, grid_max = 1;
+  int threads = 0, grid_max = 1, n1 = 0, bulk = 0;
   size_t smem = 0;
 };
 
@@ -93,7 +111,11 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
   int ost = std::max(n1, 8 * ntl);
   while (ost % 4 != 2) ++ost;                      // rows 16-byte aligned, 128-bit row accesses conflict-free
   const int hint = std::getenv("CK_JACJ_HINT") ? std::atoi(std::getenv("CK_JACJ_HINT")) : 1;
-  const bool bulk = (n1 % 2 == 0) && !(std::getenv("CK_JACJ_BULK") && std::atoi(std::getenv("CK_JACJ_BULK")) == 0);
+  // how rows leave: 2 tensor copies (needs the driver's cuTensorMapEncodeTiled), 1 bulk copies per cell, 0 plain stores
+  int bulk = (n1 % 2 == 0) ? 2 : 0;
+  if (const char *e = std::getenv("CK_JACJ_BULK")) bulk = std::min(bulk, std::max(0, std::atoi(e)));
+  if (bulk == 2 && device >= 0 && !tmap_encoder()) bulk = 1;
+  if (bulk == 2) ost = n1;
 
   // ---- launch shape: the most warps (tile = 32 cells per warp) whose tile fits shared memory ----
   int warps = 0;
@@ -104,7 +126,7 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
   if (const char *e = std::getenv("CK_JACJ_WARPS")) w_max = std::min(w_max, std::max(1, std::atoi(e)));
   for (int w = w_max; w >= 1; --w) {
     const size_t ovl = std::max((size_t)n_ranges * RP * 16 + 384, (size_t)w * 32 * ost);
-    const size_t doubles = (size_t)S * (32 * w + 8) + (size_t)n_ranges * S * 12 + ovl;
+    const size_t doubles = ((size_t)S * (32 * w + 8) + (size_t)n_ranges * S * 12 + 15) / 16 * 16 + ovl;
     if (doubles * 8 + 64 <= smem_blk) { warps = w; smem = doubles * 8; break; }
   }
   if (!warps) return "tile does not fit shared memory";
@@ -185,7 +207,7 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
     << "\n#define CJ_B " << B << "\n#define CJ_NBLK " << nblk << "\n#define CJ_G_TB0 " << spec.group_end[1]
     << "\n#define CJ_G_FO0 " << spec.group_end[3] << "\n#define CJ_NM " << spec.n_m << "\n#define CJ_NMB " << spec.n_mb
     << "\n#define CJ_NFO " << spec.n_fo << "\n#define CJ_NTL " << ntl << "\n#define CJ_OST " << ost
-    << "\n#define CJ_BULK " << (bulk ? 1 : 0) << "\n#define CJ_HINT " << hint << "\n#define CJ_MH " << (std::getenv("CK_JACJ_MH") ? std::atoi(std::getenv("CK_JACJ_MH")) : 4) << "\n#define CJ_KP " << kp << "\n#define CJ_PREF " << (std::getenv("CK_JACJ_PREF") ? std::atoi(std::getenv("CK_JACJ_PREF")) : 6) << "\n#define CJ_EXP " << (std::getenv("CK_JACJ_EXP") ? std::atoi(std::getenv("CK_JACJ_EXP")) : 0) << "\n";
+    << "\n#define CJ_BULK " << bulk << "\n#define CJ_HINT " << hint << "\n#define CJ_MH " << (std::getenv("CK_JACJ_MH") ? std::atoi(std::getenv("CK_JACJ_MH")) : 4) << "\n#define CJ_KP " << kp << "\n#define CJ_PREF " << (std::getenv("CK_JACJ_PREF") ? std::atoi(std::getenv("CK_JACJ_PREF")) : 6) << "\n#define CJ_EXP " << (std::getenv("CK_JACJ_EXP") ? std::atoi(std::getenv("CK_JACJ_EXP")) : 0) << "\n";
   auto emit = [&](const char *name, const std::vector<double> &v) {
     o << "__constant__ double " << name << "[" << (v.empty() ? 1 : v.size()) << "] = {";
     for (size_t i = 0; i < v.size(); ++i) o << (i ? "," : "") << (i % 6 == 0 ? "\n  " : " ") << lit(v[i]);
@@ -358,7 +380,7 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
     jacj_destroy(jj);
     return msg;
   }
-  jj->threads = NT; jj->grid_max = num_sms; jj->smem = smem;
+  jj->threads = NT; jj->grid_max = num_sms; jj->smem = smem; jj->n1 = n1; jj->bulk = bulk;
   jj->prm.eff_frag = d_eff_frag; jj->prm.thermo = d_thermo; jj->prm.logtab = d_logtab;
   jj->prm.tab = (const double *)((char *)jj->d_blob + o_tab);
   jj->prm.bfrag = (const double *)((char *)jj->d_blob + o_bf);
@@ -376,6 +398,7 @@ void jacj_destroy(JacJit *jj) {
 }
 
 int jacj_cells(const JacJit *jj) { return jj->threads; }
+bool jacj_takes(const JacJit *jj, const double *J) { return jj->bulk == 0 || ((uintptr_t)J & 15u) == 0; }
 
 cudaError_t jacj_launch(const JacJit *jj, const double *T, const double *P, const double *Y, int64_t N, double *J,
                         cudaStream_t stream) {
@@ -390,7 +413,19 @@ cudaError_t jacj_launch(const JacJit *jj, const double *T, const double *P, cons
   prm.tile_cells = (int)tc;
   const int64_t tiles = (N + tc - 1) / tc;
   const int grid = (int)std::min<int64_t>(tiles, jj->grid_max);
-  void *args[] = {&prm};
+  // J as a rank-3 tensor (column, row, cell) of doubles; a copy stores one row of 32 cells
+  alignas(64) CUtensorMap tmap;
+  std::memset(&tmap, 0, sizeof tmap);
+  if (jj->bulk == 2) {
+    const cuuint64_t n = (cuuint64_t)jj->n1;
+    const cuuint64_t dims[3] = {n, n, (cuuint64_t)N}, strides[2] = {n * 8, n * n * 8};
+    const cuuint32_t box[3] = {(cuuint32_t)n, 1, 32}, estr[3] = {1, 1, 1};
+    const CUresult r = tmap_encoder()(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void *)J, dims, strides, box, estr,
+                                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                      CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+  }
+  void *args[] = {&prm, &tmap};
   return cudaLaunchKernel((const void *)jj->kernel, dim3(grid), dim3(jj->threads), args, jj->smem, stream);
 }
 
