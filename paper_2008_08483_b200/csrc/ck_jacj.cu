@@ -277,8 +277,8 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
   // P1b: tc_i = sum_j dnu_ij t_j, gc_i = sum_j dnu_ij e_j
   o << "__device__ __forceinline__ void cj_columns(const CjCtx &x, double (&tc)[CJ_S], double (&gc)[CJ_S]) {\n"
     << "#pragma unroll 1\n  for (int blk = 0; blk < CJ_NBLK; ++blk) {\n    double t[CJ_B], e[CJ_B];\n"
-    << "#if CJ_PREF\n    if (blk + 1 < CJ_NBLK) {\n#pragma unroll\n      for (int b = 0; b < CJ_B; ++b) { CJ_PF1(&CJ_SCR(CJ_OFF_T, (blk + 1) * CJ_B + b)); CJ_PF1(&CJ_SCR(CJ_OFF_E, (blk + 1) * CJ_B + b)); }\n    }\n#endif\n"
-    << "#pragma unroll\n    for (int b = 0; b < CJ_B; ++b) { t[b] = cj_ld(&CJ_SCR(CJ_OFF_T, blk * CJ_B + b), x.ps); e[b] = cj_ld(&CJ_SCR(CJ_OFF_E, blk * CJ_B + b), x.ps); }\n"
+    << "#if CJ_PREF\n    if (blk + 1 < CJ_NBLK) {\n#pragma unroll\n      for (int b = 0; b < CJ_B; ++b) CJ_PF1(&CJ_SCR2(CJ_R + (blk + 1) * CJ_B + b));\n    }\n#endif\n"
+    << "#pragma unroll\n    for (int b = 0; b < CJ_B; ++b) { const double2 te = CJ_TE(blk * CJ_B + b); t[b] = te.x; e[b] = te.y; }\n"
     << "    switch (blk) {\n";
   for (int k = 0; k < nblk; ++k) {
     o << "      case " << k << ":\n";
@@ -312,9 +312,7 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
     // the next row's (a, b) towards L2 (the scratch of the cells in flight does not stay resident)
     if (pf_rows > 0 && i + pf_rows < S) {
       for (const auto &rj : row_list(i + pf_rows)) {
-        o << "      CJ_PFA(" << rj.first << ");";
-        if (spec.rxn[rj.first].reversible) o << " CJ_PFB(" << rj.first << ");";
-        o << "\n";
+        o << "      CJ_PFAB(" << rj.first << ");\n";
       }
     }
     // the loads of a chunk of reactions first (they keep their order), then the chunk's FMAs
@@ -323,17 +321,15 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
       o << "      {\n";
       for (size_t c = c0; c < c1; ++c) {
         const int jj = rows[c].first;
-        o << "        const double a" << jj << " = CJ_A(" << jj << ")";
-        if (spec.rxn[jj].reversible) o << ", b" << jj << " = CJ_Bq(" << jj << ")";
-        o << ";\n";
+        o << "        const double2 ab" << jj << " = CJ_AB(" << jj << ");\n";
       }
       for (size_t c = c0; c < c1; ++c) {
         const int jj = rows[c].first;
         const double dnu = rows[c].second;
         const JitReaction &r = spec.rxn[jj];
-        for (const auto &e : r.reac) o << "        " << fma_line("acc[" + std::to_string(e.first) + "]", dnu * e.second, "a" + std::to_string(jj)) << "\n";
+        for (const auto &e : r.reac) o << "        " << fma_line("acc[" + std::to_string(e.first) + "]", dnu * e.second, "ab" + std::to_string(jj) + ".x") << "\n";
         if (r.reversible)
-          for (const auto &e : r.prod) o << "        " << fma_line("acc[" + std::to_string(e.first) + "]", -dnu * e.second, "b" + std::to_string(jj)) << "\n";
+          for (const auto &e : r.prod) o << "        " << fma_line("acc[" + std::to_string(e.first) + "]", -dnu * e.second, "ab" + std::to_string(jj) + ".y") << "\n";
       }
       o << "      }\n";
     }
