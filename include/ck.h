@@ -202,7 +202,9 @@ int ck_rk4_integrate(ck_mech *m, double *T, const double *P, double *Y, int64_t 
  * T, P, Y: DEVICE pointers laid out as for ck_source_terms.  J: DEVICE, [N][S+1][S+1]
  * doubles, cell-major and row-major per cell (a strided batch of matrices, lda = S+1); row
  * i < S is wdot_i, row S is dT/dt; column l < S is Y_l, column S is T; every entry is written.
- * Asynchronous on `stream`, allocates nothing, deterministic run to run (no atomics).  Calls on ONE
+ * Asynchronous on `stream`, deterministic run to run (no atomics).  The FIRST call on a handle compiles
+ * the mechanism-specialised kernel (NVRTC; cached on disk like the source-term kernel) and allocates its
+ * scratch (that synchronises); later calls allocate nothing.  Calls on ONE
  * handle must be ordered on one stream: the per-(reaction, cell) scalars of the cells in flight
  * live in a scratch area the handle owns (ck_source_terms has no such restriction).
  * N == 0 is a successful no-op.  Errors: CK_EINVAL (NULL handle or pointer with N > 0, N < 0,

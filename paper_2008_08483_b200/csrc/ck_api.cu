@@ -956,8 +956,19 @@ extern "C" int ck_jacobian(const ck_mech *m, const double *T, const double *P, c
   if (!m->jac)
     return fail(CK_EUNSUPPORTED, "ck_jacobian: not available for this mechanism (approximate-ANN Kc, S > 127, "
                                  "or the tile does not fit shared memory)");
-  const cudaError_t ce = (m->jacj && ck::jacj_takes(m->jacj, J)) ? ck::jacj_launch(m->jacj, T, P, Y, N, J, (cudaStream_t)stream)
-                                 : ck::jac_launch(m->jac, T, P, Y, N, J, (cudaStream_t)stream);
+  // the specialised kernel is compiled, and its scratch allocated, on the first call; if that fails
+  // the table-driven kernels take this and every later call (ck_mech_note-style: jacj_note says why)
+  bool jit = m->jacj && ck::jacj_takes(m->jacj, J);
+  if (jit) {
+    const std::string err = ck::jacj_ensure(m->jacj);
+    if (!err.empty()) {
+      const char *e = std::getenv("CK_JAC_KERNEL");
+      if (e && std::string(e) == "v3") return fail(CK_EUNSUPPORTED, "CK_JAC_KERNEL=v3 but " + err);
+      jit = false;
+    }
+  }
+  const cudaError_t ce = jit ? ck::jacj_launch(m->jacj, T, P, Y, N, J, (cudaStream_t)stream)
+                             : ck::jac_launch(m->jac, T, P, Y, N, J, (cudaStream_t)stream);
   if (ce != cudaSuccess) return fail_cuda(ce, "ck_jacobian launch");
   return CK_OK;
 }

@@ -76,12 +76,15 @@ cudaError_t jac_launch(const JacMech *jm, const double *T, const double *P, cons
                        double *J, cudaStream_t stream);
 
 // The mechanism-specialised Jacobian kernel (ck_jacj.cu / ck_jacj_kernel.cuh), NVRTC-compiled.
-// jacj_create returns "" and sets *out, or returns why the kernel is not available (*out NULL; the
-// table-driven kernels of ck_jac.cu remain).  device < 0: only generate the source (CK_JACJ_DUMP).
+// jacj_create generates the kernel text and its tables (no device work) and returns "" with *out set, or
+// returns why the kernel is not available (*out NULL; the table-driven kernels of ck_jac.cu remain).
+// device < 0: only generate the source (CK_JACJ_DUMP).
 struct JacJit;
 std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::vector<double> &tab10,
                         const double *d_thermo, const double *d_logtab, const double *d_eff_frag, int device,
                         int num_sms, size_t smem_blk, JacJit **out);
+// First use: compiles and loads the kernel, uploads its tables, allocates its scratch ("" or the error text).
+std::string jacj_ensure(JacJit *jj);
 void jacj_destroy(JacJit *jj);
 int jacj_cells(const JacJit *jj);
 // false if J is not aligned for the kernel's bulk row stores (16 bytes): the table-driven kernels take the call

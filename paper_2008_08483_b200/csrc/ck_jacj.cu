@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <sstream>
 #include <string>
 #include <vector>
@@ -89,8 +90,13 @@ struct JacJit {
   JacjParams prm{};
   void *d_blob = nullptr;
   double *d_scratch = nullptr;
-  int threads = 0, grid_max = 1, n1 = 0, bulk = 0;
-  size_t smem = 0;
+  int threads = 0, grid_max = 1, n1 = 0, bulk = 0, device = 0;
+  size_t smem = 0, scr_rows = 0;
+  // until the first ck_jacobian call: the generated text and the host copies of the tables
+  std::string src, error;
+  std::vector<double> tab16, bfrag;
+  bool ready = false;
+  std::mutex mu;
 };
 
 // Returns "" on success (*out set), or the reason the kernel is not available for this mechanism
@@ -346,13 +352,31 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
   }
   if (device < 0) return "source only";
 
-  // ---- compile, load ---------------------------------------------------------------------------------
+  // Everything that needs the device -- compiling the text, loading it, the tables and the scratch of
+  // the cells in flight (hundreds of MB) -- waits for the first ck_jacobian call (jacj_ensure).
   JacJit *jj = new JacJit;
+  jj->src = src;
+  jj->tab16.swap(tab16);
+  jj->bfrag.swap(bfrag);
+  jj->scr_rows = (size_t)4 * RP + (size_t)2 * spec.n_mb * 8 + (size_t)3 * S;
+  jj->device = device;
+  jj->threads = NT; jj->grid_max = num_sms; jj->smem = smem; jj->n1 = n1; jj->bulk = bulk;
+  jj->prm.eff_frag = d_eff_frag; jj->prm.thermo = d_thermo; jj->prm.logtab = d_logtab;
+  *out = jj;
+  return "";
+}
+
+// Compiles and loads the kernel, uploads its tables and allocates the scratch, once.  Returns "" or
+// the error text (then, and on every later call, the caller falls back to the table-driven kernels).
+std::string jacj_ensure(JacJit *jj) {
+  std::lock_guard<std::mutex> lock(jj->mu);
+  if (jj->ready) return "";
+  if (!jj->error.empty()) return jj->error;
   std::vector<char> cubin;
   cudaError_t ce = cudaSuccess;
   for (int attempt = 0; attempt < 2; ++attempt) {
-    const std::string err = jit_compile(src, &cubin, attempt == 0);
-    if (!err.empty()) { delete jj; return err; }
+    const std::string err = jit_compile(jj->src, &cubin, attempt == 0);
+    if (!err.empty()) return jj->error = err;
     ce = cudaLibraryLoadData(&jj->lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
     if (ce == cudaSuccess) break;
     cudaGetLastError();
@@ -360,28 +384,28 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
   }
   if (ce == cudaSuccess) ce = cudaLibraryGetKernel(&jj->kernel, jj->lib, "ck_jacobian_jit");
   if (ce == cudaSuccess)
-    ce = cudaKernelSetAttributeForDevice(jj->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem, device);
-  // ---- tables and scratch ------------------------------------------------------------------------------
+    ce = cudaKernelSetAttributeForDevice(jj->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)jj->smem, jj->device);
   size_t o_tab = 0, o_bf = 0, bytes = 0;
   auto place = [&](size_t n) { const size_t off = (bytes + 255) / 256 * 256; bytes = off + n; return off; };
-  o_tab = place(tab16.size() * 8); o_bf = place(bfrag.size() * 8);
+  o_tab = place(jj->tab16.size() * 8); o_bf = place(jj->bfrag.size() * 8);
   if (ce == cudaSuccess) ce = cudaMalloc(&jj->d_blob, bytes);
-  if (ce == cudaSuccess) ce = cudaMemcpy((char *)jj->d_blob + o_tab, tab16.data(), tab16.size() * 8, cudaMemcpyHostToDevice);
-  if (ce == cudaSuccess) ce = cudaMemcpy((char *)jj->d_blob + o_bf, bfrag.data(), bfrag.size() * 8, cudaMemcpyHostToDevice);
-  const size_t scr_rows = (size_t)4 * RP + (size_t)2 * spec.n_mb * 8 + (size_t)3 * S;
-  if (ce == cudaSuccess) ce = cudaMalloc((void **)&jj->d_scratch, (size_t)num_sms * scr_rows * NT * sizeof(double));
+  if (ce == cudaSuccess) ce = cudaMemcpy((char *)jj->d_blob + o_tab, jj->tab16.data(), jj->tab16.size() * 8, cudaMemcpyHostToDevice);
+  if (ce == cudaSuccess) ce = cudaMemcpy((char *)jj->d_blob + o_bf, jj->bfrag.data(), jj->bfrag.size() * 8, cudaMemcpyHostToDevice);
+  if (ce == cudaSuccess) ce = cudaMalloc((void **)&jj->d_scratch, (size_t)jj->grid_max * jj->scr_rows * jj->threads * sizeof(double));
   if (ce != cudaSuccess) {
-    const std::string msg = std::string("specialised Jacobian kernel: ") + cudaGetErrorString(ce);
+    jj->error = std::string("specialised Jacobian kernel: ") + cudaGetErrorString(ce);
     cudaGetLastError();
-    jacj_destroy(jj);
-    return msg;
+    if (jj->d_blob) { cudaFree(jj->d_blob); jj->d_blob = nullptr; }
+    if (jj->lib) { cudaLibraryUnload(jj->lib); jj->lib = nullptr; }
+    return jj->error;
   }
-  jj->threads = NT; jj->grid_max = num_sms; jj->smem = smem; jj->n1 = n1; jj->bulk = bulk;
-  jj->prm.eff_frag = d_eff_frag; jj->prm.thermo = d_thermo; jj->prm.logtab = d_logtab;
   jj->prm.tab = (const double *)((char *)jj->d_blob + o_tab);
   jj->prm.bfrag = (const double *)((char *)jj->d_blob + o_bf);
   jj->prm.scratch = jj->d_scratch;
-  *out = jj;
+  std::string().swap(jj->src);
+  std::vector<double>().swap(jj->tab16);
+  std::vector<double>().swap(jj->bfrag);
+  jj->ready = true;
   return "";
 }
 

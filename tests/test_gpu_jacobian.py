@@ -227,3 +227,29 @@ def test_errors(ck):
         with pytest.raises(ck.CkError) as e:
             ck.ck_jacobian(gm.handle, 8, 8, 8, -1, 8)
         assert e.value.status == 1
+
+
+def test_kernel_in_use_and_a_J_that_is_only_8_byte_aligned(ck, jac_kernel):
+    """ck_mech_info 22 names the kernel; the specialised kernel stores rows by 16-byte bulk / tensor
+    copies, so a J that is only 8-byte aligned goes through the table-driven kernels: same values
+    to the parity bound, every entry written."""
+    cfg = ckgen.CONFIGS["mid_1m"]
+    mech = ckgen.mechanism(cfg.mech)
+    N, S = 77, mech.n_species
+    T, P, Y = ckgen.states(cfg, N=N)
+    dev = torch.device("cuda:0")
+    Td, Pd, Yd = (torch.from_numpy(a).to(dev) for a in (T, P, Y))
+    with ck.Mechanism(mech) as gm:
+        assert gm.info("jac_kernel") == {"jit": 3, "v2": 2, "v1": 1}[jac_kernel]
+        buf = torch.full((N * (S + 1) * (S + 1) + 1,), float("nan"), dtype=torch.float64, device=dev)
+        Jm = buf[1:].view(N, S + 1, S + 1)                 # 8 bytes past a 16-byte boundary
+        assert Jm.data_ptr() % 16 == 8
+        gm.jacobian(Td, Pd, Yd, Jm, stream=torch.cuda.current_stream().cuda_stream)
+        Ja = gpu_jacobian(ck, gm, T, P, Y)
+        torch.cuda.synchronize()
+    Jm = Jm.cpu().numpy()
+    assert np.isnan(buf[0].item())
+    Jr = oracle.jacobian(oracle.OracleMechanism(mech), T, P, Y)
+    for Jx in (Jm, Ja):
+        rs, re = violations(mech, T, P, Y, Jx, Jr)
+        assert rs <= 1.0 and re <= 1.0, (rs, re)
