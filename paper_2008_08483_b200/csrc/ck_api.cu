@@ -331,9 +331,66 @@ void finalize_jit(const ck_mech_desc *d, HostBuild *hb, const std::vector<double
   for (int g = 0; g < 6; ++g) {
     // within a falloff group the Troe reactions first: the kernel decides Troe / Lindemann per
     // block from its first reaction
-    for (int pass = 0; pass < 2; ++pass)
+    const size_t g0 = order.size();
+    for (int pass = 0; pass < 2; ++pass) {
+      const size_t p0 = order.size();
       for (int j = 0; j < R; ++j)
         if (group_of(orig[j]) == g && (orig[j].type == 3) == (pass == 0)) order.push_back(j);
+      // Within the pass, reactions that gather the same species are put into the same block: their
+      // ln C loads are then shared (one LDS instead of two: less unique code, less load latency).
+      // Greedy: a block takes, one after the other, the remaining reaction that shares the most
+      // species with what the block already reads (ties: input order).  CK_JIT_CLUSTER=0 turns it off.
+      if (env_int("CK_JIT_CLUSTER", 1) != 0 && order.size() - p0 > (size_t)kJitBlock) {
+        std::vector<int> rest(order.begin() + p0, order.end()), out;
+        std::vector<char> in_blk(S, 0);
+        while (!rest.empty()) {
+          const size_t pos_in_blk = (g0 + (order.size() - rest.size() - g0)) % kJitBlock;   // position within the group's blocks
+          (void)pos_in_blk;
+          if ((out.size() + (p0 - g0)) % kJitBlock == 0) std::fill(in_blk.begin(), in_blk.end(), 0);
+          size_t best = 0;
+          int best_share = -1;
+          for (size_t c = 0; c < rest.size(); ++c) {
+            int share = 0;
+            for (const auto &e : orig[rest[c]].reac) share += in_blk[e.first];
+            for (const auto &e : orig[rest[c]].prod) share += in_blk[e.first];
+            if (share > best_share) { best_share = share; best = c; }
+          }
+          const int j = rest[best];
+          rest.erase(rest.begin() + best);
+          out.push_back(j);
+          for (const auto &e : orig[j].reac) in_blk[e.first] = 1;
+          for (const auto &e : orig[j].prod) in_blk[e.first] = 1;
+        }
+        std::copy(out.begin(), out.end(), order.begin() + p0);
+        // then pairwise swaps between blocks while the number of distinct species read per block,
+        // summed over the blocks, goes down (a fixed, deterministic sweep order)
+        auto blk_cost = [&](size_t blk_first) {   // distinct species gathered by the block starting at this position
+          std::fill(in_blk.begin(), in_blk.end(), 0);
+          int n = 0;
+          for (size_t q = blk_first; q < blk_first + (size_t)kJitBlock && q < order.size(); ++q) {
+            if (q < g0) continue;
+            const ck::JitReaction &r = orig[order[q]];
+            for (const auto &e : r.reac) if (!in_blk[e.first]) { in_blk[e.first] = 1; ++n; }
+            if (r.reversible) for (const auto &e : r.prod) if (!in_blk[e.first]) { in_blk[e.first] = 1; ++n; }
+          }
+          return n;
+        };
+        auto first_of = [&](size_t pos) { return g0 + (pos - g0) / kJitBlock * kJitBlock; };
+        for (int sweep = 0; sweep < 8; ++sweep) {
+          bool improved = false;
+          for (size_t a = p0; a < order.size(); ++a)
+            for (size_t b = a + 1; b < order.size(); ++b) {
+              const size_t fa = first_of(a), fb = first_of(b);
+              if (fa == fb) continue;
+              const int before = blk_cost(fa) + blk_cost(fb);
+              std::swap(order[a], order[b]);
+              if (blk_cost(fa) + blk_cost(fb) < before) improved = true;
+              else std::swap(order[a], order[b]);
+            }
+          if (!improved) break;
+        }
+      }
+    }
     while (order.size() % kJitBlock) order.push_back(-1);
     spec.group_end[g] = (int)order.size() / kJitBlock;
   }

@@ -372,6 +372,12 @@ std::string jacj_ensure(JacJit *jj) {
   std::lock_guard<std::mutex> lock(jj->mu);
   if (jj->ready) return "";
   if (!jj->error.empty()) return jj->error;
+  // (tables and scratch belong on the handle's device, whatever device is current in this thread)
+  struct DeviceGuard {
+    int prev = -1, want;
+    explicit DeviceGuard(int w) : want(w) { if (cudaGetDevice(&prev) == cudaSuccess && prev != want) cudaSetDevice(want); else prev = -1; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+  } guard(jj->device);
   std::vector<char> cubin;
   cudaError_t ce = cudaSuccess;
   for (int attempt = 0; attempt < 2; ++attempt) {
