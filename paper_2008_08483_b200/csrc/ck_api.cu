@@ -275,6 +275,7 @@ std::string choose_jit_shape(ck::JitSpec &spec, size_t smem_sm, size_t smem_blk,
   if (const char *e = std::getenv("CK_JIT_SYNC")) spec.sync_every = std::atoi(e);
   if (const char *e = std::getenv("CK_JIT_KCONST")) spec.kconst = std::atoi(e) != 0;
   spec.straight = env_int("CK_JIT_STRAIGHT", 0);
+  spec.pin = env_int("CK_JIT_PIN", 0);
   // (CK_JIT_KC=none, the ablation that removes the equilibrium layer, changes the RESULT: it is
   //  honoured only together with CK_ALLOW_ABLATION=1, see setup_jit, and shows in ck_mech_info 18)
   if (const char *e = std::getenv("CK_JIT_KC")) spec.kc_none = std::string(e) == "none";

@@ -60,6 +60,7 @@ struct JitSpec {
   std::vector<double> ann_const;   // mean | 1/std | W_in | B | W_hid
   int lut_rep = 1;             // interleaved copies of the exp table (16: conflict-free lookups)
   bool kconst = false;         // polynomial coefficients as constant-bank operands (else literals)
+  int pin = 0;                 // species whose ln C the reaction walk keeps in registers (the most gathered ones)
   int straight = 0;            // n > 0: the reaction walk in straight-line code, rate core inlined per block (measurement knob CK_JIT_STRAIGHT)
   int group_end[6] = {0, 0, 0, 0, 0, 0};   // end block of (elementary, three-body, falloff) x (rev, irrev)
   std::vector<JitReaction> rxn;

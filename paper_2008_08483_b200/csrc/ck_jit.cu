@@ -11,6 +11,7 @@
 #include <sys/stat.h>
 #include <unistd.h>
 
+#include <algorithm>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -73,12 +74,14 @@ std::string lit(double v) {
   return s;
 }
 
-// nu^T ln C of one side of a reaction as an expression: sums and fmas of CK_LNC(k)
-std::string gather_expr(const std::vector<std::pair<int, double>> &side) {
+// nu^T ln C of one side of a reaction as an expression: sums and fmas of CK_LNC(k) (or, for the
+// species in `pinned`, of the register copy lcp<k> made at the top of ck_reactions)
+std::string gather_expr(const std::vector<std::pair<int, double>> &side, const std::vector<char> &pinned) {
   if (side.empty()) return "CK_LIT(0.0)";
   std::string e;
   for (size_t i = 0; i < side.size(); ++i) {
-    const std::string c = "CK_LNC(" + std::to_string(side[i].first) + ")";
+    const std::string c = pinned[side[i].first] ? "lcp" + std::to_string(side[i].first)
+                                                 : "CK_LNC(" + std::to_string(side[i].first) + ")";
     const double nu = side[i].second;
     const std::string l = "CK_LIT(" + lit(nu) + ")";
     if (i == 0) e = (nu == 1.0) ? c : (l + " * " + c);
@@ -197,6 +200,18 @@ std::string jit_generate_source(const JitSpec &s) {
   o << text.substr(0, at);
   const int B = s.block, nblk = (int)s.rxn.size() / B;
   const int nhot = s.pair ? std::min(2 * s.s_reg, s.S) : s.s_reg;
+  // the s.pin species that the gathers read most often keep their ln C in a register for the whole walk
+  std::vector<char> pinned(s.S, 0);
+  if (s.pin > 0 && !s.pair && s.split <= 1) {
+    std::vector<int> cnt(s.S, 0), idx(s.S);
+    for (const JitReaction &r : s.rxn) {
+      for (const auto &e : r.reac) cnt[e.first]++;
+      if (r.reversible) for (const auto &e : r.prod) cnt[e.first]++;
+    }
+    for (int k = 0; k < s.S; ++k) idx[k] = k;
+    std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return cnt[a] > cnt[b]; });
+    for (int i = 0; i < std::min(s.pin, s.S); ++i) pinned[idx[i]] = 1;
+  }
   // accumulator of internal species sp, and (pair mode) the half of the cell's thread pair that owns it
   auto acc_of = [&](int sp, int *owner) {
     if (sp < nhot) {
@@ -226,9 +241,9 @@ std::string jit_generate_source(const JitSpec &s) {
   auto gathers = [&](int k) {
     for (int bb = 0; bb < B; ++bb) {
       const JitReaction &r = s.rxn[(size_t)k * B + bb];
-      o << "        gf[" << bb << "] = " << gather_expr(r.reac) << ";";
+      o << "        gf[" << bb << "] = " << gather_expr(r.reac, pinned) << ";";
       if (r.index >= 0) o << "  // reaction " << r.index;
-      o << "\n        gr[" << bb << "] = " << (r.reversible ? gather_expr(r.prod) : std::string("CK_LIT(0.0)")) << ";\n";
+      o << "\n        gr[" << bb << "] = " << (r.reversible ? gather_expr(r.prod, pinned) : std::string("CK_LIT(0.0)")) << ";\n";
     }
   };
   const char *names[6] = {"ck_core<0, 1>", "ck_core<0, 0>", "ck_core<1, 1>", "ck_core<1, 0>",
@@ -245,6 +260,8 @@ std::string jit_generate_source(const JitSpec &s) {
   };
   o << "__device__ __forceinline__ void ck_reactions(const CkCtx &x, double (&w)[CK_SREG > 0 ? CK_SREG : 1]) {\n"
     << "  ck_real gf[CK_B], gr[CK_B];\n  double q[CK_B];\n";
+  for (int k = 0; k < s.S; ++k)
+    if (pinned[k]) o << "  const ck_real lcp" << k << " = CK_LNC(" << k << ");\n";
   if (s.split > 1) {
     // Small-batch shape: part x.half of a cell's CK_SPLIT threads walks blocks x.half, x.half + K, ..;
     // a block's gathers, its rate core and its scatters (into this thread's own accumulators of
