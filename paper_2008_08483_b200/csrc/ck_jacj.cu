@@ -207,13 +207,18 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
   if (coef.empty()) coef.push_back(CjCoef{0.0, -1, 0});
   if (bfrag.empty()) bfrag.push_back(0.0);
 
+  // Dead scratch lines are dropped from L2 (discard.global.L2) where the scratch of all blocks fits L2: then
+  // they would otherwise be written back behind the output stream (S=9: 2.18 -> 1.23 GB of DRAM traffic per
+  // 2^20 cells); where it does not fit (S=53: 457 MB) the lines are gone before they die and the discards only cost time
+  int discard = ((size_t)num_sms * ((size_t)4 * RP + (size_t)2 * spec.n_mb * 8 + (size_t)3 * S) * NT * 8 <= ((size_t)100 << 20)) ? 1 : 0;
+  if (const char *e = std::getenv("CK_JACJ_DISCARD")) discard = std::atoi(e) != 0;
   // ---- source text -------------------------------------------------------------------------------
   std::ostringstream o;
   o << "#define CJ_S " << S << "\n#define CJ_R " << RP << "\n#define CJ_NT " << NT << "\n#define CJ_NRANGES " << n_ranges
     << "\n#define CJ_B " << B << "\n#define CJ_NBLK " << nblk << "\n#define CJ_G_TB0 " << spec.group_end[1]
     << "\n#define CJ_G_FO0 " << spec.group_end[3] << "\n#define CJ_NM " << spec.n_m << "\n#define CJ_NMB " << spec.n_mb
     << "\n#define CJ_NFO " << spec.n_fo << "\n#define CJ_NTL " << ntl << "\n#define CJ_OST " << ost
-    << "\n#define CJ_BULK " << bulk << "\n#define CJ_HINT " << hint << "\n#define CJ_MH " << (std::getenv("CK_JACJ_MH") ? std::atoi(std::getenv("CK_JACJ_MH")) : 4) << "\n#define CJ_KP " << kp << "\n#define CJ_PREF " << (std::getenv("CK_JACJ_PREF") ? std::atoi(std::getenv("CK_JACJ_PREF")) : 6) << "\n#define CJ_EXP " << (std::getenv("CK_JACJ_EXP") ? std::atoi(std::getenv("CK_JACJ_EXP")) : 0) << "\n";
+    << "\n#define CJ_BULK " << bulk << "\n#define CJ_HINT " << hint << "\n#define CJ_MH " << (std::getenv("CK_JACJ_MH") ? std::atoi(std::getenv("CK_JACJ_MH")) : 4) << "\n#define CJ_KP " << kp << "\n#define CJ_PREF " << (std::getenv("CK_JACJ_PREF") ? std::atoi(std::getenv("CK_JACJ_PREF")) : 6) << "\n#define CJ_DISCARD " << discard << "\n#define CJ_EXP " << (std::getenv("CK_JACJ_EXP") ? std::atoi(std::getenv("CK_JACJ_EXP")) : 0) << "\n";
   auto emit = [&](const char *name, const std::vector<double> &v) {
     o << "__constant__ double " << name << "[" << (v.empty() ? 1 : v.size()) << "] = {";
     for (size_t i = 0; i < v.size(); ++i) o << (i ? "," : "") << (i % 6 == 0 ? "\n  " : " ") << lit(v[i]);
