@@ -139,6 +139,7 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
   const int NT = 32 * warps;
   const int env_chunk = std::getenv("CK_JACJ_CHUNK") ? std::atoi(std::getenv("CK_JACJ_CHUNK")) : 8;
   const int pf_rows = std::getenv("CK_JACJ_PFROWS") ? std::atoi(std::getenv("CK_JACJ_PFROWS")) : 0;
+  const int pf_l1 = std::getenv("CK_JACJ_PFL1") ? std::atoi(std::getenv("CK_JACJ_PFL1")) : 8;
 
   // ---- rate table rows of 16 doubles ----------------------------------------------------------
   std::vector<double> range_T = spec.range_T;
@@ -326,6 +327,11 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
         o << "      CJ_PFAB(" << rj.first << ");\n";
       }
     }
+    // the first (a, b) pairs of the next row towards L1: its first loads then do not wait for L2 / DRAM
+    if (pf_l1 > 0 && i + 1 < S) {
+      const std::vector<std::pair<int, double>> nx = row_list(i + 1);
+      for (size_t c = 0; c < nx.size() && (int)c < pf_l1; ++c) o << "      CJ_PF1(&CJ_SCR2(" << nx[c].first << "));\n";
+    }
     // the loads of a chunk of reactions first (they keep their order), then the chunk's FMAs
     for (size_t c0 = 0; c0 < rows.size(); c0 += chunk) {
       const size_t c1 = std::min(rows.size(), c0 + chunk);
@@ -441,6 +447,8 @@ cudaError_t jacj_launch(const JacJit *jj, const double *T, const double *P, cons
   const int64_t waves = (N + per_wave - 1) / per_wave;
   int64_t tc = (N + waves * jj->grid_max - 1) / (waves * jj->grid_max);
   tc = std::min<int64_t>(jj->threads, (tc + 31) / 32 * 32);
+  // (test knob: CK_JACJ_TILE forces the tile size; a cell's bits do not depend on it)
+  if (const char *e = std::getenv("CK_JACJ_TILE")) tc = std::min<int64_t>(jj->threads, std::max(32, std::atoi(e) / 32 * 32));
   prm.tile_cells = (int)tc;
   const int64_t tiles = (N + tc - 1) / tc;
   const int grid = (int)std::min<int64_t>(tiles, jj->grid_max);

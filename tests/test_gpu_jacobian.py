@@ -253,3 +253,37 @@ def test_kernel_in_use_and_a_J_that_is_only_8_byte_aligned(ck, jac_kernel):
     for Jx in (Jm, Ja):
         rs, re = violations(mech, T, P, Y, Jx, Jr)
         assert rs <= 1.0 and re <= 1.0, (rs, re)
+
+
+@pytest.mark.parametrize("cfg_name,N", [("mid_1m", 148 * 224 + 1234), ("tiny_1k", 148 * 512 * 2 + 99)])
+def test_every_tile_size_gives_the_same_bits(ck, jac_kernel, monkeypatch, cfg_name, N):
+    """The specialised kernel with its tile size forced (CK_JACJ_TILE: other grids, other numbers of tiles
+    per block, other hand-offs between the out buffers, the tensor copies and the scratch) returns,
+    bit for bit, what the balanced default returns."""
+    if jac_kernel != "jit":
+        pytest.skip("specialised kernel only")
+    cfg = ckgen.CONFIGS[cfg_name]
+    mech = ckgen.mechanism(cfg.mech)
+    T, P, Y = ckgen.states(cfg, N=N)
+    dev = torch.device("cuda:0")
+    S = mech.n_species
+    Td, Pd, Yd = (torch.from_numpy(a).to(dev) for a in (T, P, Y))
+
+    def run(gm):
+        J = torch.full((N, S + 1, S + 1), float("nan"), dtype=torch.float64, device=dev)
+        gm.jacobian(Td, Pd, Yd, J, stream=torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        return J
+
+    with ck.Mechanism(mech) as gm:
+        assert gm.info("jac_kernel") == 3
+        J0 = run(gm)
+        assert torch.isfinite(J0).all()
+        for tile in (32, 96, 160, 224, 384, 512):
+            if tile > gm.info("jac_cells"):
+                continue
+            monkeypatch.setenv("CK_JACJ_TILE", str(tile))
+            J = run(gm)
+            assert torch.equal(J, J0), (cfg_name, tile)
+            del J
+        monkeypatch.delenv("CK_JACJ_TILE")

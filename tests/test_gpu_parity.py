@@ -529,6 +529,44 @@ def test_small_batch_shape_variants(ck, kernel_variant, monkeypatch):
         assert gm.info("small_batch_max") == 128 * 148    # (rate table in fp32: half the size)
 
 
+@pytest.mark.parametrize("cfg_name,N", [("mid_1m", 148 * 256 * 2 + 4321), ("large_256k", 148 * 128 + 777), ("tiny_1k", 70001)])
+def test_every_tile_size_gives_the_same_bits(ck, kernel_variant, monkeypatch, cfg_name, N):
+    """A cell's arithmetic does not depend on the tile it falls into or on how many tiles a block
+    walks: the specialised kernel with its tile size forced to 32, 64, 96, 160, ... cells (CK_JIT_TILE;
+    other grids, other numbers of tiles per block, other interleavings of the bulk loads, the
+    mbarrier phases, the pair barriers and the M-scratch slots) returns, bit for bit, what the
+    balanced default returns.  Stresses the hand-offs the parity tests only see in one schedule."""
+    if kernel_variant != "auto":
+        pytest.skip("specialised kernel only")
+    cfg = ckgen.CONFIGS[cfg_name]
+    mech = ckgen.mechanism(cfg.mech)
+    T, P, Y = ckgen.states(cfg, N=N)
+    dev = torch.device("cuda:0")
+    Td, Pd, Yd = (torch.from_numpy(a).to(dev) for a in (T, P, Y))
+    st = torch.cuda.current_stream().cuda_stream
+
+    def run(gm):
+        w = torch.full((mech.n_species, N), float("nan"), dtype=torch.float64, device=dev)
+        d = torch.full((N,), float("nan"), dtype=torch.float64, device=dev)
+        gm.source_terms(Td, Pd, Yd, w, d, stream=st)
+        torch.cuda.synchronize()
+        return w, d
+
+    with ck.Mechanism(mech) as gm:
+        assert gm.info("jit") == 1
+        w0, d0 = run(gm)
+        assert torch.isfinite(w0).all() and torch.isfinite(d0).all()
+        cells = gm.info("threads") // (2 if gm.info("pair") else 1)
+        for tile in (32, 64, 96, 160, 224, 256):
+            if tile > cells:
+                continue
+            monkeypatch.setenv("CK_JIT_TILE", str(tile))
+            for _ in range(2):
+                w, d = run(gm)
+                assert torch.equal(w, w0) and torch.equal(d, d0), (cfg_name, tile)
+        monkeypatch.delenv("CK_JIT_TILE")
+
+
 def test_error_codes(ck):
     mech = ckgen.mechanism(ckgen.MECH_TINY)
     gm = ck.Mechanism(mech)
