@@ -219,7 +219,7 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
     << "\n#define CJ_B " << B << "\n#define CJ_NBLK " << nblk << "\n#define CJ_G_TB0 " << spec.group_end[1]
     << "\n#define CJ_G_FO0 " << spec.group_end[3] << "\n#define CJ_NM " << spec.n_m << "\n#define CJ_NMB " << spec.n_mb
     << "\n#define CJ_NFO " << spec.n_fo << "\n#define CJ_NTL " << ntl << "\n#define CJ_OST " << ost
-    << "\n#define CJ_BULK " << bulk << "\n#define CJ_HINT " << hint << "\n#define CJ_MH " << (std::getenv("CK_JACJ_MH") ? std::atoi(std::getenv("CK_JACJ_MH")) : 4) << "\n#define CJ_KP " << kp << "\n#define CJ_PREF " << (std::getenv("CK_JACJ_PREF") ? std::atoi(std::getenv("CK_JACJ_PREF")) : 6) << "\n#define CJ_DISCARD " << discard << "\n#define CJ_STAGGER " << (std::getenv("CK_JACJ_STAGGER") ? std::atoi(std::getenv("CK_JACJ_STAGGER")) : 0) << "\n#define CJ_EXP " << (std::getenv("CK_JACJ_EXP") ? std::atoi(std::getenv("CK_JACJ_EXP")) : 0) << "\n";
+    << "\n#define CJ_BULK " << bulk << "\n#define CJ_HINT " << hint << "\n#define CJ_MH " << (std::getenv("CK_JACJ_MH") ? std::atoi(std::getenv("CK_JACJ_MH")) : 4) << "\n#define CJ_KP " << kp << "\n#define CJ_PREF " << (std::getenv("CK_JACJ_PREF") ? std::atoi(std::getenv("CK_JACJ_PREF")) : 6) << "\n#define CJ_DISCARD " << discard << "\n#define CJ_TIMING " << (std::getenv("CK_JACJ_TIMING") ? 1 : 0) << "\n#define CJ_NOALLOC " << (std::getenv("CK_JACJ_NOALLOC") ? std::atoi(std::getenv("CK_JACJ_NOALLOC")) : 0) << "\n#define CJ_STAGGER " << (std::getenv("CK_JACJ_STAGGER") ? std::atoi(std::getenv("CK_JACJ_STAGGER")) : 0) << "\n#define CJ_EXP " << (std::getenv("CK_JACJ_EXP") ? std::atoi(std::getenv("CK_JACJ_EXP")) : 0) << "\n";
   auto emit = [&](const char *name, const std::vector<double> &v) {
     o << "__constant__ double " << name << "[" << (v.empty() ? 1 : v.size()) << "] = {";
     for (size_t i = 0; i < v.size(); ++i) o << (i ? "," : "") << (i % 6 == 0 ? "\n  " : " ") << lit(v[i]);
