@@ -153,6 +153,46 @@ int ck_mech_create(const ck_mech_desc *desc, ck_mech **out);
 int ck_source_terms(const ck_mech *m, const double *T, const double *P, const double *Y,
                     int64_t N, double *wdot, double *dTdt, void *stream);
 
+/* ck_source_terms for callers that cannot allocate device memory: same arguments, same layout,
+ * same results to rounding (Eq. 2-11 as listed at the top of this file), but no byte of global
+ * memory beyond the handle's tables, the inputs and the outputs comes from an allocator.
+ *
+ * Who needs it: a solver that hands the whole device to its own memory pool after set-up, so that
+ * a later cudaMalloc fails or eats into memory the pool was sized without; a solver that overlaps
+ * chemistry with other work on other streams, which cudaMalloc / cudaFree would stall because they
+ * synchronise the device; a process that shares a GPU under a fixed memory budget and needs the
+ * library's footprint known up front.  Create the handle (ck_mech_create does allocate its tables)
+ * during set-up; call this from the time loop.
+ *
+ * How: it runs the table-driven kernel, one thread per cell (about 6-10 x slower than the
+ * specialised kernel of ck_source_terms; this entry point is about where the memory lives, not
+ * about speed).  That kernel's only scratch, the third-body concentrations M = C E of the cells a
+ * block works on, sits in a fixed array of 32 MiB inside the library image.  Every
+ * GPU this library's code is loaded on holds those 32 MiB until the process exits, used or not.
+ * Limit: a mechanism may have at most CK_STATIC_MAX_M_ROWS third-body + falloff reactions (rows
+ * of M); beyond that the call returns CK_EUNSUPPORTED and says so in ck_last_error(), as it does
+ * for handles with the approximate-ANN Kc or a reduced precision (those exist only in the
+ * specialised kernel).  N is not limited.
+ *
+ * First call on a device: it looks up the array's device address and sets the kernel's
+ * shared-memory limit (once per device, no allocation, but the CUDA runtime may load the
+ * library's code onto the device at that moment).  Make that first call during set-up, before any
+ * stream capture; the handle's device must be the current one (CK_EINVAL otherwise).
+ *
+ * The array is shared by all handles and all calls on a device and is divided by block index, so
+ * NOT re-entrant: two calls that can be on the GPU at the same time (different streams or host
+ * threads) overwrite each other's M values and return wrong rates without any error.  Order all
+ * calls of this function on a device on one stream (or with events).  The array keeps whatever the
+ * last call left; nothing in it needs clearing, because a block writes every M row of a tile
+ * before it reads one.  It does not interfere with ck_source_terms, ck_jacobian or
+ * ck_rk4_integrate, which keep using the handle's own scratch.
+ * Asynchronous on `stream`, deterministic run to run.  Calls no cudaMalloc, cudaFree or other
+ * allocating routine, on the first call or later.
+ * Errors: CK_EINVAL (as ck_source_terms; wrong current device), CK_EUNSUPPORTED (above), CK_ECUDA. */
+#define CK_STATIC_MAX_M_ROWS 512
+int ck_source_terms_static(const ck_mech *m, const double *T, const double *P, const double *Y,
+                           int64_t N, double *wdot, double *dTdt, void *stream);
+
 /* Same computation with HOST buffers: copies T, P, Y to the device, runs
  * ck_source_terms and copies wdot, dTdt back, then synchronises `stream`.  Batches of
  * 2^17 cells or more are split into up to 16 chunks of cells that are pipelined: a chunk's

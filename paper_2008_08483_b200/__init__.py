@@ -20,7 +20,7 @@ import numpy as np
 
 from . import _build
 
-__all__ = ["Mechanism", "CkError", "ck_mech_create", "ck_source_terms", "ck_source_terms_host",
+__all__ = ["Mechanism", "CkError", "ck_mech_create", "ck_source_terms", "ck_source_terms_static", "ck_source_terms_host",
            "ck_rk4_integrate", "ck_jacobian",
            "ck_mech_destroy", "ck_last_error", "ck_mech_info", "ck_mech_note", "ck_measure_fp64_peak", "ck_measure_peaks",
            "ck_mech_jit_source",
@@ -73,6 +73,8 @@ def _load():
     lib.ck_mech_create.argtypes = [C.POINTER(_Desc), C.POINTER(C.c_void_p)]
     lib.ck_source_terms.restype = C.c_int
     lib.ck_source_terms.argtypes = [C.c_void_p] * 4 + [C.c_int64] + [C.c_void_p] * 3
+    lib.ck_source_terms_static.restype = C.c_int
+    lib.ck_source_terms_static.argtypes = [C.c_void_p] * 4 + [C.c_int64] + [C.c_void_p] * 3
     lib.ck_source_terms_host.restype = C.c_int
     lib.ck_source_terms_host.argtypes = [C.c_void_p] * 4 + [C.c_int64] + [C.c_void_p] * 3
     lib.ck_rk4_integrate.restype = C.c_int
@@ -132,6 +134,14 @@ def ck_mech_create(desc: "_Desc") -> int:
 def ck_source_terms(handle, T, P, Y, N, wdot, dTdt, stream=0) -> None:
     _check(_lib.ck_source_terms(handle, _addr(T), _addr(P), _addr(Y), int(N), _addr(wdot),
                                 _addr(dTdt), stream or None))
+
+
+def ck_source_terms_static(handle, T, P, Y, N, wdot, dTdt, stream=0) -> None:
+    """ck_source_terms for callers that must not allocate device memory (a solver whose memory pool owns
+    the device, or one that cannot afford cudaMalloc's device-wide synchronisation in its time loop): the
+    kernel's scratch is a fixed 32 MiB array inside libck.so.  Not re-entrant; see include/ck.h."""
+    _check(_lib.ck_source_terms_static(handle, _addr(T), _addr(P), _addr(Y), int(N), _addr(wdot),
+                                       _addr(dTdt), stream or None))
 
 
 def ck_source_terms_host(handle, T, P, Y, N, wdot, dTdt, stream=0) -> None:
@@ -261,6 +271,13 @@ class Mechanism:
         if N is None:
             N = T.shape[0]
         ck_source_terms(self.handle, T, P, Y, N, wdot, dTdt, stream)
+
+    def source_terms_static(self, T, P, Y, wdot, dTdt, N=None, stream=0) -> None:
+        """source_terms without any device allocation behind it (ck_source_terms_static): device buffers,
+        asynchronous on `stream`; calls must not overlap on the GPU."""
+        if N is None:
+            N = T.shape[0]
+        ck_source_terms_static(self.handle, T, P, Y, N, wdot, dTdt, stream)
 
     def jacobian(self, T, P, Y, J, N=None, stream=0) -> None:
         """J[N, S+1, S+1] = d(wdot, dT/dt)/d(Y, T) at constant P; device buffers; asynchronous."""

@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libck.so")
-SOURCES = ["ck_api.cu", "ck_kernels.cu", "ck_jit.cu", "ck_rk4.cu", "ck_jac.cu", "ck_peaks.cu", "ck_nu.cu", "ck_jacj.cu"]
+SOURCES = ["ck_api.cu", "ck_kernels.cu", "ck_jit.cu", "ck_rk4.cu", "ck_jac.cu", "ck_peaks.cu", "ck_nu.cu", "ck_jacj.cu", "ck_static.cu"]
 HEADERS = ["ck_internal.h", "ck_program.h", "ck_jit_kernel.cuh", "ck_jit_math.cuh", "ck_nu_kernel.cuh", "ck_jac_v2.cuh", "ck_jacj_kernel.cuh"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC"]

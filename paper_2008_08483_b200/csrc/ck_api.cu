@@ -1003,6 +1003,21 @@ extern "C" int ck_source_terms(const ck_mech *m, const double *T, const double *
   return CK_OK;
 }
 
+// The no-allocation variant (ck_static.cu): argument checks here as for ck_source_terms, the kernel,
+// its static scratch and the per-device set-up there.
+extern "C" int ck_source_terms_static(const ck_mech *m, const double *T, const double *P, const double *Y,
+                                      int64_t N, double *wdot, double *dTdt, void *stream) {
+  if (!m) return fail(CK_EINVAL, "mechanism handle is NULL");
+  if (N < 0) return fail(CK_EINVAL, "N must be >= 0");
+  if (N == 0) return CK_OK;
+  if (!T || !P || !Y || !wdot || !dTdt) return fail(CK_EINVAL, "a state or result pointer is NULL");
+  if (((uintptr_t)T | (uintptr_t)P | (uintptr_t)Y | (uintptr_t)wdot | (uintptr_t)dTdt) & 7u)
+    return fail(CK_EINVAL, "pointers must be 8-byte aligned");
+  std::string err;
+  const int st = ck::static_source_terms(m, T, P, Y, N, wdot, dTdt, (cudaStream_t)stream, &err);
+  return st == CK_OK ? CK_OK : fail(st, err);
+}
+
 extern "C" int ck_jacobian(const ck_mech *m, const double *T, const double *P, const double *Y,
                            int64_t N, double *J, void *stream) {
   if (!m) return fail(CK_EINVAL, "mechanism handle is NULL");

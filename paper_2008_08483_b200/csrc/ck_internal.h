@@ -178,6 +178,11 @@ cudaError_t launch_source_terms(const ck_mech *m, const double *T, const double 
                                 const double *Y, int64_t N, double *wdot, double *dTdt,
                                 cudaStream_t stream);
 
+// ck_source_terms_static's launch (ck_static.cu): the table-driven kernel with its M scratch in a
+// file-scope device array.  Returns a ck_status; *err carries the message of a non-zero one.
+int static_source_terms(const ck_mech *m, const double *T, const double *P, const double *Y, int64_t N,
+                        double *wdot, double *dTdt, cudaStream_t stream, std::string *err);
+
 // One RK4 stage's update kernel (ck_rk4.cu); stage = 1..4.
 cudaError_t launch_rk4_stage(int stage, const ck_mech *m, const double *P, double *T0, double *Y0, double *Ts,
                              double *Ys, const double *wdot, const double *dTdt, double *accT, double *accY,
