@@ -768,10 +768,15 @@ int setup_jit(ck_mech *m, ck::JitSpec &spec, const std::string &why, size_t smem
   // M = C E scratch in slots (ck_jit_kernel.cuh): one per block that can be resident on the device.
   // Shared memory bounds the resident blocks per SM from above (registers can only lower it).
   const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(std::min<size_t>(32, 2048 / spec.threads), smem_sm / (smem + 1024)));
-  if (int st = alloc_scratch(m, m->num_sms * per_sm, (size_t)std::max(spec.n_mb, 1) * ck::kMBlock * m->jit_cells)) return st;
+  // A slot is sized for this (the main) shape; the small-batch shapes below and the RK4 stage variant
+  // work on tiles of at most as many cells and index the slots with the same stride, so slot s is the
+  // same bytes in every kernel of the handle and one set of busy flags guards it.
+  const size_t slot_elems = (size_t)std::max(spec.n_mb, 1) * ck::kMBlock * m->jit_cells;
+  if (int st = alloc_scratch(m, m->num_sms * per_sm, slot_elems)) return st;
   m->jit_params.m_scratch = m->d_scratch;
   m->jit_params.slot_busy = m->d_slot_busy;
   m->jit_params.n_slots = m->num_sms * per_sm;
+  m->jit_params.slot_elems = (int)slot_elems;
 
   // ---- the small-batch shape (CK_SPLIT = 8 threads per cell, tiles of 32 cells): one warp no longer
   //      walks the whole mechanism alone when the batch is a few thousand cells.  Same tables, same
@@ -1053,6 +1058,10 @@ extern "C" int ck_source_terms_host(ck_mech *m, const double *T, const double *P
   if (N < 0) return fail(CK_EINVAL, "N must be >= 0");
   if (N == 0) return CK_OK;
   if (!T || !P || !Y || !wdot || !dTdt) return fail(CK_EINVAL, "a state or result pointer is NULL");
+  if (!jit) {
+    const std::string err = ck::jac_ensure(m->jac);
+    if (!err.empty()) return fail(CK_ENOMEM, err);
+  }
   const int64_t S = m->dev.S;
   cudaStream_t st = (cudaStream_t)stream;
   cudaError_t ce;
@@ -1257,13 +1266,13 @@ extern "C" int64_t ck_mech_info(const ck_mech *m, int what) {
     case 13: return m->nnz_eff;
     case 14: return m->jit_kernel ? 1 : 0;
     case 15: return m->jit_kernel ? m->jit_s_reg : 0;
-    case 16: return m->jacj ? ck::jacj_cells(m->jacj) : (m->jac ? ck::jac_cells_per_tile(m->jac) : 0);
+    case 16: return (m->jacj && !ck::jacj_failed(m->jacj)) ? ck::jacj_cells(m->jacj) : (m->jac ? ck::jac_cells_per_tile(m->jac) : 0);
     case 17: return (m->jit_kernel && m->jit_spec.pair) ? 1 : 0;
     case 18: return (m->jit_kernel && m->jit_spec.kc_none) ? 1 : 0;
     case 19: return m->jit_kernel ? m->jit_spec.prec : 0;
     case 20: return m->nu ? 1 : 0;
     case 21: return m->n_split ? (int64_t)m->split_cells[m->n_split - 1] * m->num_sms : 0;
-    case 22: return m->jacj ? 3 : (m->jac ? (ck::jac_cells_per_tile(m->jac) == 32 && ck::jac_is_v2(m->jac) ? 2 : 1) : 0);
+    case 22: return (m->jacj && !ck::jacj_failed(m->jacj)) ? 3 : (m->jac ? (ck::jac_cells_per_tile(m->jac) == 32 && ck::jac_is_v2(m->jac) ? 2 : 1) : 0);
     default: return -1;
   }
 }

@@ -22,6 +22,7 @@ struct JitParams {
   double *m_scratch;
   int *slot_busy;
   int n_slots;
+  int slot_elems;              // doubles per slot, one value for every shape built on the handle
   const double *T, *P, *Y;
   double *wdot, *dTdt;
   long long N;
@@ -73,6 +74,9 @@ std::string jac_create(const ck_mech_desc *d, int num_sms, size_t smem_block_max
 void jac_destroy(JacMech *jm);
 int jac_cells_per_tile(const JacMech *jm);
 bool jac_is_v2(const JacMech *jm);
+// First launch of the second table-driven kernel: allocates its scratch ("" or the error text); a no-op later
+// and for the first kernel.
+std::string jac_ensure(JacMech *jm);
 cudaError_t jac_launch(const JacMech *jm, const double *T, const double *P, const double *Y, int64_t N,
                        double *J, cudaStream_t stream);
 
@@ -88,6 +92,8 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
 std::string jacj_ensure(JacJit *jj);
 void jacj_destroy(JacJit *jj);
 int jacj_cells(const JacJit *jj);
+// true once jacj_ensure has failed: the table-driven kernels serve the handle from then on
+bool jacj_failed(const JacJit *jj);
 // false if J is not aligned for the kernel's bulk row stores (16 bytes): the table-driven kernels take the call
 bool jacj_takes(const JacJit *jj, const double *J);
 cudaError_t jacj_launch(const JacJit *jj, const double *T, const double *P, const double *Y, int64_t N, double *J,

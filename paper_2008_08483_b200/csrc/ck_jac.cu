@@ -92,7 +92,8 @@ struct JacMech {
   int v2_mt = 0, v2_nth = 4, v2_nw = 0;
   size_t v2_smem = 0;
   void *v2_tables = nullptr;    // host copy of Jac2Tables (device pointers inside)
-  double *d_v2_scratch = nullptr;
+  double *d_v2_scratch = nullptr;   // allocated by jac_ensure
+  size_t v2_scratch_elems = 0;
   int v2_grid = 1;
   int cells = 8;               // cells per tile
   int warps = 16, minb = 1;    // warps per block, blocks per SM
@@ -721,13 +722,11 @@ std::string jac_create(const ck_mech_desc *d, int num_sms, size_t smem_block_max
       u->row_order = (const int *)(b + o_ro);
       u->ks_start = (const int *)(b + o_ks); u->coef = (const Jac2Coef *)(b + o_co); u->afrag = (const double *)(b + o_af);
       u->scratch_per_block = (size_t)4 * R * 32 + (size_t)2 * S * 32 + (size_t)nw * n1 * 32;
-      ce = cudaMalloc((void **)&jm->d_v2_scratch, (size_t)num_sms * v2_bps * u->scratch_per_block * sizeof(double));
-      if (ce != cudaSuccess) {
-        delete u;
-        jac_destroy(jm);
-        return std::string("Jacobian scratch: ") + cudaGetErrorString(ce);
-      }
-      u->scratch = jm->d_v2_scratch;
+      // (the scratch itself, num_sms * v2_bps * scratch_per_block doubles, is allocated by jac_ensure on
+      //  the first launch of this kernel: a handle whose calls all go to the specialised kernel, or that
+      //  never calls ck_jacobian, does not pay for it)
+      u->scratch = nullptr;
+      jm->v2_scratch_elems = (size_t)num_sms * v2_bps * u->scratch_per_block;
       jm->v2 = true; jm->v2_mt = v2_mt; jm->v2_nth = v2_nth; jm->v2_nw = nw; jm->v2_smem = smem2;
       jm->v2_tables = u;
       jm->v2_grid = num_sms * v2_bps;
@@ -747,6 +746,17 @@ void jac_destroy(JacMech *jm) {
 
 int jac_cells_per_tile(const JacMech *jm) { return jm->v2 ? 32 : jm->cells; }
 bool jac_is_v2(const JacMech *jm) { return jm->v2; }
+
+std::string jac_ensure(JacMech *jm) {
+  if (!jm->v2 || jm->d_v2_scratch) return "";
+  const cudaError_t ce = cudaMalloc((void **)&jm->d_v2_scratch, jm->v2_scratch_elems * sizeof(double));
+  if (ce != cudaSuccess) {
+    cudaGetLastError();
+    return std::string("Jacobian scratch: ") + cudaGetErrorString(ce);
+  }
+  ((Jac2Tables *)jm->v2_tables)->scratch = jm->d_v2_scratch;
+  return "";
+}
 
 cudaError_t jac_launch(const JacMech *jm, const double *T, const double *P, const double *Y, int64_t N,
                        double *J, cudaStream_t stream) {

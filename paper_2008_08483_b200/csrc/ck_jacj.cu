@@ -436,6 +436,7 @@ void jacj_destroy(JacJit *jj) {
 
 int jacj_cells(const JacJit *jj) { return jj->threads; }
 bool jacj_takes(const JacJit *jj, const double *J) { return jj->bulk == 0 || ((uintptr_t)J & 15u) == 0; }
+bool jacj_failed(const JacJit *jj) { return !jj->ready && !jj->error.empty(); }
 
 cudaError_t jacj_launch(const JacJit *jj, const double *T, const double *P, const double *Y, int64_t N, double *J,
                         cudaStream_t stream) {

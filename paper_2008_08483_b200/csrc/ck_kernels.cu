@@ -56,6 +56,7 @@ source_terms_kernel(const DeviceMech m, const double *__restrict__ Tg, const dou
   if (tid == 0) {
     int s = blockIdx.x % m.n_slots;
     while (atomicCAS(m.slot_busy + s, 0, 1) != 0) s = (s + 1 == m.n_slots) ? 0 : s + 1;
+    __threadfence();   // acquire: the last owner's stores are ordered before this block's
     s_slot = s;
   }
   __syncthreads();
@@ -166,7 +167,10 @@ source_terms_kernel(const DeviceMech m, const double *__restrict__ Tg, const dou
     if (valid) dTdt[i] = -(T * hw) / (rho * cp_sum);
   }
   __syncthreads();
-  if (tid == 0) atomicExch(m.slot_busy + s_slot, 0);
+  if (tid == 0) {
+    __threadfence();   // release: the block's accesses to the slot end before the flag clears
+    atomicExch(m.slot_busy + s_slot, 0);
+  }
 }
 
 }  // namespace

@@ -180,17 +180,20 @@ def full_batch_parity(ck, mech, T, P, Y, label, variants=("auto", "generic"), ho
                     # the bound taken on the sum's own scale, and no farther from a long-double
                     # evaluation than that bound allows (the fp64 oracle is itself off by ~1e-15 kappa).
                     over, kappa, ratio = dTdt_conditioned_violations(mech, T, dg, wr, dr)
-                    exact = longdouble_dTdt(mech, T[over[:32]], P[over[:32]], Y[:, over[:32]])
-                    e_gpu = np.abs((dg[over[:32]] - exact) / exact).astype(float)
-                    e_orc = np.abs((dr[over[:32]] - exact) / exact).astype(float)
+                    # (few first: that also bounds the work of the long-double arbiter, which then takes
+                    #  EVERY such cell, not a sample of them)
+                    assert over.size <= max(1, N // 20000), (label, variant, what, over.size)
+                    exact = longdouble_dTdt(mech, T[over], P[over], Y[:, over])
+                    e_gpu = np.abs((dg[over] - exact) / exact).astype(float)
+                    e_orc = np.abs((dr[over] - exact) / exact).astype(float)
                     print("%s [%s, %s]: %d of %d cells over the north_star dT/dt bound, all by cancellation: "
                           "kappa %.3g .. %.3g, worst err / Q19 bound %.3g; against long double: GPU rel err "
-                          "%.3g, fp64 oracle rel err %.3g (worst of the first %d)"
+                          "%.3g, fp64 oracle rel err %.3g (worst of all %d)"
                           % (label, variant, what, over.size, N, kappa.min(), kappa.max(), ratio.max(),
                              e_gpu.max(), e_orc.max(), e_gpu.size))
-                    assert over.size <= max(1, N // 20000) and kappa.min() > 1e3 and ratio.max() <= 1.0, \
+                    assert kappa.min() > 1e3 and ratio.max() <= 1.0, \
                         (label, variant, what, over.size, kappa.min(), ratio.max())
-                    assert (e_gpu <= 1e-10 + 1e-14 * kappa[:32]).all()
+                    assert (e_gpu <= 1e-10 + 1e-14 * kappa).all()
                 worst_w, worst_t = max(worst_w, rw), max(worst_t, rt)
     finally:
         if saved is None:
@@ -480,6 +483,81 @@ def test_concurrent_calls_on_two_streams_share_one_handle(ck, cfg_name, N):
 
 
 @pytest.mark.parametrize("N", [1, 31, 32, 33, 256, 1000, 4096, 4736, 4737, 9472, 9473, 18944, 18945])
+@pytest.mark.parametrize("N_a,N_b", [(2048, 40000), (3000, 8000), (4736, 4737), (9472, 9473), (777, 300000)])
+def test_concurrent_calls_of_different_shapes_share_one_handle(ck, kernel_variant, N_a, N_b):
+    """The kernel shapes built on one handle (8 and 4 threads per cell for small batches, thread <-> cell
+    beyond) share the M = C E scratch and its busy flags, so slot s has to be the same bytes in all of
+    them: two streams launch calls that select DIFFERENT shapes on one handle at the same time, over and
+    over; every result is bitwise what the call gives alone (and that one matches the oracle)."""
+    cfg = ckgen.CONFIGS["mid_1m"]
+    mech = ckgen.mechanism(cfg.mech)
+    S = mech.n_species
+    dev = torch.device("cuda:0")
+    om = oracle.OracleMechanism(mech)
+    batches = [ckgen.states(cfg, N=n, seed_offset=o) for o, n in enumerate((N_a, N_b))]
+    with ck.Mechanism(mech) as gm:
+        if kernel_variant == "auto":
+            assert gm.info("small_batch_max") == 9472
+        alone = [gpu_run(ck, mech, *b, gm) for b in batches]
+        for b, (wa, da) in zip(batches, alone):
+            n = min(b[0].shape[0], 4000)          # (the oracle on a sample; full batches have their own tests)
+            wr, dr, _ = oracle.source_terms(om, b[0][:n], b[1][:n], np.ascontiguousarray(b[2][:, :n]))
+            rw, rt = parity_violations(wa[:, :n], da[:n], wr, dr)
+            assert rw <= 1.0 and rt <= 1.0, (N_a, N_b, rw, rt)
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        bufs = []
+        for b, st in zip(batches, streams):
+            with torch.cuda.stream(st):
+                Td, Pd, Yd = (torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in b)
+                w = torch.empty((S, b[0].shape[0]), dtype=torch.float64, device=dev)
+                d = torch.empty((b[0].shape[0],), dtype=torch.float64, device=dev)
+            bufs.append((Td, Pd, Yd, w, d))
+        torch.cuda.synchronize()
+        # the shorter call is repeated more often so that both streams stay busy for about as long
+        reps = [max(1, int(25 * max(N_a, N_b) / max(n, 8192))) for n in (N_a, N_b)]
+        for rep in range(max(reps)):
+            for (Td, Pd, Yd, w, d), st, r in zip(bufs, streams, reps):
+                if rep < r:
+                    gm.source_terms(Td, Pd, Yd, w, d, stream=st.cuda_stream)
+        torch.cuda.synchronize()
+        for (Td, Pd, Yd, w, d), (wa, da) in zip(bufs, alone):
+            assert np.array_equal(w.cpu().numpy(), wa) and np.array_equal(d.cpu().numpy(), da)
+
+
+def test_source_terms_beside_rk4_on_one_handle(ck, kernel_variant):
+    """ck_rk4_integrate's stage kernels take their M = C E slots from the same scratch and flags as
+    ck_source_terms: a reactor run on one stream and source-term calls of a small-batch shape on another,
+    on ONE handle, both give the bits they give alone."""
+    from helpers import tame
+    cfg = ckgen.CONFIGS["mid_rk4"]
+    mech = tame(ckgen.mechanism(cfg.mech))
+    S = mech.n_species
+    dev = torch.device("cuda:0")
+    N_rk, N_st, steps, dt = 20000, 3000, 12, 1e-9
+    Tr, Pr, Yr = ckgen.states(cfg, N=N_rk, seed_offset=3)
+    Ts, Ps, Ys = ckgen.states(cfg, N=N_st, seed_offset=4)
+    put = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    with ck.Mechanism(mech) as gm:
+        w_alone, d_alone = gpu_run(ck, mech, Ts, Ps, Ys, gm)
+        T1, P1, Y1 = put(Tr), put(Pr), put(Yr)
+        gm.rk4_integrate(T1, P1, Y1, dt, steps, use_graph=False)
+        torch.cuda.synchronize()
+        T_alone, Y_alone = T1.cpu().numpy(), Y1.cpu().numpy()
+        assert np.isfinite(T_alone).all() and np.isfinite(Y_alone).all()
+        sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+        T2, P2, Y2 = put(Tr), put(Pr), put(Yr)
+        Td, Pd, Yd = put(Ts), put(Ps), put(Ys)
+        w = torch.empty((S, N_st), dtype=torch.float64, device=dev)
+        d = torch.empty((N_st,), dtype=torch.float64, device=dev)
+        torch.cuda.synchronize()
+        gm.rk4_integrate(T2, P2, Y2, dt, steps, use_graph=False, stream=sa.cuda_stream)
+        for rep in range(40):
+            gm.source_terms(Td, Pd, Yd, w, d, stream=sb.cuda_stream)
+        torch.cuda.synchronize()
+        assert np.array_equal(T2.cpu().numpy(), T_alone) and np.array_equal(Y2.cpu().numpy(), Y_alone)
+        assert np.array_equal(w.cpu().numpy(), w_alone) and np.array_equal(d.cpu().numpy(), d_alone)
+
+
 def test_small_batch_shape_is_selected_and_matches_the_oracle(ck, kernel_variant, N):
     """Below one wave of 32-cell tiles (N <= 32 x 148) ck_source_terms runs the small-batch shape of
     the specialised kernel: 8 threads per cell taking alternate reaction blocks, partial accumulators
