@@ -42,7 +42,8 @@ _lib = None
 def _load():
     global _lib
     if _lib is None:
-        lib = C.CDLL(_build())
+        # (CK_ORACLE_LIB: another build of the same sources, e.g. the sanitizer build of oracle/build.py)
+        lib = C.CDLL(os.environ.get("CK_ORACLE_LIB") or _build())
         lib.ck_oracle_source_terms.restype = C.c_int
         lib.ck_oracle_source_terms.argtypes = [C.POINTER(_Mech), _dp, _dp, _dp, C.c_int64,
                                                _dp, _dp, C.c_int]

@@ -25,5 +25,17 @@ def build(force: bool = False) -> str:
     return LIB
 
 
+def build_sanitized(outdir: str) -> str:
+    """The same sources with AddressSanitizer and UndefinedBehaviorSanitizer, into `outdir` (SURVEY.md
+    section 5): loaded instead of the normal build when CK_ORACLE_LIB names it, in a process that has
+    libasan preloaded (tests/test_oracle_sanitized.py)."""
+    lib = os.path.join(outdir, "libck_oracle_san.so")
+    cmd = ["gcc", "-O1", "-g", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra",
+           "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer",
+           "-o", lib, SRC, SRC_JAC, "-lm"]
+    subprocess.run(cmd, check=True, cwd=HERE)
+    return lib
+
+
 if __name__ == "__main__":
     print(build(force=True))
