@@ -199,7 +199,7 @@ int ck_source_terms_static(const ck_mech *m, const double *T, const double *P, c
  * rows are copied up on a stream owned by the handle while the previous chunk computes on
  * `stream` and the one before is copied back on a second owned stream; the work starts
  * after everything queued on `stream` at the call and `stream` ends after the last copy
- * (environment CK_HOST_CHUNKS=n overrides the chunk count, 1 = everything on `stream`).
+ * (environment CK_HOST_CHUNKS=n, read by ck_mech_create, overrides the chunk count, 1 = everything on `stream`).
  * Pinned host memory makes the copies asynchronous; pageable memory also works.
  * Device staging buffers, the two copy streams and their events are owned by the handle and grow
  * on demand: unlike ck_source_terms, calls of this function on ONE handle must not overlap. */
@@ -272,7 +272,10 @@ const char *ck_last_error(void);
  *       block works on half that many cells),
  *       18 1 if the handle was built as a measurement-only ABLATION whose results are not the
  *       source term (environment CK_JIT_KC=none together with CK_ALLOW_ABLATION=1: the
- *       equilibrium layer removed, used by bench.py --ann to cost that layer); 0 otherwise,
+ *       equilibrium layer removed, used by bench.py --ann to cost that layer; or CK_JACJ_EXP /
+ *       CK_JACJ_TIMING with CK_ALLOW_ABLATION=1: the specialised Jacobian kernel with passes skipped or
+ *       printing cycle counters, J is then not the Jacobian; without CK_ALLOW_ABLATION=1 ck_mech_create
+ *       refuses all of these with CK_EINVAL); 0 otherwise,
  *       19 the handle's precision (CK_PREC_*),
  *       20 1 if ck_source_terms runs the all-DMMA small-mechanism kernel (environment
  *       CK_JIT_NU=dmma, at most 16 species and 64 reactions: every contraction of Eq. 2 and 4

@@ -828,6 +828,11 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   ce = cudaGetDeviceProperties(&prop, m->device);
   if (ce != cudaSuccess) { delete m; return fail_cuda(ce, "cudaGetDeviceProperties"); }
   m->num_sms = prop.multiProcessorCount;
+  // environment knobs of the per-call paths, read here once (see ck_mech in ck_internal.h)
+  m->env_tile = env_int("CK_JIT_TILE", 0);
+  m->env_host_chunks = env_int("CK_HOST_CHUNKS", 0);
+  m->env_rk4_fused = env_int("CK_RK4_FUSED", 1) != 0;
+  { const char *e = std::getenv("CK_JAC_KERNEL"); m->env_jac_v3_required = e && std::string(e) == "v3"; }
 
   // ---- launch shape: as many resident cells per SM as shared memory allows ----------
   int best_threads = 0, best_bps = 0;
@@ -927,10 +932,19 @@ extern "C" int ck_mech_create(const ck_mech_desc *d, ck_mech **out) {
   {
     const char *e = std::getenv("CK_JAC_KERNEL");
     const std::string which = e ? e : "";
+    // CK_JACJ_EXP skips passes of the kernel or feeds it constants, CK_JACJ_TIMING makes it print cycle
+    // counters: measurement-only builds whose J is not the Jacobian, behind the same guard as CK_JIT_KC=none
+    const bool jac_ablation = env_int("CK_JACJ_EXP", 0) != 0 || std::getenv("CK_JACJ_TIMING") != nullptr;
+    if (jac_ablation && env_int("CK_ALLOW_ABLATION", 0) != 1) {
+      ck_mech_destroy(m);
+      return fail(CK_EINVAL, "CK_JACJ_EXP / CK_JACJ_TIMING build a measurement-only Jacobian kernel whose results "
+                             "are not the Jacobian; set CK_ALLOW_ABLATION=1 to build it");
+    }
     if (which != "v1" && which != "v2" && m->jac) {
       m->jacj_note = ck::jacj_create(d, spec, hb.jit_tab, m->jit_params.thermo, m->jit_params.logtab,
                                      m->jit_params.eff_frag, m->device, m->num_sms,
                                      (size_t)prop.sharedMemPerBlockOptin, &m->jacj);
+      m->jac_ablation = jac_ablation && m->jacj;
       if (!m->jacj && which == "v3") {
         const std::string why = m->jacj_note;
         ck_mech_destroy(m);
@@ -1040,10 +1054,13 @@ extern "C" int ck_jacobian(const ck_mech *m, const double *T, const double *P, c
   if (jit) {
     const std::string err = ck::jacj_ensure(m->jacj);
     if (!err.empty()) {
-      const char *e = std::getenv("CK_JAC_KERNEL");
-      if (e && std::string(e) == "v3") return fail(CK_EUNSUPPORTED, "CK_JAC_KERNEL=v3 but " + err);
+      if (m->env_jac_v3_required) return fail(CK_EUNSUPPORTED, "CK_JAC_KERNEL=v3 but " + err);
       jit = false;
     }
+  }
+  if (!jit) {
+    const std::string err = ck::jac_ensure(m->jac);
+    if (!err.empty()) return fail(CK_ENOMEM, err);
   }
   const cudaError_t ce = jit ? ck::jacj_launch(m->jacj, T, P, Y, N, J, (cudaStream_t)stream)
                              : ck::jac_launch(m->jac, T, P, Y, N, J, (cudaStream_t)stream);
@@ -1058,10 +1075,6 @@ extern "C" int ck_source_terms_host(ck_mech *m, const double *T, const double *P
   if (N < 0) return fail(CK_EINVAL, "N must be >= 0");
   if (N == 0) return CK_OK;
   if (!T || !P || !Y || !wdot || !dTdt) return fail(CK_EINVAL, "a state or result pointer is NULL");
-  if (!jit) {
-    const std::string err = ck::jac_ensure(m->jac);
-    if (!err.empty()) return fail(CK_ENOMEM, err);
-  }
   const int64_t S = m->dev.S;
   cudaStream_t st = (cudaStream_t)stream;
   cudaError_t ce;
@@ -1077,7 +1090,7 @@ extern "C" int ck_source_terms_host(ck_mech *m, const double *T, const double *P
   // Each chunk has its own compact SoA region of the staging buffer: T | P | Y[S] | wdot[S] | dTdt.
   int64_t n_chunks = N / 65536;
   if (n_chunks > CK_HOST_CHUNKS) n_chunks = CK_HOST_CHUNKS;
-  if (const char *e = std::getenv("CK_HOST_CHUNKS")) n_chunks = std::atoi(e);
+  if (m->env_host_chunks) n_chunks = m->env_host_chunks;
   if (n_chunks < 1) n_chunks = 1;
   if (n_chunks > CK_HOST_CHUNKS) n_chunks = CK_HOST_CHUNKS;
   if (n_chunks > 1 && !m->host_in) {
@@ -1137,7 +1150,7 @@ void ensure_rk4_kernel(ck_mech *m) {
   if (m->rk4_tried) return;
   m->rk4_tried = true;
   if (!m->jit_kernel || m->jit_spec.pair) return;   // (the two-threads-per-cell kernel has no stage variant)
-  if (const char *e = std::getenv("CK_RK4_FUSED")) if (std::atoi(e) == 0) return;
+  if (!m->env_rk4_fused) return;
   ck::JitSpec spec = m->jit_spec;
   spec.rk4 = true;
   std::vector<char> cubin;
@@ -1161,7 +1174,7 @@ int jit_tiling(const ck_mech *m, int64_t N, int *tile_cells) {
   const int64_t waves = ((N + nt - 1) / nt + m->jit_grid_max - 1) / m->jit_grid_max;
   int64_t tc = (N + m->jit_grid_max * waves - 1) / (m->jit_grid_max * waves);
   tc = std::min<int64_t>(nt, (tc + 31) / 32 * 32);
-  if (const char *e = std::getenv("CK_JIT_TILE")) tc = std::min<int64_t>(nt, std::max(32, std::atoi(e) / 32 * 32));
+  if (m->env_tile) tc = std::min<int64_t>(nt, std::max(32, m->env_tile / 32 * 32));   // (test knob, read at create)
   *tile_cells = (int)tc;
   return (int)std::min<int64_t>((N + tc - 1) / tc, m->jit_grid_max);
 }
@@ -1268,7 +1281,7 @@ extern "C" int64_t ck_mech_info(const ck_mech *m, int what) {
     case 15: return m->jit_kernel ? m->jit_s_reg : 0;
     case 16: return (m->jacj && !ck::jacj_failed(m->jacj)) ? ck::jacj_cells(m->jacj) : (m->jac ? ck::jac_cells_per_tile(m->jac) : 0);
     case 17: return (m->jit_kernel && m->jit_spec.pair) ? 1 : 0;
-    case 18: return (m->jit_kernel && m->jit_spec.kc_none) ? 1 : 0;
+    case 18: return ((m->jit_kernel && m->jit_spec.kc_none) || m->jac_ablation) ? 1 : 0;
     case 19: return m->jit_kernel ? m->jit_spec.prec : 0;
     case 20: return m->nu ? 1 : 0;
     case 21: return m->n_split ? (int64_t)m->split_cells[m->n_split - 1] * m->num_sms : 0;

@@ -156,6 +156,7 @@ struct ck_mech {
   ck::JacMech *jac = nullptr;
   ck::JacJit *jacj = nullptr;   // the mechanism-specialised Jacobian kernel, used when present
   std::string jacj_note;        // why it is not, if so
+  bool jac_ablation = false;    // it was built with CK_JACJ_EXP / CK_JACJ_TIMING (CK_ALLOW_ABLATION=1): J is not the Jacobian
   // all-DMMA small-mechanism kernel (CK_JIT_NU=dmma), used by ck_source_terms when present
   ck::NuMech *nu = nullptr;
   // staging for ck_source_terms_host
@@ -169,6 +170,12 @@ struct ck_mech {
   double *d_rk4 = nullptr;
   int64_t rk4_cells = 0;
   cudaGraphExec_t rk4_graph = nullptr;
+  // Environment knobs of the calls below, read ONCE by ck_mech_create: the asynchronous entry points
+  // (ck_source_terms, ck_jacobian, ck_rk4_integrate, ck_source_terms_host) never call getenv.
+  int env_tile = 0;               // CK_JIT_TILE: forced tile size of the specialised kernel (test knob; 0 = balanced)
+  int env_host_chunks = 0;        // CK_HOST_CHUNKS (0 = unset: by batch size)
+  bool env_rk4_fused = true;      // CK_RK4_FUSED=0: unfused RK4 stages
+  bool env_jac_v3_required = false;   // CK_JAC_KERNEL=v3: a failed specialisation is an error
   const void *rk4_key[3] = {nullptr, nullptr, nullptr};   // T, P, Y the graph was captured for
   int64_t rk4_key_N = 0;
   double rk4_key_dt = 0.0;

@@ -96,6 +96,7 @@ struct JacJit {
   std::string src, error;
   std::vector<double> tab16, bfrag;
   bool ready = false;
+  int env_tile = 0;            // CK_JACJ_TILE at create time (0 = balanced tiles)
   std::mutex mu;
 };
 
@@ -371,6 +372,7 @@ std::string jacj_create(const ck_mech_desc *d, const JitSpec &spec, const std::v
   jj->bfrag.swap(bfrag);
   jj->scr_rows = (size_t)4 * RP + (size_t)2 * spec.n_mb * 8 + (size_t)3 * S;
   jj->device = device;
+  if (const char *e = std::getenv("CK_JACJ_TILE")) jj->env_tile = std::atoi(e);
   jj->threads = NT; jj->grid_max = num_sms; jj->smem = smem; jj->n1 = n1; jj->bulk = bulk;
   jj->prm.eff_frag = d_eff_frag; jj->prm.thermo = d_thermo; jj->prm.logtab = d_logtab;
   *out = jj;
@@ -434,9 +436,9 @@ void jacj_destroy(JacJit *jj) {
   delete jj;
 }
 
+bool jacj_failed(const JacJit *jj) { return !jj->ready && !jj->error.empty(); }
 int jacj_cells(const JacJit *jj) { return jj->threads; }
 bool jacj_takes(const JacJit *jj, const double *J) { return jj->bulk == 0 || ((uintptr_t)J & 15u) == 0; }
-bool jacj_failed(const JacJit *jj) { return !jj->ready && !jj->error.empty(); }
 
 cudaError_t jacj_launch(const JacJit *jj, const double *T, const double *P, const double *Y, int64_t N, double *J,
                         cudaStream_t stream) {
@@ -448,8 +450,8 @@ cudaError_t jacj_launch(const JacJit *jj, const double *T, const double *P, cons
   const int64_t waves = (N + per_wave - 1) / per_wave;
   int64_t tc = (N + waves * jj->grid_max - 1) / (waves * jj->grid_max);
   tc = std::min<int64_t>(jj->threads, (tc + 31) / 32 * 32);
-  // (test knob: CK_JACJ_TILE forces the tile size; a cell's bits do not depend on it)
-  if (const char *e = std::getenv("CK_JACJ_TILE")) tc = std::min<int64_t>(jj->threads, std::max(32, std::atoi(e) / 32 * 32));
+  // (test knob: CK_JACJ_TILE, read at ck_mech_create, forces the tile size; a cell's bits do not depend on it)
+  if (jj->env_tile) tc = std::min<int64_t>(jj->threads, std::max(32, jj->env_tile / 32 * 32));
   prm.tile_cells = (int)tc;
   const int64_t tiles = (N + tc - 1) / tc;
   const int grid = (int)std::min<int64_t>(tiles, jj->grid_max);

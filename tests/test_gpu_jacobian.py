@@ -279,11 +279,13 @@ def test_every_tile_size_gives_the_same_bits(ck, jac_kernel, monkeypatch, cfg_na
         assert gm.info("jac_kernel") == 3
         J0 = run(gm)
         assert torch.isfinite(J0).all()
-        for tile in (32, 96, 160, 224, 384, 512):
-            if tile > gm.info("jac_cells"):
-                continue
-            monkeypatch.setenv("CK_JACJ_TILE", str(tile))
+        cells = gm.info("jac_cells")
+    for tile in (32, 96, 160, 224, 384, 512):
+        if tile > cells:
+            continue
+        monkeypatch.setenv("CK_JACJ_TILE", str(tile))      # (read by ck_mech_create, not by the call)
+        with ck.Mechanism(mech) as gm:
             J = run(gm)
-            assert torch.equal(J, J0), (cfg_name, tile)
-            del J
-        monkeypatch.delenv("CK_JACJ_TILE")
+        assert torch.equal(J, J0), (cfg_name, tile)
+        del J
+    monkeypatch.delenv("CK_JACJ_TILE")

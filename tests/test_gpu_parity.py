@@ -163,9 +163,10 @@ def full_batch_parity(ck, mech, T, P, Y, label, variants=("auto", "generic"), ho
                 results = [("device", w.cpu().numpy(), d.cpu().numpy())]
                 del w, d
                 for chunks in (host_chunks if variant == "auto" else ()):
-                    os.environ["CK_HOST_CHUNKS"] = str(chunks)
+                    os.environ["CK_HOST_CHUNKS"] = str(chunks)      # (read by ck_mech_create)
                     try:
-                        wh, dh = gm.source_terms_host(T, P, Y)
+                        with ck.Mechanism(mech) as gh:
+                            wh, dh = gh.source_terms_host(T, P, Y)
                     finally:
                         del os.environ["CK_HOST_CHUNKS"]
                     results.append(("host, %d chunks" % chunks, wh, dh))
@@ -482,7 +483,6 @@ def test_concurrent_calls_on_two_streams_share_one_handle(ck, cfg_name, N):
             assert rw <= 1.0 and rt <= 1.0, (cfg_name, rw, rt)
 
 
-@pytest.mark.parametrize("N", [1, 31, 32, 33, 256, 1000, 4096, 4736, 4737, 9472, 9473, 18944, 18945])
 @pytest.mark.parametrize("N_a,N_b", [(2048, 40000), (3000, 8000), (4736, 4737), (9472, 9473), (777, 300000)])
 def test_concurrent_calls_of_different_shapes_share_one_handle(ck, kernel_variant, N_a, N_b):
     """The kernel shapes built on one handle (8 and 4 threads per cell for small batches, thread <-> cell
@@ -558,6 +558,7 @@ def test_source_terms_beside_rk4_on_one_handle(ck, kernel_variant):
         assert np.array_equal(w.cpu().numpy(), w_alone) and np.array_equal(d.cpu().numpy(), d_alone)
 
 
+@pytest.mark.parametrize("N", [1, 31, 32, 33, 256, 1000, 4096, 4736, 4737, 9472, 9473, 18944, 18945])
 def test_small_batch_shape_is_selected_and_matches_the_oracle(ck, kernel_variant, N):
     """Below one wave of 32-cell tiles (N <= 32 x 148) ck_source_terms runs the small-batch shape of
     the specialised kernel: 8 threads per cell taking alternate reaction blocks, partial accumulators
@@ -635,14 +636,35 @@ def test_every_tile_size_gives_the_same_bits(ck, kernel_variant, monkeypatch, cf
         w0, d0 = run(gm)
         assert torch.isfinite(w0).all() and torch.isfinite(d0).all()
         cells = gm.info("threads") // (2 if gm.info("pair") else 1)
-        for tile in (32, 64, 96, 160, 224, 256):
-            if tile > cells:
-                continue
-            monkeypatch.setenv("CK_JIT_TILE", str(tile))
+    for tile in (32, 64, 96, 160, 224, 256):
+        if tile > cells:
+            continue
+        monkeypatch.setenv("CK_JIT_TILE", str(tile))           # (read by ck_mech_create, not by the call)
+        with ck.Mechanism(mech) as gm:
             for _ in range(2):
                 w, d = run(gm)
                 assert torch.equal(w, w0) and torch.equal(d, d0), (cfg_name, tile)
-        monkeypatch.delenv("CK_JIT_TILE")
+    monkeypatch.delenv("CK_JIT_TILE")
+
+
+@pytest.mark.parametrize("knob,value", [("CK_JIT_KC", "none"), ("CK_JACJ_EXP", "1"), ("CK_JACJ_TIMING", "1")])
+def test_result_changing_knobs_are_refused_without_the_ablation_switch(ck, monkeypatch, kernel_variant, knob, value):
+    """Environment knobs that make a kernel compute something other than the source term or the Jacobian
+    (measurement-only ablations) are refused by ck_mech_create unless CK_ALLOW_ABLATION=1 is set as well,
+    and a handle built with them says so through ck_mech_info 18 ("ablation")."""
+    if kernel_variant != "auto":
+        pytest.skip("the knobs exist only in the specialised kernels")
+    mech = ckgen.mechanism(ckgen.MECH_TINY)
+    with ck.Mechanism(mech) as gm:
+        assert gm.info("ablation") == 0
+    monkeypatch.setenv(knob, value)
+    with pytest.raises(ck.CkError) as e:
+        ck.Mechanism(mech)
+    assert e.value.status == 1 and "CK_ALLOW_ABLATION" in str(e.value)
+    if knob != "CK_JACJ_TIMING":            # (that one makes the kernel print: not built here)
+        monkeypatch.setenv("CK_ALLOW_ABLATION", "1")
+        with ck.Mechanism(mech) as gm:
+            assert gm.info("ablation") == 1
 
 
 def test_error_codes(ck):
