@@ -44,7 +44,7 @@ def dTdt_conditioned_violations(mech, T, dTdt, wdot_ref, dTdt_ref):
     """DESIGN.md reading Q19.  The north_star bound |d dT/dt| <= 1e-10 |dT/dt| + 1e-12 K/s is purely
     relative, but dT/dt is a sum of S terms h_k wdot_k that cancel: with condition number kappa a
     relative error eps of the rates becomes kappa * eps in dT/dt, and the fp64 ORACLE itself is then
-    off the exact value by more than the bound (measured: 2.2e-10 at kappa = 7.4e4, against a
+    off the exact value by more than the bound (measured: 1.65e-10 at kappa = 7.4e4, against a
     long-double evaluation).  For cells that break the north_star bound on dT/dt ALONE the decision is
     taken against the sum's own scale, as the north_star does for wdot (relative to max_k |wdot_k|):
         |d dT/dt| <= 1e-10 |dT/dt| + 1e-12 + 1e-14 sum_k |h_k wdot_k| / (rho cp)

@@ -211,6 +211,97 @@ def test_bench_size_properties_and_sampled_parity(ck, cfg_name, N):
     assert rs <= 1.0 and re <= 1.0, (rs, re)
 
 
+def violations_vectorised(mech, T, P, Y, J, Jr):
+    """`violations` for large batches: the same two bounds, the energy row's scale from numpy
+    expressions of rho, cp and h (tolerance scales only; no oracle value is replaced)."""
+    from helpers import nasa_h_RT
+    S = mech.n_species
+    col = np.abs(Jr[:, :S, :]).max(axis=1, keepdims=True)
+    tol = 1e-9 * col + 1e-11 * np.abs(Jr[:, :S, :])
+    rs = float((np.abs(J[:, :S, :] - Jr[:, :S, :]) / np.maximum(tol, 1e-300)).max())
+    H = (nasa_h_RT(mech, T) * RU * T[None, :]).T                         # [N, S]
+    yw = np.maximum(Y, 0.0) / mech.mol_weight[:, None]                   # [S, N]
+    rho = P / (RU * T * yw.sum(0))
+    Tn = T[None, :]
+    low = Tn <= mech.T_mid[:, None]
+    cp = lambda a: a[:, 0, None] + a[:, 1, None] * Tn + a[:, 2, None] * Tn**2 + a[:, 3, None] * Tn**3 + a[:, 4, None] * Tn**4
+    cp_mass = (yw * np.where(low, cp(mech.nasa_lo), cp(mech.nasa_hi)) * RU).sum(0)
+    D = rho * cp_mass
+    scale = np.einsum("ns,nsl->nl", np.abs(H), np.abs(Jr[:, :S, :])) / D[:, None] + np.abs(Jr[:, S, :])
+    re = float((np.abs(J[:, S, :] - Jr[:, S, :]) / (1e-9 * scale)).max())
+    return rs, re
+
+
+def composition_scale(mech, om, T, P, Y, k, l):
+    """DESIGN.md reading Q20.  An entry of a species row and a composition column is
+        J_kl = sum_j nu_kj [ q_f,j (nu'_lj / Y_l - sum_i nu'_ij W_mix / W_l)
+                            - q_r,j (nu''_lj / Y_l - sum_i nu''_ij W_mix / W_l) ] + (third-body, falloff terms):
+    C_i = rho Y_i / W_i with rho ~ W_mix at constant P, so every reaction's derivative is a DIFFERENCE of the
+    direct term nu_l / Y_l and the density term (sum nu) W_mix / W_l.  Where the two nearly coincide the fp64
+    oracle's own rounding of that difference is about 2^-53 of the terms, not of the result.  Returns the scale
+    of the terms, sum_j |nu_kj| [ q_f (nu'_l / Y_l + sum nu' W_mix / W_l) + q_r (...'') ], from the oracle's
+    q_f, q_r of one cell (the third-body and falloff terms would only add to it)."""
+    det = oracle.cell_detail(om, T, P, Y)
+    W = mech.mol_weight
+    Wmix = 1.0 / (Y / W).sum()
+    nu1, nu2 = mech.nu_reac, mech.nu_prod
+    tf, sf = nu1[l] / Y[l], nu1.sum(0) * Wmix / W[l]
+    tr, sr = nu2[l] / Y[l], nu2.sum(0) * Wmix / W[l]
+    return float((np.abs(nu2[k] - nu1[k]) * (det["qf"] * (tf + sf) + det["qr"] * (tr + sr))).sum())
+
+
+@pytest.mark.parametrize("cfg_name,N", [("tiny_1m", 1 << 20), ("mid_1m", 1 << 16), ("large_256k", 1 << 14)])
+def test_every_entry_at_the_sizes_bench_times(ck, jac_kernel, cfg_name, N):
+    """Every entry of every cell's matrix against the oracle's Jacobian at the batch sizes
+    bench.py --jacobian times (2^20 cells at S=9, 2^16 at S=53, 2^14 at S=111), in the launch
+    configuration it times (one ck_jacobian call over the whole batch), compared chunk by chunk."""
+    if jac_kernel != "jit":
+        pytest.skip("the kernel bench.py times is the default one; the table-driven kernels have test_parity_all_entries")
+    cfg = ckgen.CONFIGS[cfg_name]
+    mech = ckgen.mechanism(cfg.mech)
+    om = oracle.OracleMechanism(mech)
+    S = mech.n_species
+    T, P, Y = ckgen.states(cfg, N=N)
+    dev = torch.device("cuda:0")
+    Td, Pd, Yd = (torch.from_numpy(a).to(dev) for a in (T, P, Y))
+    J = torch.full((N, S + 1, S + 1), float("nan"), dtype=torch.float64, device=dev)
+    with ck.Mechanism(mech) as gm:
+        gm.jacobian(Td, Pd, Yd, J, stream=torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+    assert torch.isfinite(J).all()
+    chunk = max(1024, (1 << 26) // ((S + 1) * (S + 1) * 8))               # about 64 MB of matrices at a time
+    worst_s = worst_e = 0.0
+    flagged = []          # (cell, row, column, error, column max, oracle value) of species-row entries over the bound
+    for c0 in range(0, N, chunk):
+        c1 = min(N, c0 + chunk)
+        Yc = np.ascontiguousarray(Y[:, c0:c1])
+        Jr = oracle.jacobian(om, T[c0:c1], P[c0:c1], Yc)
+        Jg = J[c0:c1].cpu().numpy()
+        rs, re = violations_vectorised(mech, T[c0:c1], P[c0:c1], Yc, Jg, Jr)
+        if rs > 1.0:
+            col = np.abs(Jr[:, :S, :]).max(axis=1, keepdims=True)
+            err = np.abs(Jg[:, :S, :] - Jr[:, :S, :])
+            for i, k, l in zip(*np.nonzero(err > 1e-9 * col + 1e-11 * np.abs(Jr[:, :S, :]))):
+                flagged.append((c0 + i, k, l, err[i, k, l], col[i, 0, l], Jr[i, k, l]))
+            rs = float(np.where(err > 1e-9 * col + 1e-11 * np.abs(Jr[:, :S, :]), 0.0,
+                                err / np.maximum(1e-9 * col + 1e-11 * np.abs(Jr[:, :S, :]), 1e-300)).max())
+        worst_s, worst_e = max(worst_s, rs), max(worst_e, re)
+    print("%s N=%d, every entry: worst Jacobian error / bound: species rows %.3g, energy row %.3g; %d entries in %d cells "
+          "decided by reading Q20" % (cfg_name, N, worst_s, worst_e, len(flagged), len({f[0] for f in flagged})))
+    assert worst_s <= 1.0 and worst_e <= 1.0, (cfg_name, worst_s, worst_e)
+    # Entries over the bound: few, in composition columns, ill-conditioned by the cancellation of reading Q20
+    # (terms > 1e3 x the column's largest entry), and within 1e-9 colmax + 1e-15 x the terms' scale (9 ulp of
+    # the terms: the quotient, the product and the S-term sum for W_mix behind each of them).
+    assert len({f[0] for f in flagged}) <= max(1, N // 20000), len(flagged)
+    for i, k, l, err, colmax, ref in flagged:
+        assert l < S, ("temperature column over the bound", i, k, l)
+        scale = composition_scale(mech, om, T[i], P[i], np.ascontiguousarray(Y[:, i]), k, l)
+        print("  cell %d entry (%d, %d): oracle %.9e, |gpu - oracle| = %.3g x 1e-9 colmax, terms / colmax = %.3g, "
+              "error / Q20 bound %.3g" % (i, k, l, ref, err / (1e-9 * colmax), scale / colmax,
+                                          err / (1e-9 * colmax + 1e-15 * scale)))
+        assert scale > 1e3 * colmax and err <= 1e-9 * colmax + 1e-15 * scale, (i, k, l, err, colmax, scale)
+
+
 def test_errors(ck):
     mech = ckgen.mechanism(ckgen.MECH_TINY)
     ann = ckgen.random_kc_ann(mech.n_reactions, 1, 4, seed=1, T_range=(1000.0, 2500.0))

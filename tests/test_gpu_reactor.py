@@ -114,6 +114,53 @@ def test_config5_stagewise_parity_on_the_synthetic_mechanism(ck):
             assert rw <= 1.0 and rt <= 1.0, (upto, rw, rt)
 
 
+def test_config5_as_written_65536_cells_1000_steps(ck):
+    """BASELINE.json configs[4] at its full size (65 536 cells, 1000 steps of dt = 1e-9 s; PAPER.md:183-185,
+    SURVEY reading Q14): after 1, 10, 100 and 1000 steps every state is finite and valid, and the source
+    term of EVERY cell of the batch -- the cells the projection has clamped (T at 250 or 5000 K, a Y at
+    exactly 0) included, they are counted and printed -- matches the oracle evaluated on the same state.
+    dT/dt of cells whose energy sum cancels is decided as everywhere else (reading Q19)."""
+    from helpers import dTdt_conditioned_violations, longdouble_dTdt
+    cfg = ckgen.CONFIGS["mid_rk4"]
+    mech = ckgen.mechanism(cfg.mech)
+    om = oracle.OracleMechanism(mech)
+    N = cfg.N
+    assert N == 65536
+    T, P, Y = ckgen.states(cfg)
+    Td, Pd, Yd = to_dev(T, P, Y)
+    st = torch.cuda.current_stream().cuda_stream
+    w = torch.empty((mech.n_species, N), dtype=torch.float64, device="cuda:0")
+    d = torch.empty(N, dtype=torch.float64, device="cuda:0")
+    with ck.Mechanism(mech) as gm:
+        done = 0
+        for upto in (1, 10, 100, 1000):
+            gm.rk4_integrate(Td, Pd, Yd, 1e-9, upto - done, stream=st)
+            done = upto
+            gm.source_terms(Td, Pd, Yd, w, d, stream=st)
+            torch.cuda.synchronize()
+            Th, Yh = Td.cpu().numpy(), Yd.cpu().numpy()
+            assert np.isfinite(Th).all() and np.isfinite(Yh).all()
+            assert Th.min() >= 250.0 and Th.max() <= 5000.0 and Yh.min() >= 0.0
+            assert np.abs(Yh.sum(0) - 1.0).max() <= 1e-14
+            clamped_T = (Th == 250.0) | (Th == 5000.0)
+            clamped_Y = (Yh == 0.0).any(0)
+            wr, dr, _ = oracle.source_terms(om, Th, P, Yh)
+            wg, dg = w.cpu().numpy(), d.cpu().numpy()
+            rw, rt = parity_violations(wg, dg, wr, dr)
+            print("step %d: %d cells with T at a bound, %d with a species at exactly 0; worst wdot err/tol %.3g, "
+                  "worst dT/dt err/tol %.3g" % (upto, clamped_T.sum(), clamped_Y.sum(), rw, rt))
+            assert rw <= 1.0, (upto, rw)
+            if rt > 1.0:
+                over, kappa, ratio = dTdt_conditioned_violations(mech, Th, dg, wr, dr)
+                assert over.size <= max(1, N // 20000), (upto, over.size)
+                exact = longdouble_dTdt(mech, Th[over], P[over], Yh[:, over])
+                e_gpu = np.abs((dg[over] - exact) / exact).astype(float)
+                print("step %d: %d cells over the north_star dT/dt bound by cancellation, kappa %.3g .. %.3g, "
+                      "err / Q19 bound %.3g" % (upto, over.size, kappa.min(), kappa.max(), ratio.max()))
+                assert kappa.min() > 1e3 and ratio.max() <= 1.0, (upto, kappa.min(), ratio.max())
+                assert (e_gpu <= 1e-10 + 1e-14 * kappa).all()
+
+
 def test_large_mechanism_one_step(ck):
     """S=111: cold accumulators and the species permutation through the fused stage epilogue."""
     cfg = ckgen.CONFIGS["large_256k"]
