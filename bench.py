@@ -131,6 +131,25 @@ def time_oracle(mech, T, P, Y, target_s=12.0):
                             "sample": "first %d cells, one pass, %.1f s, one thread" % (n1, dt1)}}
 
 
+def sample_parity(mech, T, P, Y, w, d, n=32768):
+    """The timed step's own results (device buffers w, d) against the oracle on the first n cells of the
+    workload, under the north_star tolerance; `q19_cells` counts the cells whose dT/dt alone is over the
+    bound (reading Q19: decided on the energy sum's scale by the tests, 0 on this workload).
+    Outside the timed region; part of the cpu_baseline leg (rank 0, N = 1)."""
+    import oracle
+    n = int(min(n, T.shape[0]))
+    wr, dr, _ = oracle.source_terms(oracle.OracleMechanism(mech), T[:n], P[:n], np.ascontiguousarray(Y[:, :n]))
+    wg, dg = w[:, :n].cpu().numpy(), d[:n].cpu().numpy()
+    tol_w = 1e-10 * np.abs(wr).max(axis=0, keepdims=True) + 1e-12 * np.abs(wr)
+    tol_t = 1e-10 * np.abs(dr) + 1e-12
+    rw = np.abs(wg - wr) / np.maximum(tol_w, 1e-300)
+    rt = np.abs(dg - dr) / tol_t
+    finite = bool(np.isfinite(wg).all() and np.isfinite(dg).all())
+    return {"cells": n, "finite": finite, "worst_wdot_err_over_tol": float(rw.max()),
+            "worst_dTdt_err_over_tol": float(rt.max()), "q19_cells": int((rt > 1.0).sum()),
+            "cells_over_wdot_tol": int((rw > 1.0).any(axis=0).sum())}
+
+
 def run_reference(args, cfg, mech):
     """--impl reference: the CPU oracle on the host cores, rank 0 only."""
     import ckgen
@@ -684,6 +703,7 @@ def main():
     }
     if world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = time_oracle(mech, T, P, Y)
+        out["parity"] = sample_parity(mech, T, P, Y, w, d)
     print(json.dumps(out))
     gm.close()
     if dist is not None:

@@ -72,6 +72,88 @@ def longdouble_dTdt(mech, T, P, Y):
     return dT
 
 
+def mp_source_terms(mech, T, P, Y, dps=40):
+    """One cell's (wdot[S], dT/dt) at `dps` decimal digits with mpmath, in the PRODUCT form of the paper's
+    equations and in the oracle's order of steps (PAPER.md:56 concentrations; Eq. 5 Arrhenius; Eq. 8 Kc;
+    PAPER.md:157-159 third bodies, Lindemann / Troe; Eq. 7 k_r = k_f / Kc; Eq. 3 mass action; Eq. 2; the
+    constant-pressure energy equation): the arbiter for cells where the fp64 oracle's own rounding is of the
+    size of the tolerance (reading Q19).  A third derivation, beside the fp64 C oracle and the
+    log-matrix numpy form below; it shares no code with either.  Returns mpmath numbers."""
+    from mpmath import mp, mpf, exp, log, log10
+    old = mp.dps
+    mp.dps = dps
+    try:
+        S, R = mech.n_species, mech.n_reactions
+        Ru = mpf(RU)
+        T, P = mpf(float(T)), mpf(float(P))
+        W = [mpf(float(x)) for x in mech.mol_weight]
+        Yk = [mpf(float(y)) if y > 0 else mpf(0) for y in Y]                      # reading Q9
+        inv_Wmix = sum(Yk[k] / W[k] for k in range(S))
+        rho = P / (Ru * T * inv_Wmix)
+        C = [max(rho * Yk[k] / W[k], mpf("1e-300")) for k in range(S)]
+        lnT = log(T)
+        cp_R, h_RT, g_RT = [], [], []
+        for k in range(S):
+            a = [mpf(float(x)) for x in (mech.nasa_lo[k] if float(T) <= mech.T_mid[k] else mech.nasa_hi[k])]
+            cp_R.append(a[0] + a[1] * T + a[2] * T**2 + a[3] * T**3 + a[4] * T**4)
+            h = a[0] + a[1] * T / 2 + a[2] * T**2 / 3 + a[3] * T**3 / 4 + a[4] * T**4 / 5 + a[5] / T
+            s_ = a[0] * lnT + a[1] * T + a[2] * T**2 / 2 + a[3] * T**3 / 3 + a[4] * T**4 / 4 + a[6]
+            h_RT.append(h)
+            g_RT.append(h - s_)
+        arrh = lambda lnA, b, EaR: exp(mpf(float(lnA))) * T**mpf(float(b)) * exp(-mpf(float(EaR)) / T)
+        wdot = [mpf(0)] * S
+        for j in range(R):
+            kf = arrh(mech.ln_A[j], mech.b[j], mech.Ea_over_R[j])
+            reac = [(k, mpf(float(mech.nu_reac[k, j]))) for k in np.flatnonzero(mech.nu_reac[:, j])]
+            prod = [(k, mpf(float(mech.nu_prod[k, j]))) for k in np.flatnonzero(mech.nu_prod[:, j])]
+            dnu_sum = sum(n for _, n in prod) - sum(n for _, n in reac)
+            dG = sum(n * g_RT[k] for k, n in prod) - sum(n * g_RT[k] for k, n in reac)
+            Kc = exp(-dG) * (mpf(float(mech.p_ref)) / (Ru * T))**dnu_sum
+            typ = int(mech.rxn_type[j])
+            phi = mpf(1)
+            if typ != 0:
+                M = sum(mpf(float(mech.eff[k, j])) * C[k] for k in range(S))
+                if typ == 1:
+                    phi = M
+                else:
+                    k0 = arrh(mech.ln_A0[j], mech.b0[j], mech.Ea0_over_R[j])
+                    Pr = k0 * M / kf
+                    F = mpf(1)
+                    if typ == 3:
+                        al, T3, T1, T2 = (float(x) for x in mech.troe[j])
+                        Fc = (1 - mpf(al)) * exp(-T / mpf(T3)) + mpf(al) * exp(-T / mpf(T1))
+                        if np.isfinite(T2):
+                            Fc += exp(-mpf(T2) / T)
+                        lFc = log10(Fc)
+                        c = mpf("-0.4") - mpf("0.67") * lFc
+                        n = mpf("0.75") - mpf("1.27") * lFc
+                        lPr = log10(max(Pr, mpf("1e-300")))
+                        f1 = (lPr + c) / (n - mpf("0.14") * (lPr + c))
+                        F = mpf(10)**(lFc / (1 + f1 * f1))
+                    kf = kf * (Pr / (1 + Pr)) * F
+            kr = kf / Kc if mech.reversible[j] else mpf(0)
+            qf, qr = kf, kr
+            for k, n in reac:
+                qf *= C[k]**n
+            for k, n in prod:
+                qr *= C[k]**n
+            Q = phi * (qf - qr)
+            for k, n in prod:
+                wdot[k] += n * Q
+            for k, n in reac:
+                wdot[k] -= n * Q
+        cp = sum(Yk[k] * cp_R[k] * Ru / W[k] for k in range(S))
+        hw = sum(h_RT[k] * Ru * T * wdot[k] for k in range(S))
+        return wdot, -hw / (rho * cp)
+    finally:
+        mp.dps = old
+
+
+def mp_dTdt(mech, T, P, Y, dps=40):
+    """dT/dt of the cells T[n], P[n], Y[S, n] from mp_source_terms, rounded to float64."""
+    return np.array([float(mp_source_terms(mech, T[i], P[i], Y[:, i], dps)[1]) for i in range(len(T))])
+
+
 def energy_condition_number(mech, T, wdot_ref, h_RT):
     """kappa = sum|h_k wdot_k| / |sum h_k wdot_k| per cell."""
     hw = h_RT * RU * T[None, :] * wdot_ref

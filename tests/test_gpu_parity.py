@@ -9,7 +9,7 @@ import pytest
 
 import ckgen
 import oracle
-from helpers import RU, dTdt_conditioned_violations, longdouble_dTdt, parity_violations
+from helpers import RU, dTdt_conditioned_violations, mp_dTdt, parity_violations
 
 pytestmark = pytest.mark.gpu
 
@@ -178,17 +178,17 @@ def full_batch_parity(ck, mech, T, P, Y, label, variants=("auto", "generic"), ho
                 if rt > 1.0:
                     # Cells over the north_star bound on dT/dt ALONE: the energy sum cancels there
                     # (reading Q19).  They must be few, ill-conditioned (kappa > 1e3), inside
-                    # the bound taken on the sum's own scale, and no farther from a long-double
-                    # evaluation than that bound allows (the fp64 oracle is itself off by ~1e-15 kappa).
+                    # the bound taken on the sum's own scale, and no farther from a 40-digit
+                    # evaluation in the oracle's product form (helpers.mp_dTdt) than that bound allows (the fp64 oracle is itself off by ~1e-15 kappa).
                     over, kappa, ratio = dTdt_conditioned_violations(mech, T, dg, wr, dr)
                     # (few first: that also bounds the work of the long-double arbiter, which then takes
                     #  EVERY such cell, not a sample of them)
                     assert over.size <= max(1, N // 20000), (label, variant, what, over.size)
-                    exact = longdouble_dTdt(mech, T[over], P[over], Y[:, over])
+                    exact = mp_dTdt(mech, T[over], P[over], Y[:, over])      # 40 digits, the oracle's product form
                     e_gpu = np.abs((dg[over] - exact) / exact).astype(float)
                     e_orc = np.abs((dr[over] - exact) / exact).astype(float)
                     print("%s [%s, %s]: %d of %d cells over the north_star dT/dt bound, all by cancellation: "
-                          "kappa %.3g .. %.3g, worst err / Q19 bound %.3g; against long double: GPU rel err "
+                          "kappa %.3g .. %.3g, worst err / Q19 bound %.3g; against a 40-digit evaluation: GPU rel err "
                           "%.3g, fp64 oracle rel err %.3g (worst of all %d)"
                           % (label, variant, what, over.size, N, kappa.min(), kappa.max(), ratio.max(),
                              e_gpu.max(), e_orc.max(), e_gpu.size))

@@ -120,7 +120,7 @@ def test_config5_as_written_65536_cells_1000_steps(ck):
     term of EVERY cell of the batch -- the cells the projection has clamped (T at 250 or 5000 K, a Y at
     exactly 0) included, they are counted and printed -- matches the oracle evaluated on the same state.
     dT/dt of cells whose energy sum cancels is decided as everywhere else (reading Q19)."""
-    from helpers import dTdt_conditioned_violations, longdouble_dTdt
+    from helpers import dTdt_conditioned_violations, mp_dTdt
     cfg = ckgen.CONFIGS["mid_rk4"]
     mech = ckgen.mechanism(cfg.mech)
     om = oracle.OracleMechanism(mech)
@@ -153,7 +153,7 @@ def test_config5_as_written_65536_cells_1000_steps(ck):
             if rt > 1.0:
                 over, kappa, ratio = dTdt_conditioned_violations(mech, Th, dg, wr, dr)
                 assert over.size <= max(1, N // 20000), (upto, over.size)
-                exact = longdouble_dTdt(mech, Th[over], P[over], Yh[:, over])
+                exact = mp_dTdt(mech, Th[over], P[over], Yh[:, over])      # 40 digits, the oracle's product form
                 e_gpu = np.abs((dg[over] - exact) / exact).astype(float)
                 print("step %d: %d cells over the north_star dT/dt bound by cancellation, kappa %.3g .. %.3g, "
                       "err / Q19 bound %.3g" % (upto, over.size, kappa.min(), kappa.max(), ratio.max()))

@@ -8,7 +8,7 @@ import pytest
 
 import ckgen
 import oracle
-from helpers import RU, paper_matrix_form
+from helpers import RU, paper_matrix_form, parity_violations
 
 SPECS = [ckgen.MECH_TINY, ckgen.MECH_MID]
 CFG_OF = {"S9_R21": "tiny_1k", "S53_R325": "mid_1m", "S111_R784": "large_256k"}
@@ -212,3 +212,46 @@ def test_non_positive_mass_fractions_are_absent_species():
     wn, dn, _ = oracle.source_terms(om, T, P, Yn)
     assert np.array_equal(w0, wn) and np.array_equal(d0, dn)
     assert np.isfinite(w0).all() and np.isfinite(d0).all()
+
+
+# ---------------------------------------------------------------------------------------------
+# The 40-digit arbiter of DESIGN.md reading Q19 (helpers.mp_source_terms: mpmath, the paper's product
+# form in the oracle's order of steps, no code shared with the oracle or with the log-matrix form).
+
+@pytest.mark.parametrize("cfg_name,n", [("tiny_1k", 6), ("mid_1m", 3), ("large_256k", 1)])
+def test_oracle_against_the_40_digit_product_form(cfg_name, n):
+    """On ordinary cells the fp64 oracle is within 1 % of the north_star tolerance of the 40-digit value
+    (every reaction type of the generated mechanisms is in these: third bodies, Troe falloff)."""
+    from helpers import mp_source_terms
+    cfg = ckgen.CONFIGS[cfg_name]
+    mech = ckgen.mechanism(cfg.mech)
+    T, P, Y = ckgen.states(cfg, N=n)
+    wr, dr, _ = oracle.source_terms(oracle.OracleMechanism(mech), T, P, Y)
+    for i in range(n):
+        w, d = mp_source_terms(mech, T[i], P[i], Y[:, i])
+        w = np.array([float(x) for x in w])
+        rw, rt = parity_violations(wr[:, i:i + 1], dr[i:i + 1], w[:, None], np.array([float(d)]))
+        assert rw <= 1e-2 and rt <= 1e-2, (cfg_name, i, rw, rt)
+
+
+def test_reading_q19_the_fp64_oracle_itself_breaks_the_dTdt_bound_where_the_energy_sum_cancels():
+    """Cell 96243 of config 4 (S=111/R=784, 2^18 cells) has the most cancelling energy sum of the batch,
+    kappa = sum|h_k wdot_k| / |sum h_k wdot_k| = 7.4e4.  There the fp64 oracle is 1.6e-10 (relative) away
+    from the 40-digit value of dT/dt: more than the north_star's 1e-10, which is why a cell like this one is
+    decided on the sum's own scale, (1e-10 + 1e-14 kappa) |dT/dt| -- and the oracle is well inside that.
+    Its wdot, which does not cancel, is within 1 % of the tolerance."""
+    from helpers import energy_kappa, mp_source_terms
+    cfg = ckgen.CONFIGS["large_256k"]
+    mech = ckgen.mechanism(cfg.mech)
+    T, P, Y = ckgen.states(cfg)
+    i = 96243
+    Tc, Pc, Yc = T[i:i + 1], P[i:i + 1], np.ascontiguousarray(Y[:, i:i + 1])
+    wr, dr, _ = oracle.source_terms(oracle.OracleMechanism(mech), Tc, Pc, Yc)
+    kappa = float(energy_kappa(mech, Tc, wr)[0])
+    assert 7e4 < kappa < 8e4
+    w, d = mp_source_terms(mech, Tc[0], Pc[0], Yc[:, 0])
+    rel = abs(dr[0] - float(d)) / abs(float(d))
+    assert 1e-10 < rel < 0.5 * (1e-10 + 1e-14 * kappa), rel
+    w = np.array([float(x) for x in w])
+    rw, _ = parity_violations(wr, dr, w[:, None], dr)
+    assert rw <= 1e-2
